@@ -1,0 +1,160 @@
+/*
+ * qmc.h -- C ABI of the B200-native batched Slater-Jastrow electron-move engine.
+ *
+ * The library implements, in hand-written CUDA for sm_100a, the hot path behind the double-precision
+ * DMC runs of arXiv 2504.07948: the walker-batched particle-by-particle electron move for a
+ * Slater-Jastrow trial function in a contracted-Gaussian (LCAO) basis.
+ *
+ *   Psi_T = exp[J] D_up D_dn,  phi_j = sum_l C_lj Phi_l            PAPER.md L125-127 (eq. 2), M = 1
+ *   A_pj = phi_j(r_p) and its inverse
+ *   d ln D / d lambda = tr(A^-1 dA/d lambda)                       PAPER.md L173 (eq. 3)
+ *   walker-level batching of all of the above
+ *   fixed-node rejection
+ * Everything the paper leaves open (basis functional form, Pade Jastrow, drift-diffusion proposal,
+ * Philox stream, delayed rank-k update, local energy) follows BASELINE.json `north_star`/`configs`
+ * with the readings listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - Units: bohr and hartree.  All floating point is IEEE FP64.
+ *   - Electrons 0..n_up-1 are spin-up, n_up..n_up+n_dn-1 spin-down.  One "step" of qmc_sweep is one
+ *     sweep: one proposed move for every electron, ups first, index ascending, all walkers in lockstep.
+ *   - Every function returns QMC_OK (0) or a negative error code; nothing throws, aborts or prints.
+ *     qmc_last_error() gives a thread-local message for the last failing call.
+ *   - Pointer arguments marked "host or device" may be either (unified virtual addressing decides);
+ *     inputs are copied before the call returns, so the caller may free them afterwards.
+ *   - Output buffers are caller-owned (normally torch tensors).  Device buffers are written
+ *     asynchronously on the walker set's stream; host buffers are written synchronously.
+ *   - The library owns its internal state (cudaMalloc at create time, freed at destroy).
+ *   - There is NO CPU fallback: every entry point fails with QMC_ERR_CUDA when no sm_100 device works.
+ */
+#ifndef QMC_B200_H
+#define QMC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QMC_OK 0
+#define QMC_ERR_ARG (-1)      /* null pointer, inconsistent sizes, l > 2, delay_k < 1, tau <= 0, ... */
+#define QMC_ERR_CUDA (-2)     /* a CUDA call failed (message in qmc_last_error) */
+#define QMC_ERR_SINGULAR (-3) /* zero pivot while inverting a Slater matrix at walker creation */
+#define QMC_ERR_NOMEM (-4)
+#define QMC_ERR_STATE (-5)    /* call not valid in the current state (e.g. log requested but not enabled) */
+
+/* flags of qmc_walkers_create */
+#define QMC_LOG_RATIOS 1u /* also record rho_D*exp(dJ) and p_acc of every proposed move */
+
+typedef struct qmc_system qmc_system;   /* immutable after qmc_init: atoms, basis, MO coefficients, Jastrow (device) */
+typedef struct qmc_walkers qmc_walkers; /* mutable crowd state */
+
+typedef struct {
+    int n_atoms;
+    const double* xyz; /* [n_atoms][3], host or device */
+    const double* Z;   /* [n_atoms] charge used by the e-n Jastrow and the bare Coulomb potential */
+} qmc_atoms;
+
+/* Contracted Gaussian shells, Phi = S_lm(x) * sum_p coef_p exp(-alpha_p |x|^2), x = r - R_atom.
+ * l = 0: {1};  l = 1: {x, y, z};
+ * l = 2: {sqrt3 xy, sqrt3 yz, z^2 - (x^2+y^2)/2, sqrt3 xz, (sqrt3/2)(x^2-y^2)}  (5 components, reading A1).
+ * Basis-function order: shells in input order, functions of a shell in the order above.
+ * coef already contains all normalisation (the library never normalises); alpha = 0 is legal. */
+typedef struct {
+    int n_shells;
+    const int* atom;        /* [n_shells] index into qmc_atoms */
+    const int* l;           /* [n_shells] 0, 1 or 2 */
+    const int* n_prim;      /* [n_shells] >= 1 */
+    const int* prim_offset; /* [n_shells] offset into alpha / coef */
+    int n_prim_total;
+    const double* alpha; /* [n_prim_total] */
+    const double* coef;  /* [n_prim_total] */
+} qmc_basis;
+
+typedef struct {
+    int n_basis; /* must equal sum over shells of 2l+1 */
+    int n_up, n_dn;
+    const double* C_up; /* [n_basis][n_up] row-major: C_up[l][j] = coefficient of Phi_l in orbital j */
+    const double* C_dn; /* [n_basis][n_dn]; may be NULL when n_dn == 0 */
+} qmc_mo;
+
+/* u_ee(r) = a r / (1 + b_ee r), a = a_anti (opposite spins) or a_para (same spin);
+ * u_en(r) = -Z_I r / (1 + b_en r);  Psi ~ exp(+J). */
+typedef struct {
+    double a_anti, a_para, b_ee, b_en;
+} qmc_jastrow;
+
+/* Build the immutable system on the current CUDA device.  `cuda_stream` is a cudaStream_t (may be 0). */
+int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basis* basis, const qmc_mo* mo,
+             const qmc_jastrow* jastrow, void* cuda_stream);
+void qmc_finalize(qmc_system* sys);
+
+/* Create a crowd of n_walkers walkers at `positions` ([n_walkers][n_elec][3], ups first, host or device).
+ * Evaluates all orbital rows, inverts the Slater matrices (Gauss-Jordan with partial pivoting on the
+ * device), and sets log|Psi|, sign and E_L.  RNG streams are keyed (seed; first_walker_id + w, step,
+ * electron) with the step counter starting at first_step, so any crowd is a slice of one infinite
+ * crowd (reading A20) and sweeps can be resumed bit for bit.  Returns QMC_ERR_SINGULAR if any Slater
+ * matrix has a zero pivot.  All later work is enqueued on `cuda_stream`. */
+int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int n_walkers, const double* positions,
+                       uint64_t seed, uint32_t first_walker_id, uint32_t first_step, uint32_t flags,
+                       void* cuda_stream);
+void qmc_walkers_destroy(qmc_walkers* w);
+
+/* Run nsteps sweeps with time step tau (> 0) and delay rank delay_k (1 <= delay_k <= 128).
+ * Per electron i, for all walkers (BASELINE.json north_star items 1-6):
+ *   drift G = grad_i ln|Psi|; r' = r + tau G + sqrt(tau) chi (Philox4x32-10 -> Box-Muller);
+ *   basis functions and orbital rows at r' (FP64 contraction C^T Phi); rho_D from the effective
+ *   inverse column; Pade Jastrow ratio; accept iff u < rho_D^2 exp(2 dJ + Delta) and rho_D > 0;
+ *   accepted rows enter a delay window that is flushed into A^-1 every delay_k proposals and at the
+ *   end of each spin block as FP64 GEMMs.  E_L = K + V is evaluated at the end of every sweep.
+ * delay_k changes performance only; results differ from delay_k = 1 by rounding.
+ * Asynchronous on the walker set's stream.  The accept log of this call replaces the previous one. */
+int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k);
+
+/* Getters.  `out` may be host or device memory. */
+int qmc_get_positions(const qmc_walkers* w, double* out /* [W][n_elec][3] */);
+/* out[w][p][j] = (A^-1)[j][p] of spin (0 up, 1 down): row p is the vector dotted with a new orbital row (A18) */
+int qmc_get_Ainv(const qmc_walkers* w, int spin, double* out /* [W][n_s][n_s] */);
+int qmc_get_logpsi(const qmc_walkers* w, double* logabs /* [W] */, int8_t* sign /* [W], may be NULL */);
+int qmc_get_eloc(const qmc_walkers* w, double* eloc /* [W], K+V */, double* ekin /* [W], may be NULL */);
+/* log of the most recent qmc_sweep call: bits[t][i][w], bit0 = accepted, bit1 = tie-flagged
+ * (|u - p_acc| < 1e-12 or |rho_D| < 1e-12), bit2 = non-finite value seen (move rejected). */
+int qmc_get_accept_log(const qmc_walkers* w, uint8_t* bits /* [T][n_elec][W] */);
+/* needs QMC_LOG_RATIOS: ratio = rho_D * exp(dJ), pacc = p_acc (0 when rejected at the node) */
+int qmc_get_ratio_log(const qmc_walkers* w, double* ratio /* [T][n_elec][W] */, double* pacc /* may be NULL */);
+/* totals since creation */
+int qmc_get_stats(const qmc_walkers* w, uint64_t* n_proposed, uint64_t* n_accepted, uint64_t* n_ties,
+                  uint64_t* n_nonfinite);
+int qmc_synchronize(const qmc_walkers* w);
+
+/* Stage-level entry points (used by the per-stage parity tests and the per-stage roofline bench).
+ * Basis functions at n_points positions: out[n][5][n_basis] = value, d/dx, d/dy, d/dz, laplacian. */
+int qmc_eval_basis(const qmc_system* sys, int n_points, const double* xyz /* [n][3] */, double* out, void* cuda_stream);
+/* Orbital rows at n_points positions: out[n][5][n_s] (basis kernel + FP64 contraction kernel). */
+int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream);
+/* Time `reps` launches of one stage of the move on the walker set's current state with CUDA events on its
+ * stream (no state is committed).  stage: 0 = propose (drift + RNG + Jastrow), 1 = basis, 2 = MO contraction,
+ * 3 = ratio/accept (decision suppressed), 4 = delayed-update flush at full window (A^-1 unchanged: zero
+ * correction), 5 = local energy.  Returns mean milliseconds per launch. */
+int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, double* ms_per_launch);
+/* In-situ stage timing: with stride > 0, qmc_sweep brackets the four per-electron stages of every
+ * stride-th electron, every flush and every local-energy evaluation with CUDA events on the walker set's
+ * stream.  qmc_get_stage_times synchronises and returns accumulated milliseconds and launch counts per
+ * stage id (same ids as qmc_time_stage; a "launch" of stage 4 is the whole flush = 4 kernels, of stage 5
+ * two kernels).  stride = 0 turns it off and clears the totals. */
+int qmc_set_profiling(qmc_walkers* w, int stride);
+int qmc_get_stage_times(qmc_walkers* w, double* ms /* [6] */, uint64_t* counts /* [6] */);
+/* Register-resident DMMA issue-rate loop for `ms_target` milliseconds: the FP64 ceiling of this GPU as
+ * it runs now (used as the roofline denominator of the contraction stages). */
+int qmc_measure_fp64_peak(double ms_target, double* tflops, void* cuda_stream);
+/* number of kernels this library launched on this thread's calls since load (for bench.py gpu_launches) */
+uint64_t qmc_launch_count(void);
+
+const char* qmc_last_error(void);
+const char* qmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_B200_H */

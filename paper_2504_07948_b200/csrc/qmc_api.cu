@@ -1,0 +1,673 @@
+// qmc_api.cu -- the C ABI of include/qmc.h: argument checking, device memory, and the host-side
+// scheduler that enqueues the per-electron kernels of a sweep (no host synchronisation inside a sweep).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/qmc.h"
+#include "qmc_kernels.cuh"
+
+using namespace qmc;
+
+static thread_local std::string g_err;
+
+static int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+#define CU(call)                                                                                            \
+    do {                                                                                                    \
+        cudaError_t _e = (call);                                                                            \
+        if (_e != cudaSuccess) {                                                                            \
+            cudaGetLastError();                                                                             \
+            return fail(_e == cudaErrorMemoryAllocation ? QMC_ERR_NOMEM : QMC_ERR_CUDA,                     \
+                        std::string(#call) + ": " + cudaGetErrorString(_e) + " (" __FILE__ ":" + std::to_string(__LINE__) + ")"); \
+        }                                                                                                   \
+    } while (0)
+
+static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+struct DevPool {  // owns cudaMalloc'ed blocks
+    std::vector<void*> blocks;
+    cudaError_t alloc(void** p, size_t bytes, cudaStream_t st, bool zero = true) {
+        *p = nullptr;
+        if (bytes == 0) bytes = 16;
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) return e;
+        blocks.push_back(*p);
+        if (zero) e = cudaMemsetAsync(*p, 0, bytes, st);
+        return e;
+    }
+    void release(void* p) {
+        for (auto& b : blocks)
+            if (b == p) { cudaFree(b); b = nullptr; }
+    }
+    void free_all() {
+        for (void* b : blocks)
+            if (b) cudaFree(b);
+        blocks.clear();
+    }
+};
+
+struct qmc_system {
+    SysDev d;
+    DevPool pool;
+    cudaStream_t stream;
+    int device;
+};
+
+struct StageTimer {
+    std::vector<cudaEvent_t> ev;  // pairs
+    std::vector<int> stage;
+    size_t used = 0;
+};
+
+struct qmc_walkers {
+    const qmc_system* sys;
+    WalkDev d;
+    DevPool pool;
+    DevPool winpool;
+    DevPool logpool;
+    cudaStream_t stream;
+    uint32_t step;       // global sweep counter (A12)
+    uint32_t flags;
+    int T_last;          // sweeps in the most recent qmc_sweep call
+    int* d_status;
+    int prof_stride;     // 0 = off
+    StageTimer timer;
+    double stage_ms[8];
+    uint64_t stage_n[8];
+};
+
+extern "C" const char* qmc_last_error(void) { return g_err.c_str(); }
+extern "C" const char* qmc_version(void) { return "paper_2504_07948_b200 r1 (sm_100a, FP64 DMMA)"; }
+extern "C" uint64_t qmc_launch_count(void) { return launch_count(); }
+
+static int check_device() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(QMC_ERR_CUDA, std::string("no CUDA device: ") + cudaGetErrorString(e)); }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(QMC_ERR_CUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e)); }
+    if (prop.major != 10) return fail(QMC_ERR_CUDA, "this library is built for sm_100a only (found sm_" + std::to_string(prop.major) + std::to_string(prop.minor) + "); there is no fallback path");
+    return QMC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ qmc_init
+
+template <class T>
+static cudaError_t fetch(std::vector<T>& dst, const T* src, size_t n) {
+    dst.resize(n);
+    if (n == 0) return cudaSuccess;
+    return cudaMemcpy(dst.data(), src, n * sizeof(T), cudaMemcpyDefault);
+}
+
+extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basis* basis, const qmc_mo* mo,
+                        const qmc_jastrow* jas, void* cuda_stream) {
+    if (!out || !atoms || !basis || !mo || !jas) return fail(QMC_ERR_ARG, "qmc_init: null argument");
+    *out = nullptr;
+    if (atoms->n_atoms < 1 || !atoms->xyz || !atoms->Z) return fail(QMC_ERR_ARG, "qmc_init: atoms");
+    if (basis->n_shells < 1 || !basis->atom || !basis->l || !basis->n_prim || !basis->prim_offset || !basis->alpha || !basis->coef || basis->n_prim_total < 1)
+        return fail(QMC_ERR_ARG, "qmc_init: basis");
+    if (mo->n_basis < 1 || mo->n_up < 0 || mo->n_dn < 0 || mo->n_up + mo->n_dn < 1 || (mo->n_up > 0 && !mo->C_up) || (mo->n_dn > 0 && !mo->C_dn))
+        return fail(QMC_ERR_ARG, "qmc_init: mo");
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    std::vector<double> xyz, Z, alpha, coef;
+    std::vector<int> sh_atom, sh_l, sh_np, sh_off;
+    CU(fetch(xyz, atoms->xyz, (size_t)3 * atoms->n_atoms));
+    CU(fetch(Z, atoms->Z, (size_t)atoms->n_atoms));
+    CU(fetch(sh_atom, basis->atom, (size_t)basis->n_shells));
+    CU(fetch(sh_l, basis->l, (size_t)basis->n_shells));
+    CU(fetch(sh_np, basis->n_prim, (size_t)basis->n_shells));
+    CU(fetch(sh_off, basis->prim_offset, (size_t)basis->n_shells));
+    CU(fetch(alpha, basis->alpha, (size_t)basis->n_prim_total));
+    CU(fetch(coef, basis->coef, (size_t)basis->n_prim_total));
+
+    std::vector<ShellRec> recs(basis->n_shells);
+    int f = 0;
+    for (int i = 0; i < basis->n_shells; i++) {
+        if (sh_l[i] < 0 || sh_l[i] > 2) return fail(QMC_ERR_ARG, "qmc_init: shell angular momentum must be 0, 1 or 2");
+        if (sh_atom[i] < 0 || sh_atom[i] >= atoms->n_atoms) return fail(QMC_ERR_ARG, "qmc_init: shell atom index out of range");
+        if (sh_np[i] < 1 || sh_off[i] < 0 || sh_off[i] + sh_np[i] > basis->n_prim_total) return fail(QMC_ERR_ARG, "qmc_init: primitive range out of bounds");
+        recs[i].x = xyz[3 * sh_atom[i]]; recs[i].y = xyz[3 * sh_atom[i] + 1]; recs[i].z = xyz[3 * sh_atom[i] + 2];
+        recs[i].l = sh_l[i]; recs[i].f0 = f; recs[i].nprim = sh_np[i]; recs[i].poff = sh_off[i];
+        f += 2 * sh_l[i] + 1;
+    }
+    if (f != mo->n_basis) return fail(QMC_ERR_ARG, "qmc_init: n_basis != sum over shells of 2l+1");
+
+    qmc_system* S = new qmc_system();
+    S->stream = st;
+    cudaGetDevice(&S->device);
+    SysDev& d = S->d;
+    memset(&d, 0, sizeof(d));
+    d.n_atoms = atoms->n_atoms; d.n_shells = basis->n_shells; d.n_basis = mo->n_basis; d.nbp = round_up(mo->n_basis, 16);
+    d.ns[0] = mo->n_up; d.ns[1] = mo->n_dn; d.nsp[0] = round_up(mo->n_up, 16); d.nsp[1] = round_up(mo->n_dn, 16);
+    d.ne = mo->n_up + mo->n_dn;
+    d.a_anti = jas->a_anti; d.a_para = jas->a_para; d.b_ee = jas->b_ee; d.b_en = jas->b_en;
+    auto cleanup = [&](int code, const std::string& m) { S->pool.free_all(); delete S; return fail(code, m); };
+#define CUS(call)                                                                                       \
+    do {                                                                                                \
+        cudaError_t _e = (call);                                                                        \
+        if (_e != cudaSuccess) { cudaGetLastError(); return cleanup(_e == cudaErrorMemoryAllocation ? QMC_ERR_NOMEM : QMC_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e)); } \
+    } while (0)
+    double *dxyz, *dZ, *dal, *dco, *denn;
+    ShellRec* drec;
+    CUS(S->pool.alloc((void**)&dxyz, xyz.size() * 8, st));
+    CUS(S->pool.alloc((void**)&dZ, Z.size() * 8, st));
+    CUS(S->pool.alloc((void**)&dal, alpha.size() * 8, st));
+    CUS(S->pool.alloc((void**)&dco, coef.size() * 8, st));
+    CUS(S->pool.alloc((void**)&drec, recs.size() * sizeof(ShellRec), st));
+    CUS(S->pool.alloc((void**)&denn, 8, st));
+    CUS(cudaMemcpyAsync(dxyz, xyz.data(), xyz.size() * 8, cudaMemcpyHostToDevice, st));
+    CUS(cudaMemcpyAsync(dZ, Z.data(), Z.size() * 8, cudaMemcpyHostToDevice, st));
+    CUS(cudaMemcpyAsync(dal, alpha.data(), alpha.size() * 8, cudaMemcpyHostToDevice, st));
+    CUS(cudaMemcpyAsync(dco, coef.data(), coef.size() * 8, cudaMemcpyHostToDevice, st));
+    CUS(cudaMemcpyAsync(drec, recs.data(), recs.size() * sizeof(ShellRec), cudaMemcpyHostToDevice, st));
+    d.atom_xyz = dxyz; d.atom_Z = dZ; d.alpha = dal; d.coef = dco; d.shells = drec;
+    for (int sp = 0; sp < 2; sp++) {
+        double* dC;
+        CUS(S->pool.alloc((void**)&dC, (size_t)d.nbp * d.nsp[sp] * 8, st));
+        d.C[sp] = dC;
+        const double* src = sp == 0 ? mo->C_up : mo->C_dn;
+        if (d.ns[sp] > 0) {
+            double* tmp;  // stage (host or device source) -> device, then pad on the device
+            size_t bytes = (size_t)d.n_basis * d.ns[sp] * 8;
+            CUS(cudaMalloc((void**)&tmp, bytes));
+            cudaError_t e = cudaMemcpyAsync(tmp, src, bytes, cudaMemcpyDefault, st);
+            if (e == cudaSuccess) e = launch_pad_C(tmp, d.n_basis, d.ns[sp], dC, d.nsp[sp], st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            cudaFree(tmp);
+            CUS(e);
+        }
+    }
+    CUS(launch_enn(d, denn, st));
+    CUS(cudaMemcpyAsync(&d.e_nn, denn, 8, cudaMemcpyDeviceToHost, st));
+    CUS(cudaStreamSynchronize(st));
+    *out = S;
+    return QMC_OK;
+}
+
+extern "C" void qmc_finalize(qmc_system* sys) {
+    if (!sys) return;
+    sys->pool.free_all();
+    delete sys;
+}
+
+// ------------------------------------------------------------------------------------------------ walkers
+
+static int alloc_window(qmc_walkers* w, int kp) {
+    WalkDev& d = w->d;
+    const SysDev& s = w->sys->d;
+    cudaStream_t st = w->stream;
+    CU(cudaStreamSynchronize(st));
+    w->winpool.free_all();
+    const int nspm = d.ldv;
+    d.kp = kp;
+    CU(w->winpool.alloc((void**)&d.Vbuf, (size_t)d.W * kp * nspm * 8, st));
+    CU(w->winpool.alloc((void**)&d.Wbuf, (size_t)d.W * kp * nspm * 8, st));
+    CU(w->winpool.alloc((void**)&d.W2, (size_t)d.W * kp * nspm * 8, st));
+    CU(w->winpool.alloc((void**)&d.SinvT, (size_t)d.W * kp * kp * 8, st));
+    CU(w->winpool.alloc((void**)&d.YT, (size_t)d.W * nspm * kp * 8, st));
+    CU(w->winpool.alloc((void**)&d.bvec, (size_t)d.W * kp * 8, st));
+    CU(w->winpool.alloc((void**)&d.cvec, (size_t)d.W * kp * 8, st));
+    CU(w->winpool.alloc((void**)&d.plist, (size_t)d.W * kp * 4, st));
+    (void)s;
+    return QMC_OK;
+}
+
+static void destroy_walkers(qmc_walkers* w) {
+    if (!w) return;
+    cudaStreamSynchronize(w->stream);
+    for (cudaEvent_t e : w->timer.ev) cudaEventDestroy(e);
+    w->pool.free_all();
+    w->winpool.free_all();
+    w->logpool.free_all();
+    delete w;
+}
+
+extern "C" void qmc_walkers_destroy(qmc_walkers* w) { destroy_walkers(w); }
+
+extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int n_walkers, const double* positions,
+                                  uint64_t seed, uint32_t first_walker_id, uint32_t first_step, uint32_t flags,
+                                  void* cuda_stream) {
+    if (!sys || !out || !positions) return fail(QMC_ERR_ARG, "qmc_walkers_create: null argument");
+    *out = nullptr;
+    if (n_walkers < 1) return fail(QMC_ERR_ARG, "qmc_walkers_create: n_walkers < 1");
+    int rc = check_device();
+    if (rc) return rc;
+    const SysDev& s = sys->d;
+    qmc_walkers* w = new qmc_walkers();
+    w->sys = sys;
+    w->stream = (cudaStream_t)cuda_stream;
+    w->step = first_step;
+    w->flags = flags;
+    w->T_last = 0;
+    w->prof_stride = 0;
+    memset(w->stage_ms, 0, sizeof(w->stage_ms));
+    memset(w->stage_n, 0, sizeof(w->stage_n));
+    cudaStream_t st = w->stream;
+    WalkDev& d = w->d;
+    memset(&d, 0, sizeof(d));
+    d.W = n_walkers; d.ne = s.ne; d.nep = round_up(s.ne, 8);
+    d.ldv = s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1];
+    d.seed = seed; d.first_walker = first_walker_id;
+    const size_t W = n_walkers;
+#define CUW(call)                                                                                      \
+    do {                                                                                               \
+        cudaError_t _e = (call);                                                                       \
+        if (_e != cudaSuccess) {                                                                       \
+            cudaGetLastError();                                                                        \
+            std::string m = std::string(#call) + ": " + cudaGetErrorString(_e);                        \
+            destroy_walkers(w);                                                                        \
+            return fail(_e == cudaErrorMemoryAllocation ? QMC_ERR_NOMEM : QMC_ERR_CUDA, m);            \
+        }                                                                                              \
+    } while (0)
+    CUW(w->pool.alloc((void**)&d.R, W * 3 * d.nep * 8, st));
+    for (int sp = 0; sp < 2; sp++) {
+        CUW(w->pool.alloc((void**)&d.AinvT[sp], W * s.nsp[sp] * s.nsp[sp] * 8, st));
+        CUW(w->pool.alloc((void**)&d.Orb[sp], W * s.nsp[sp] * 5 * s.nsp[sp] * 8, st));
+    }
+    CUW(w->pool.alloc((void**)&d.Phi, W * 5 * s.nbp * 8, st));
+    CUW(w->pool.alloc((void**)&d.V, W * 5 * d.ldv * 8, st));
+    CUW(w->pool.alloc((void**)&d.xcol, W * d.ldv * 8, st));
+    CUW(w->pool.alloc((void**)&d.mcount, W * 4, st));
+    CUW(w->pool.alloc((void**)&d.rp, W * 3 * 8, st));
+    CUW(w->pool.alloc((void**)&d.G, W * 3 * 8, st));
+    CUW(w->pool.alloc((void**)&d.u, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.dJ, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.gJn, W * 3 * 8, st));
+    CUW(w->pool.alloc((void**)&d.logpsi, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.sign, W * 4, st));
+    CUW(w->pool.alloc((void**)&d.flags, W * 4, st));
+    CUW(w->pool.alloc((void**)&d.eloc, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.ekin, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.ebuf, W * s.ne * 2 * 8, st));
+    CUW(w->pool.alloc((void**)&d.stats, 4 * 8, st));
+    CUW(w->pool.alloc((void**)&w->d_status, 4, st));
+    rc = alloc_window(w, 16);
+    if (rc) { std::string m = g_err; destroy_walkers(w); return fail(rc, m); }
+
+    // positions in (host or device) -> walker-major SoA
+    {
+        double* tmp;
+        size_t bytes = W * s.ne * 3 * 8;
+        CUW(cudaMalloc((void**)&tmp, bytes));
+        cudaError_t e = cudaMemcpyAsync(tmp, positions, bytes, cudaMemcpyDefault, st);
+        if (e == cudaSuccess) e = launch_import_positions(d, tmp, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(tmp);
+        CUW(e);
+    }
+    CUW(launch_fill_int(d.sign, n_walkers, 1, st));
+    // orbital rows of every electron: basis kernel + FP64 contraction, one electron index at a time
+    for (int sp = 0; sp < 2; sp++) {
+        const int e0 = sp == 0 ? 0 : s.ns[0];
+        for (int p = 0; p < s.ns[sp]; p++) {
+            CUW(launch_gather_rp(d, e0 + p, st));
+            CUW(launch_basis(s, d.rp, n_walkers, d.Phi, s.nbp, st));
+            CUW(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, st));
+            CUW(launch_store_init_rows(s, d, sp, p, st));
+        }
+        CUW(launch_gj_inverse(d.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp], s.ns[sp], s.nsp[sp], n_walkers, d.logpsi, d.sign, w->d_status, st));
+    }
+    int status = 0;
+    CUW(cudaMemcpyAsync(&status, w->d_status, 4, cudaMemcpyDeviceToHost, st));
+    CUW(cudaStreamSynchronize(st));
+    if (status != 0) {
+        destroy_walkers(w);
+        return fail(QMC_ERR_SINGULAR, "qmc_walkers_create: singular Slater matrix (zero pivot)");
+    }
+    CUW(launch_jastrow_total(s, d, st));
+    CUW(launch_window_reset(d, st));
+    CUW(launch_eloc(s, d, st));
+    CUW(cudaStreamSynchronize(st));
+    *out = w;
+    return QMC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ profiling hooks
+
+static void prof_begin(qmc_walkers* w, int stage, bool on) {
+    if (!on) return;
+    StageTimer& t = w->timer;
+    if (t.used + 2 > t.ev.size()) {
+        cudaEvent_t a, b;
+        cudaEventCreate(&a);
+        cudaEventCreate(&b);
+        t.ev.push_back(a);
+        t.ev.push_back(b);
+    }
+    t.stage.resize(t.ev.size() / 2);
+    t.stage[t.used / 2] = stage;
+    cudaEventRecord(t.ev[t.used], w->stream);
+}
+static void prof_end(qmc_walkers* w, bool on) {
+    if (!on) return;
+    StageTimer& t = w->timer;
+    cudaEventRecord(t.ev[t.used + 1], w->stream);
+    t.used += 2;
+}
+static void prof_collect(qmc_walkers* w) {
+    StageTimer& t = w->timer;
+    if (t.used == 0) return;
+    cudaStreamSynchronize(w->stream);
+    for (size_t i = 0; i < t.used; i += 2) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, t.ev[i], t.ev[i + 1]) == cudaSuccess) {
+            w->stage_ms[t.stage[i / 2]] += ms;
+            w->stage_n[t.stage[i / 2]] += 1;
+        }
+    }
+    t.used = 0;
+}
+
+/* stage ids: 0 propose, 1 basis, 2 MO contraction, 3 accept, 4 flush, 5 local energy */
+extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
+    if (!w || stride < 0) return fail(QMC_ERR_ARG, "qmc_set_profiling");
+    prof_collect(w);
+    w->prof_stride = stride;
+    memset(w->stage_ms, 0, sizeof(w->stage_ms));
+    memset(w->stage_n, 0, sizeof(w->stage_n));
+    return QMC_OK;
+}
+extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t* counts /*[6]*/) {
+    if (!w || !ms || !counts) return fail(QMC_ERR_ARG, "qmc_get_stage_times");
+    prof_collect(w);
+    for (int i = 0; i < 6; i++) { ms[i] = w->stage_ms[i]; counts[i] = w->stage_n[i]; }
+    return QMC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ qmc_sweep
+
+extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
+    if (nsteps < 0) return fail(QMC_ERR_ARG, "qmc_sweep: nsteps < 0");
+    if (!(tau > 0.0) || !isfinite(tau)) return fail(QMC_ERR_ARG, "qmc_sweep: tau must be > 0");
+    if (delay_k < 1 || delay_k > 128) return fail(QMC_ERR_ARG, "qmc_sweep: delay_k must be in 1..128");
+    const SysDev& s = w->sys->d;
+    WalkDev& d = w->d;
+    cudaStream_t st = w->stream;
+    const int kp = round_up(delay_k, 16);
+    if (kp != d.kp) {
+        int rc = alloc_window(w, kp);
+        if (rc) return rc;
+        CU(launch_window_reset(d, st));
+    }
+    // accept / ratio logs of this call
+    CU(cudaStreamSynchronize(st));
+    w->logpool.free_all();
+    d.bits = nullptr; d.ratio_log = nullptr; d.pacc_log = nullptr;
+    const size_t nlog = (size_t)nsteps * s.ne * d.W;
+    CU(w->logpool.alloc((void**)&d.bits, nlog, st));
+    if (w->flags & QMC_LOG_RATIOS) {
+        CU(w->logpool.alloc((void**)&d.ratio_log, nlog * 8, st));
+        CU(w->logpool.alloc((void**)&d.pacc_log, nlog * 8, st));
+    }
+    w->T_last = nsteps;
+    for (int t = 0; t < nsteps; t++) {
+        for (int sp = 0; sp < 2; sp++) {
+            const int ns = s.ns[sp], e0 = sp == 0 ? 0 : s.ns[0];
+            int in_window = 0;
+            for (int p = 0; p < ns; p++) {
+                const int e = e0 + p;
+                const long log_off = ((long)t * s.ne + e) * d.W;
+                const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
+                prof_begin(w, 0, prof);
+                CU(launch_propose(s, d, sp, p, e, w->step, tau, st));
+                prof_end(w, prof);
+                prof_begin(w, 1, prof);
+                CU(launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st));
+                prof_end(w, prof);
+                prof_begin(w, 2, prof);
+                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, st));
+                prof_end(w, prof);
+                prof_begin(w, 3, prof);
+                CU(launch_accept(s, d, sp, p, e, log_off, tau, 1, st));
+                prof_end(w, prof);
+                in_window++;
+                if (in_window == delay_k || p == ns - 1) {
+                    const bool pf = w->prof_stride > 0;
+                    prof_begin(w, 4, pf);
+                    CU(launch_flush(s, d, sp, st));
+                    prof_end(w, pf);
+                    in_window = 0;
+                }
+            }
+        }
+        const bool pf = w->prof_stride > 0;
+        prof_begin(w, 5, pf);
+        CU(launch_eloc(s, d, st));
+        prof_end(w, pf);
+        w->step++;
+        if (w->timer.used > 8192) prof_collect(w);
+    }
+    return QMC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ getters
+
+static bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// run `produce(dev_buffer)` into `out` (device: directly; host: via a staging buffer + synchronous copy)
+template <class F>
+static int deliver(const qmc_walkers* w, void* out, size_t bytes, F&& produce) {
+    cudaStream_t st = w->stream;
+    if (bytes == 0) return QMC_OK;
+    if (is_device_ptr(out)) {
+        CU(produce(out));
+        return QMC_OK;
+    }
+    void* tmp;
+    CU(cudaMalloc(&tmp, bytes));
+    cudaError_t e = produce(tmp);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(tmp);
+    CU(e);
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_positions(const qmc_walkers* w, double* out) {
+    if (!w || !out) return fail(QMC_ERR_ARG, "qmc_get_positions: null argument");
+    return deliver(w, out, (size_t)w->d.W * w->d.ne * 3 * 8, [&](void* dst) { return launch_export_positions(w->d, (double*)dst, w->stream); });
+}
+
+extern "C" int qmc_get_Ainv(const qmc_walkers* w, int spin, double* out) {
+    if (!w || !out || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_get_Ainv: bad argument");
+    const SysDev& s = w->sys->d;
+    return deliver(w, out, (size_t)w->d.W * s.ns[spin] * s.ns[spin] * 8,
+                   [&](void* dst) { return launch_export_ainv(w->d.AinvT[spin], w->d.W, s.ns[spin], s.nsp[spin], (double*)dst, w->stream); });
+}
+
+extern "C" int qmc_get_logpsi(const qmc_walkers* w, double* logabs, int8_t* sign) {
+    if (!w || !logabs) return fail(QMC_ERR_ARG, "qmc_get_logpsi: null argument");
+    int rc = deliver(w, logabs, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.logpsi, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
+    if (rc || !sign) return rc;
+    return deliver(w, sign, (size_t)w->d.W, [&](void* dst) { return launch_sign_to_i8(w->d.sign, w->d.W, (int8_t*)dst, w->stream); });
+}
+
+extern "C" int qmc_get_eloc(const qmc_walkers* w, double* eloc, double* ekin) {
+    if (!w || !eloc) return fail(QMC_ERR_ARG, "qmc_get_eloc: null argument");
+    int rc = deliver(w, eloc, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.eloc, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
+    if (rc || !ekin) return rc;
+    return deliver(w, ekin, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.ekin, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
+}
+
+extern "C" int qmc_get_accept_log(const qmc_walkers* w, uint8_t* bits) {
+    if (!w || !bits) return fail(QMC_ERR_ARG, "qmc_get_accept_log: null argument");
+    if (!w->d.bits) return fail(QMC_ERR_STATE, "qmc_get_accept_log: no sweep has been run");
+    size_t n = (size_t)w->T_last * w->d.ne * w->d.W;
+    if (n == 0) return QMC_OK;
+    CU(cudaMemcpyAsync(bits, w->d.bits, n, cudaMemcpyDefault, w->stream));
+    if (!is_device_ptr(bits)) CU(cudaStreamSynchronize(w->stream));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_ratio_log(const qmc_walkers* w, double* ratio, double* pacc) {
+    if (!w || !ratio) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null argument");
+    if (!(w->flags & QMC_LOG_RATIOS) || !w->d.ratio_log) return fail(QMC_ERR_STATE, "qmc_get_ratio_log: walkers were not created with QMC_LOG_RATIOS, or no sweep has run");
+    size_t n = (size_t)w->T_last * w->d.ne * w->d.W * 8;
+    if (n == 0) return QMC_OK;
+    CU(cudaMemcpyAsync(ratio, w->d.ratio_log, n, cudaMemcpyDefault, w->stream));
+    if (pacc) CU(cudaMemcpyAsync(pacc, w->d.pacc_log, n, cudaMemcpyDefault, w->stream));
+    if (!is_device_ptr(ratio) || (pacc && !is_device_ptr(pacc))) CU(cudaStreamSynchronize(w->stream));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_stats(const qmc_walkers* w, uint64_t* n_proposed, uint64_t* n_accepted, uint64_t* n_ties, uint64_t* n_nonfinite) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_get_stats: null walkers");
+    unsigned long long h[4];
+    CU(cudaMemcpyAsync(h, w->d.stats, sizeof(h), cudaMemcpyDeviceToHost, w->stream));
+    CU(cudaStreamSynchronize(w->stream));
+    if (n_proposed) *n_proposed = h[0];
+    if (n_accepted) *n_accepted = h[1];
+    if (n_ties) *n_ties = h[2];
+    if (n_nonfinite) *n_nonfinite = h[3];
+    return QMC_OK;
+}
+
+extern "C" int qmc_synchronize(const qmc_walkers* w) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_synchronize: null walkers");
+    CU(cudaStreamSynchronize(w->stream));
+    return QMC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ stage-level entry points
+
+static int eval_common(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream, bool mo) {
+    if (!sys || !xyz || !out || n_points < 0 || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_eval_*: bad argument");
+    int rc = check_device();
+    if (rc) return rc;
+    if (n_points == 0) return QMC_OK;
+    const SysDev& s = sys->d;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double *pts = nullptr, *Phi = nullptr, *V = nullptr, *stage = nullptr;
+    const int width = mo ? s.ns[spin] : s.n_basis;
+    const size_t out_bytes = (size_t)n_points * 5 * width * 8;
+    cudaError_t e = cudaMalloc((void**)&pts, (size_t)n_points * 3 * 8);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&Phi, (size_t)n_points * 5 * s.nbp * 8);
+    if (e == cudaSuccess) e = cudaMemsetAsync(Phi, 0, (size_t)n_points * 5 * s.nbp * 8, st);
+    if (e == cudaSuccess && mo) e = cudaMalloc((void**)&V, (size_t)n_points * 5 * s.nsp[spin] * 8 + 16);
+    const bool dev_out = is_device_ptr(out);
+    if (e == cudaSuccess && !dev_out) e = cudaMalloc((void**)&stage, out_bytes + 16);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pts, xyz, (size_t)n_points * 3 * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = launch_basis(s, pts, n_points, Phi, s.nbp, st);
+    double* dst = dev_out ? out : stage;
+    if (e == cudaSuccess) {
+        if (mo) {
+            e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], st);
+            if (e == cudaSuccess) e = launch_export_rows(V, (long)n_points * 5, width, s.nsp[spin], dst, st);
+        } else {
+            e = launch_export_rows(Phi, (long)n_points * 5, width, s.nbp, dst, st);
+        }
+    }
+    if (e == cudaSuccess && !dev_out) e = cudaMemcpyAsync(out, stage, out_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(pts); cudaFree(Phi); cudaFree(V); cudaFree(stage);
+    CU(e);
+    return QMC_OK;
+}
+
+extern "C" int qmc_eval_basis(const qmc_system* sys, int n_points, const double* xyz, double* out, void* cuda_stream) {
+    return eval_common(sys, 0, n_points, xyz, out, cuda_stream, false);
+}
+extern "C" int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream) {
+    return eval_common(sys, spin, n_points, xyz, out, cuda_stream, true);
+}
+
+extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, double* ms_per_launch) {
+    if (!w || !ms_per_launch || stage < 0 || stage > 5 || spin < 0 || spin > 1 || reps < 1 || delay_k < 1 || delay_k > 128)
+        return fail(QMC_ERR_ARG, "qmc_time_stage: bad argument");
+    const SysDev& s = w->sys->d;
+    WalkDev& d = w->d;
+    cudaStream_t st = w->stream;
+    if (s.ns[spin] == 0) return fail(QMC_ERR_ARG, "qmc_time_stage: empty spin block");
+    const int kp = round_up(delay_k, 16);
+    if (kp != d.kp) {
+        int rc = alloc_window(w, kp);
+        if (rc) return rc;
+        CU(launch_window_reset(d, st));
+    }
+    const int p = 0, e = spin == 0 ? 0 : s.ns[0];
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    // make the inputs of the later stages valid
+    CU(launch_propose(s, d, spin, p, e, w->step, 0.005, st));
+    CU(launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st));
+    CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, st));
+    if (stage == 4) CU(launch_fill_int(d.mcount, d.W, delay_k, st));  // full window, S^-1 = 0: zero correction
+    cudaError_t err = cudaSuccess;
+    for (int r = -2; r < reps && err == cudaSuccess; r++) {
+        if (r == 0) err = cudaEventRecord(e0, st);
+        if (err != cudaSuccess) break;
+        switch (stage) {
+            case 0: err = launch_propose(s, d, spin, p, e, w->step, 0.005, st); break;
+            case 1: err = launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st); break;
+            case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, st); break;
+            case 3: err = launch_accept(s, d, spin, p, e, 0, 0.005, 0, st); break;
+            case 4:
+                err = launch_flush(s, d, spin, st);
+                if (err == cudaSuccess) err = launch_fill_int(d.mcount, d.W, delay_k, st);
+                break;
+            case 5: err = launch_eloc(s, d, st); break;
+        }
+    }
+    if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+    if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (stage == 4) { cudaError_t e2 = launch_window_reset(d, st); if (err == cudaSuccess) err = e2; }
+    CU(err);
+    CU(cudaStreamSynchronize(st));
+    *ms_per_launch = (double)ms / reps;
+    return QMC_OK;
+}
+
+extern "C" int qmc_measure_fp64_peak(double ms_target, double* tflops, void* cuda_stream) {
+    if (!tflops || !(ms_target > 0.0)) return fail(QMC_ERR_ARG, "qmc_measure_fp64_peak: bad argument");
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = sms * 2, threads = 512, iters = 20000;
+    double* buf;
+    CU(cudaMalloc((void**)&buf, (size_t)grid * threads * 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaError_t err = launch_dmma_peak(buf, grid, threads, 200, st);
+    const double flop_per_launch = 2.0 * 8 * 8 * 4 * 8.0 * iters * (double)grid * (threads / 32);
+    double total_ms = 0.0, total_flop = 0.0;
+    while (err == cudaSuccess && total_ms < ms_target) {
+        err = cudaEventRecord(e0, st);
+        if (err == cudaSuccess) err = launch_dmma_peak(buf, grid, threads, iters, st);
+        if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        total_ms += ms;
+        total_flop += flop_per_launch;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    CU(err);
+    *tflops = total_flop / (total_ms * 1e-3) * 1e-12;
+    return QMC_OK;
+}

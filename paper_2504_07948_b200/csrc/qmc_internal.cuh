@@ -1,0 +1,58 @@
+// qmc_internal.cuh -- device-side data layout shared by the kernels and the host scheduler.
+//
+// HBM layout (all FP64 unless noted; "NSP" = n_s rounded up to 16, "NBP" = n_basis rounded up to 16,
+// padding is zero and stays zero, so padded orbitals/functions contribute nothing):
+//   C[s]      [NBP][NSP]            MO coefficients of spin s (GEMM B operand, N contiguous)
+//   R         [W][3][NEP]           positions, walker-major SoA (coalesced over electrons inside a walker)
+//   AinvT[s]  [W][NSP][NSP]         AinvT[p][j] = (A^-1)[j][p]: row p is the column the ratio needs (A18)
+//   Orb[s]    [W][NSP(p)][5][NSP]   value / d/dx / d/dy / d/dz / laplacian of the orbitals at the CURRENT
+//                                   position of electron p (row cache: drift and E_L cost O(N_s) per electron)
+//   Phi       [W*5][NBP]            basis functions at the proposed positions (GEMM A operand)
+//   V         [W*5][LDV]            orbital rows at the proposed positions (GEMM output)
+//   window    Vbuf,Wbuf,W2 [W][KP][NSP], SinvT [W][KP][KP], YT [W][NSP][KP], plist [W][KP] int, mcount [W] int
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qmc {
+
+struct ShellRec {
+    double x, y, z;
+    int l, f0, nprim, poff;
+};
+
+struct SysDev {
+    int n_atoms, n_shells, n_basis, nbp;
+    int ns[2], nsp[2], ne;
+    const double* atom_xyz;  // [n_atoms][3]
+    const double* atom_Z;
+    const ShellRec* shells;
+    const double* alpha;
+    const double* coef;
+    const double* C[2];
+    double a_anti, a_para, b_ee, b_en;
+    double e_nn;  // nuclear repulsion
+};
+
+struct WalkDev {
+    int W, ne, nep, ldv, kp;
+    double* R;
+    double* AinvT[2];
+    double* Orb[2];
+    double* Phi;
+    double* V;
+    double *Vbuf, *Wbuf, *W2, *SinvT, *YT, *bvec, *cvec, *xcol;
+    int *plist, *mcount;
+    double *rp, *G, *u, *dJ, *gJn;  // per-walker proposal scalars: [W][3], [W][3], [W], [W], [W][3]
+    double* logpsi;
+    int* sign;
+    unsigned* flags;  // sticky non-finite flag per walker
+    double *eloc, *ekin, *ebuf;  // ebuf [W][ne][2]
+    uint8_t* bits;               // [T][ne][W] of the current sweep call
+    double *ratio_log, *pacc_log;
+    unsigned long long* stats;  // proposed, accepted, ties, nonfinite
+    uint64_t seed;
+    uint32_t first_walker;
+};
+
+}  // namespace qmc

@@ -1,0 +1,872 @@
+// qmc_kernels.cu -- the CUDA kernels of the batched electron move (sm_100a) and their launchers.
+// Rows a1-a9 of SURVEY.md 8(a); formulas follow BASELINE.json north_star / DESIGN.md "Readings".
+#include "qmc_kernels.cuh"
+
+#include <math.h>
+
+#include "gemm_f64.cuh"
+
+namespace qmc {
+
+thread_local uint64_t g_launches = 0;
+#define COUNT_LAUNCH() (++g_launches)
+
+// ------------------------------------------------------------------------------------------------
+// block reductions (fixed shape -> deterministic): NV sums at once over a block of NT threads
+template <int NT, int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* red /* [NV * NT/32] */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    }
+    __syncthreads();  // protect red from a previous use
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; i++) red[i * (NT / 32) + warp] = v[i];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+        double s = 0.0;
+#pragma unroll
+        for (int k = 0; k < NT / 32; k++) s += red[i * (NT / 32) + k];
+        v[i] = s;
+    }
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Philox4x32-10, key = (seed lo, seed hi), counter = (walker, step, electron, block)   [reading A11]
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+__device__ __forceinline__ double u01(uint32_t we, uint32_t wo) {
+    unsigned long long x = ((unsigned long long)we << 32) | (unsigned long long)wo;
+    return (double)(2ull * (x >> 12) + 1ull) * 0x1.0p-53;  // odd integer * 2^-53: exact, in (0,1)
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3: basis functions (value, gradient, laplacian) at one point per blockIdx.y        [north_star item 1]
+// out[(pt*5 + c)*ld + f].  One thread per shell; the shell table is read through the read-only path.
+__global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restrict__ pts, double* __restrict__ out, long ld) {
+    const int pt = blockIdx.y;
+    const int sh = blockIdx.x * blockDim.x + threadIdx.x;
+    if (sh >= s.n_shells) return;
+    const double px = pts[3 * pt], py = pts[3 * pt + 1], pz = pts[3 * pt + 2];
+    const ShellRec rec = s.shells[sh];
+    const double x = px - rec.x, y = py - rec.y, z = pz - rec.z;
+    const double t = x * x + y * y + z * z;
+    double g = 0.0, g1 = 0.0, g2 = 0.0;
+    for (int p = 0; p < rec.nprim; p++) {
+        const double al = __ldg(s.alpha + rec.poff + p);
+        const double e = __ldg(s.coef + rec.poff + p) * exp(-al * t);
+        g += e;
+        g1 -= al * e;
+        g2 += al * al * e;
+    }
+    double* o = out + (long)pt * 5 * ld + rec.f0;
+    const double lapfac = (double)(4 * rec.l + 6) * g1 + 4.0 * t * g2;
+    const double tg1 = 2.0 * g1;
+    auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
+        o[m] = S * g;
+        o[ld + m] = g * Sx + tg1 * S * x;
+        o[2 * ld + m] = g * Sy + tg1 * S * y;
+        o[3 * ld + m] = g * Sz + tg1 * S * z;
+        o[4 * ld + m] = S * lapfac;
+    };
+    const double s3 = 1.7320508075688772;
+    if (rec.l == 0) {
+        emit(0, 1.0, 0.0, 0.0, 0.0);
+    } else if (rec.l == 1) {
+        emit(0, x, 1.0, 0.0, 0.0);
+        emit(1, y, 0.0, 1.0, 0.0);
+        emit(2, z, 0.0, 0.0, 1.0);
+    } else {
+        emit(0, s3 * x * y, s3 * y, s3 * x, 0.0);
+        emit(1, s3 * y * z, 0.0, s3 * z, s3 * y);
+        emit(2, z * z - 0.5 * (x * x + y * y), -x, -y, 2.0 * z);
+        emit(3, s3 * x * z, s3 * z, 0.0, s3 * x);
+        emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
+    }
+}
+
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* out, long ld, cudaStream_t st) {
+    if (n_points == 0) return cudaSuccess;
+    dim3 grid((s.n_shells + 127) / 128, n_points);
+    k_basis<<<grid, 128, 0, st>>>(s, pts, out, ld);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4: MO rows V = Phi * C_s  (FP64 DMMA GEMM)                                          [north_star item 2]
+using CfgMO = GemmCfg<128, 128, 64, 32, false, 4>;
+
+cudaError_t launch_mo(const SysDev& s, int spin, const double* Phi, int rows, double* V, long ldv, cudaStream_t st) {
+    GemmArgs g;
+    g.A = Phi; g.lda = s.nbp; g.strideA = 0;
+    g.B = s.C[spin]; g.ldb = s.nsp[spin]; g.strideB = 0;
+    g.C = V; g.ldc = ldv; g.strideC = 0;
+    g.M = rows; g.N = s.nsp[spin]; g.K = s.nbp;
+    COUNT_LAUNCH();
+    return gemm_f64_launch<CfgMO>(g, 1, EpiStore{}, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Pade Jastrow pieces
+__device__ __forceinline__ double pade_u(double a, double b, double r) { return a * r / (1.0 + b * r); }
+__device__ __forceinline__ double pade_du(double a, double b, double r) { double q = 1.0 + b * r; return a / (q * q); }
+__device__ __forceinline__ double pade_d2u(double a, double b, double r) { double q = 1.0 + b * r; return -2.0 * a * b / (q * q * q); }
+
+// partner k of electron e: k < ne electrons (skip k == e), then atoms
+struct Partner { double x, y, z, a, b; bool ok; };
+__device__ __forceinline__ Partner partner(const SysDev& s, const double* __restrict__ Rw, int nep, int e, int k) {
+    Partner P;
+    if (k < s.ne) {
+        P.x = Rw[k]; P.y = Rw[nep + k]; P.z = Rw[2 * nep + k];
+        const bool same = (k < s.ns[0]) == (e < s.ns[0]);
+        P.a = same ? s.a_para : s.a_anti;
+        P.b = s.b_ee;
+        P.ok = (k != e);
+    } else {
+        const int I = k - s.ne;
+        P.x = s.atom_xyz[3 * I]; P.y = s.atom_xyz[3 * I + 1]; P.z = s.atom_xyz[3 * I + 2];
+        P.a = -s.atom_Z[I];
+        P.b = s.b_en;
+        P.ok = true;
+    }
+    return P;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 + a2 + a6: effective inverse column, drift, Philox proposal, Jastrow ratio and gradient at r'.
+// One CTA per walker.                                                           [north_star items 3, 4]
+constexpr int PT = 256;
+
+__global__ void __launch_bounds__(PT) k_propose(SysDev s, WalkDev wd, int spin, int p, int e, uint32_t step, double tau,
+                                                double sqrt_tau) {
+    extern __shared__ double sm[];
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
+    double* xs = sm;              // [nsp]
+    double* bs = xs + nsp;        // [kp]
+    double* cs = bs + kp;         // [kp]
+    double* red = cs + kp;        // [8 * PT/32]
+    double* bc = red + 8 * (PT / 32);  // [4] broadcast
+    const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
+    const int m = wd.mcount[w];
+    for (int j = tid; j < nsp; j += PT) xs[j] = arow[j];
+    __syncthreads();
+    if (m > 0) {
+        // b_n = v_n . a_p ;  c = S^-1 b ;  x = a_p - Wbuf^T c     (effective column of the delayed inverse)
+        const double* Vb = wd.Vbuf + (long)w * kp * nsp;
+        const double* Wb = wd.Wbuf + (long)w * kp * nsp;
+        const double* Si = wd.SinvT + (long)w * kp * kp;
+        for (int n = warp; n < m; n += PT / 32) {
+            double acc = 0.0;
+            for (int j = lane; j < nsp; j += 32) acc += Vb[(long)n * nsp + j] * xs[j];
+            acc = warp_sum(acc);
+            if (lane == 0) bs[n] = acc;
+        }
+        __syncthreads();
+        for (int n = tid; n < m; n += PT) {
+            double acc = 0.0;
+            for (int l = 0; l < m; l++) acc += Si[l * kp + n] * bs[l];
+            cs[n] = acc;
+            wd.cvec[(long)w * kp + n] = acc;
+        }
+        __syncthreads();
+        for (int j = tid; j < nsp; j += PT) {
+            double acc = xs[j];
+            for (int l = 0; l < m; l++) acc -= cs[l] * Wb[(long)l * nsp + j];
+            xs[j] = acc;
+        }
+        __syncthreads();
+    }
+    double* xcol = wd.xcol + (long)w * nsp;
+    for (int j = tid; j < nsp; j += PT) xcol[j] = xs[j];
+
+    // drift: determinant part from the cached gradient rows, Jastrow part by direct sums
+    const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
+    const double* Rw = wd.R + (long)w * 3 * nep;
+    const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
+    double acc6[6] = {0, 0, 0, 0, 0, 0};
+    for (int j = tid; j < nsp; j += PT) {
+        const double xj = xs[j];
+        acc6[0] += orb[nsp + j] * xj;
+        acc6[1] += orb[2 * nsp + j] * xj;
+        acc6[2] += orb[3 * nsp + j] * xj;
+    }
+    const int npart = s.ne + s.n_atoms;
+    for (int k = tid; k < npart; k += PT) {
+        Partner P = partner(s, Rw, nep, e, k);
+        if (P.ok) {
+            const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
+            const double r = sqrt(dx * dx + dy * dy + dz * dz);
+            const double du = pade_du(P.a, P.b, r);
+            acc6[3] += du * dx / r;
+            acc6[4] += du * dy / r;
+            acc6[5] += du * dz / r;
+        }
+    }
+    block_sum<PT, 6>(acc6, red);
+    if (tid == 0) {
+        const double Gx = acc6[0] + acc6[3], Gy = acc6[1] + acc6[4], Gz = acc6[2] + acc6[5];
+        const uint32_t wid = wd.first_walker + (uint32_t)w;
+        const uint32_t k0 = (uint32_t)(wd.seed & 0xFFFFFFFFull), k1 = (uint32_t)(wd.seed >> 32);
+        uint32_t o[4];
+        philox4x32_10(wid, step, (uint32_t)e, 0u, k0, k1, o);
+        const double U1 = u01(o[0], o[1]), U2 = u01(o[2], o[3]);
+        philox4x32_10(wid, step, (uint32_t)e, 1u, k0, k1, o);
+        const double U3 = u01(o[0], o[1]), U4 = u01(o[2], o[3]);
+        philox4x32_10(wid, step, (uint32_t)e, 2u, k0, k1, o);
+        const double U5 = u01(o[0], o[1]);
+        const double TWO_PI = 6.283185307179586;
+        const double r1 = sqrt(-2.0 * log(U1)), r2 = sqrt(-2.0 * log(U3));
+        const double chx = r1 * cos(TWO_PI * U2), chy = r1 * sin(TWO_PI * U2), chz = r2 * cos(TWO_PI * U4);
+        const double qx = rx + tau * Gx + sqrt_tau * chx;
+        const double qy = ry + tau * Gy + sqrt_tau * chy;
+        const double qz = rz + tau * Gz + sqrt_tau * chz;
+        wd.rp[3 * w] = qx; wd.rp[3 * w + 1] = qy; wd.rp[3 * w + 2] = qz;
+        wd.G[3 * w] = Gx; wd.G[3 * w + 1] = Gy; wd.G[3 * w + 2] = Gz;
+        wd.u[w] = U5;
+        bc[0] = qx; bc[1] = qy; bc[2] = qz;
+    }
+    __syncthreads();
+    const double qx = bc[0], qy = bc[1], qz = bc[2];
+    // Jastrow ratio (term by term) and gradient at r'
+    double acc4[4] = {0, 0, 0, 0};
+    for (int k = tid; k < npart; k += PT) {
+        Partner P = partner(s, Rw, nep, e, k);
+        if (P.ok) {
+            const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
+            const double ex = qx - P.x, ey = qy - P.y, ez = qz - P.z;
+            const double r_old = sqrt(dx * dx + dy * dy + dz * dz);
+            const double r_new = sqrt(ex * ex + ey * ey + ez * ez);
+            acc4[0] += pade_u(P.a, P.b, r_new) - pade_u(P.a, P.b, r_old);
+            const double du = pade_du(P.a, P.b, r_new);
+            acc4[1] += du * ex / r_new;
+            acc4[2] += du * ey / r_new;
+            acc4[3] += du * ez / r_new;
+        }
+    }
+    block_sum<PT, 4>(acc4, red);
+    if (tid == 0) {
+        wd.dJ[w] = acc4[0];
+        wd.gJn[3 * w] = acc4[1]; wd.gJn[3 * w + 1] = acc4[2]; wd.gJn[3 * w + 2] = acc4[3];
+    }
+}
+
+size_t propose_smem(const SysDev& s, const WalkDev& wd, int spin) {
+    return (size_t)(s.nsp[spin] + 2 * wd.kp + 8 * (PT / 32) + 4) * sizeof(double);
+}
+
+cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st) {
+    k_propose<<<wd.W, PT, propose_smem(s, wd, spin), st>>>(s, wd, spin, p, e, step, tau, sqrt(tau));
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 + a7: determinant ratio and gradient from the effective column, accept/reject, commit.
+// One CTA per walker.  commit == 0 evaluates everything but changes no state (stage timing).
+__global__ void __launch_bounds__(PT) k_accept(SysDev s, WalkDev wd, int spin, int p, int e, long log_off, double tau, int commit) {
+    extern __shared__ double sm[];
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
+    double* rs = sm;                   // [kp]
+    double* ts = rs + kp;              // [kp]
+    double* cs = ts + kp;              // [kp]
+    double* red = cs + kp;             // [8 * PT/32]
+    double* bc = red + 8 * (PT / 32);  // [4]
+    const double* v = wd.V + (long)w * 5 * wd.ldv;
+    const double* xcol = wd.xcol + (long)w * nsp;
+    double a4[4] = {0, 0, 0, 0};
+    for (int j = tid; j < nsp; j += PT) {
+        const double xj = xcol[j];
+        a4[0] += v[j] * xj;
+        a4[1] += v[wd.ldv + j] * xj;
+        a4[2] += v[2 * wd.ldv + j] * xj;
+        a4[3] += v[3 * wd.ldv + j] * xj;
+    }
+    block_sum<PT, 4>(a4, red);
+    const double rho = a4[0];
+    if (tid == 0) {
+        double* Rw = wd.R + (long)w * 3 * nep;
+        const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
+        const double qx = wd.rp[3 * w], qy = wd.rp[3 * w + 1], qz = wd.rp[3 * w + 2];
+        const double Gx = wd.G[3 * w], Gy = wd.G[3 * w + 1], Gz = wd.G[3 * w + 2];
+        const double u = wd.u[w], dJ = wd.dJ[w];
+        unsigned bits = 0;
+        double pacc = 0.0, jr = 0.0;
+        bool accept = false;
+        if (fabs(rho) < 1e-12) bits |= 2u;
+        if (rho > 0.0) {  // fixed node: reject rho_D <= 0 (A7); NaN fails the comparison and rejects
+            const double Hx = a4[1] / rho + wd.gJn[3 * w], Hy = a4[2] / rho + wd.gJn[3 * w + 1], Hz = a4[3] / rho + wd.gJn[3 * w + 2];
+            const double ax = qx - rx - tau * Gx, ay = qy - ry - tau * Gy, az = qz - rz - tau * Gz;
+            const double cx = rx - qx - tau * Hx, cy = ry - qy - tau * Hy, cz = rz - qz - tau * Hz;
+            const double fwd = ax * ax + ay * ay + az * az, rev = cx * cx + cy * cy + cz * cz;
+            const double Delta = (fwd - rev) / (2.0 * tau);
+            pacc = rho * rho * exp(2.0 * dJ + Delta);  // A25: linear domain, one exp
+            jr = rho * exp(dJ);
+            if (fabs(u - pacc) < 1e-12) bits |= 2u;
+            accept = (u < pacc);
+        }
+        const bool nonfinite = isnan(rho) || isnan(pacc);
+        if (nonfinite) { bits |= 4u; accept = false; }
+        if (accept) bits |= 1u;
+        if (commit) {
+            wd.bits[log_off + w] = (uint8_t)bits;
+            if (wd.ratio_log) { wd.ratio_log[log_off + w] = jr; wd.pacc_log[log_off + w] = pacc; }
+            atomicAdd(&wd.stats[0], 1ull);
+            if (accept) atomicAdd(&wd.stats[1], 1ull);
+            if (bits & 2u) atomicAdd(&wd.stats[2], 1ull);
+            if (nonfinite) { atomicAdd(&wd.stats[3], 1ull); wd.flags[w] = 1u; }
+            if (accept) {
+                Rw[e] = qx; Rw[nep + e] = qy; Rw[2 * nep + e] = qz;
+                wd.logpsi[w] += log(rho) + dJ;
+            }
+        }
+        bc[0] = (accept && commit) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    if (bc[0] == 0.0) return;
+    // ---- commit: row caches, delay window (Vbuf, Wbuf, bordered update of S^-1)
+    const int m = wd.mcount[w];
+    double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
+    double* Vb = wd.Vbuf + (long)w * kp * nsp;
+    double* Wb = wd.Wbuf + (long)w * kp * nsp;
+    double* Si = wd.SinvT + (long)w * kp * kp;
+    const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
+    for (int j = tid; j < nsp; j += PT) {
+        const double vj = v[j];
+        orb[j] = vj;
+        orb[nsp + j] = v[wd.ldv + j];
+        orb[2 * nsp + j] = v[2 * wd.ldv + j];
+        orb[3 * nsp + j] = v[3 * wd.ldv + j];
+        orb[4 * nsp + j] = v[4 * wd.ldv + j];
+        Vb[(long)m * nsp + j] = vj;
+        Wb[(long)m * nsp + j] = arow[j];
+    }
+    // r_l = v . Wbuf[l]  (row m of S)
+    for (int l = warp; l < m; l += PT / 32) {
+        double acc = 0.0;
+        for (int j = lane; j < nsp; j += 32) acc += v[j] * Wb[(long)l * nsp + j];
+        acc = warp_sum(acc);
+        if (lane == 0) rs[l] = acc;
+    }
+    for (int n = tid; n < m; n += PT) cs[n] = wd.cvec[(long)w * kp + n];
+    __syncthreads();
+    // t_l = sum_n r_n Sinv[n][l] = sum_n r_n SinvT[l][n]
+    for (int l = tid; l < m; l += PT) {
+        double acc = 0.0;
+        for (int n = 0; n < m; n++) acc += rs[n] * Si[l * kp + n];
+        ts[l] = acc;
+    }
+    __syncthreads();
+    const double sinv = 1.0 / rho;
+    for (int idx = tid; idx < m * m; idx += PT) {
+        const int l = idx / m, n = idx % m;
+        Si[l * kp + n] += cs[n] * ts[l] * sinv;
+    }
+    for (int n = tid; n < m; n += PT) {
+        Si[m * kp + n] = -cs[n] * sinv;
+        Si[n * kp + m] = -ts[n] * sinv;
+    }
+    if (tid == 0) {
+        Si[m * kp + m] = sinv;
+        wd.plist[(long)w * kp + m] = p;
+        wd.mcount[w] = m + 1;
+    }
+}
+
+cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st) {
+    size_t smem = (size_t)(3 * wd.kp + 8 * (PT / 32) + 4) * sizeof(double);
+    k_accept<<<wd.W, PT, smem, st>>>(s, wd, spin, p, e, log_off, tau, commit);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8: delayed rank-k flush as FP64 GEMMs                                           [north_star item 5]
+//   YT[q][n] = AinvT0[q][:] . Vbuf[n][:] - delta(q, p_n)           (n < m; columns n >= m are zero)
+//   W2[l][j] = sum_n SinvT[l][n] Wbuf[n][j]
+//   AinvT[q][j] -= sum_l YT[q][l] W2[l][j]
+struct EpiY {
+    const int* plist; const int* mcount; int kp;
+    __device__ bool skip(int b) const { return mcount[b] == 0; }
+    __device__ void operator()(int b, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
+        if (row >= M || col >= N) return;
+        const int m = mcount[b];
+        const int* pl = plist + (long)b * kp;
+        v0 = (col < m) ? (v0 - ((pl[col] == row) ? 1.0 : 0.0)) : 0.0;
+        v1 = (col + 1 < m) ? (v1 - ((pl[col + 1] == row) ? 1.0 : 0.0)) : 0.0;
+        *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
+    }
+};
+struct EpiStoreSkip {
+    const int* mcount;
+    __device__ bool skip(int b) const { return mcount[b] == 0; }
+    __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
+        if (row < M && col < N) *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
+    }
+};
+struct EpiSubSkip {
+    const int* mcount;
+    __device__ bool skip(int b) const { return mcount[b] == 0; }
+    __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
+        if (row < M && col < N) {
+            double2* ptr = reinterpret_cast<double2*>(Cb + (long)row * ldc + col);
+            double2 c = *ptr;
+            c.x -= v0; c.y -= v1;
+            *ptr = c;
+        }
+    }
+};
+
+using CfgY16 = GemmCfg<128, 16, 16, 16, true, 4>;
+using CfgY32 = GemmCfg<128, 32, 16, 32, true, 4>;
+using CfgY64 = GemmCfg<128, 64, 32, 32, true, 4>;
+using CfgY128 = GemmCfg<128, 128, 64, 32, true, 4>;
+using CfgW2 = GemmCfg<64, 128, 32, 32, false, 3>;
+using CfgUpd = GemmCfg<128, 128, 64, 32, false, 3>;
+
+__global__ void k_window_reset(WalkDev wd) {
+    const int w = blockIdx.x;
+    double* Si = wd.SinvT + (long)w * wd.kp * wd.kp;
+    for (int i = threadIdx.x; i < wd.kp * wd.kp; i += blockDim.x) Si[i] = 0.0;
+    if (threadIdx.x == 0) wd.mcount[w] = 0;
+}
+
+cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st) {
+    k_window_reset<<<wd.W, 256, 0, st>>>(wd);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st) {
+    const int nsp = s.nsp[spin], kp = wd.kp;
+    cudaError_t e;
+    GemmArgs g;
+    // YT = AinvT0 * Vbuf^T
+    g.A = wd.AinvT[spin]; g.lda = nsp; g.strideA = (long)nsp * nsp;
+    g.B = wd.Vbuf; g.ldb = nsp; g.strideB = (long)kp * nsp;
+    g.C = wd.YT; g.ldc = kp; g.strideC = (long)nsp * kp;
+    g.M = nsp; g.N = kp; g.K = nsp;
+    EpiY ey{wd.plist, wd.mcount, kp};
+    if (kp <= 16) e = gemm_f64_launch<CfgY16>(g, wd.W, ey, st);
+    else if (kp <= 32) e = gemm_f64_launch<CfgY32>(g, wd.W, ey, st);
+    else if (kp <= 64) e = gemm_f64_launch<CfgY64>(g, wd.W, ey, st);
+    else e = gemm_f64_launch<CfgY128>(g, wd.W, ey, st);
+    COUNT_LAUNCH();
+    if (e != cudaSuccess) return e;
+    // W2 = SinvT * Wbuf
+    g.A = wd.SinvT; g.lda = kp; g.strideA = (long)kp * kp;
+    g.B = wd.Wbuf; g.ldb = nsp; g.strideB = (long)kp * nsp;
+    g.C = wd.W2; g.ldc = nsp; g.strideC = (long)kp * nsp;
+    g.M = kp; g.N = nsp; g.K = kp;
+    e = gemm_f64_launch<CfgW2>(g, wd.W, EpiStoreSkip{wd.mcount}, st);
+    COUNT_LAUNCH();
+    if (e != cudaSuccess) return e;
+    // AinvT -= YT * W2
+    g.A = wd.YT; g.lda = kp; g.strideA = (long)nsp * kp;
+    g.B = wd.W2; g.ldb = nsp; g.strideB = (long)kp * nsp;
+    g.C = wd.AinvT[spin]; g.ldc = nsp; g.strideC = (long)nsp * nsp;
+    g.M = nsp; g.N = nsp; g.K = kp;
+    e = gemm_f64_launch<CfgUpd>(g, wd.W, EpiSubSkip{wd.mcount}, st);
+    COUNT_LAUNCH();
+    if (e != cudaSuccess) return e;
+    return launch_window_reset(wd, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a9: local energy E_L = K + V                                                     [north_star item 6]
+// One warp per electron: 4 dots over the row caches, Jastrow gradient/laplacian and Coulomb sums over
+// partners with warp-shuffle reductions; then a fixed-order per-walker reduction.
+__global__ void __launch_bounds__(256) k_eloc_elec(SysDev s, WalkDev wd) {
+    const int w = blockIdx.y;
+    const int e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (e >= s.ne) return;
+    const int spin = e < s.ns[0] ? 0 : 1, p = spin ? e - s.ns[0] : e;
+    const int nsp = s.nsp[spin], nep = wd.nep;
+    const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
+    const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
+    double gx = 0, gy = 0, gz = 0, lp = 0;
+    for (int j = lane; j < nsp; j += 32) {
+        const double a = arow[j];
+        gx += orb[nsp + j] * a;
+        gy += orb[2 * nsp + j] * a;
+        gz += orb[3 * nsp + j] * a;
+        lp += orb[4 * nsp + j] * a;
+    }
+    const double* Rw = wd.R + (long)w * 3 * nep;
+    const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
+    double jx = 0, jy = 0, jz = 0, jl = 0, pot = 0;
+    const int npart = s.ne + s.n_atoms;
+    for (int k = lane; k < npart; k += 32) {
+        Partner P = partner(s, Rw, nep, e, k);
+        if (P.ok) {
+            const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
+            const double r = sqrt(dx * dx + dy * dy + dz * dz);
+            const double du = pade_du(P.a, P.b, r);
+            jx += du * dx / r; jy += du * dy / r; jz += du * dz / r;
+            jl += pade_d2u(P.a, P.b, r) + 2.0 * du / r;
+            if (k >= s.ne) pot += P.a / r;          // P.a = -Z_I
+            else if (k > e) pot += 1.0 / r;         // each pair once
+        }
+    }
+    gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz); lp = warp_sum(lp);
+    jx = warp_sum(jx); jy = warp_sum(jy); jz = warp_sum(jz); jl = warp_sum(jl); pot = warp_sum(pot);
+    if (lane == 0) {
+        const double g2 = gx * gx + gy * gy + gz * gz;
+        const double tx = gx + jx, ty = gy + jy, tz = gz + jz;
+        const double kin = lp - g2 + jl + (tx * tx + ty * ty + tz * tz);
+        wd.ebuf[((long)w * s.ne + e) * 2] = kin;
+        wd.ebuf[((long)w * s.ne + e) * 2 + 1] = pot;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_eloc_reduce(SysDev s, WalkDev wd) {
+    __shared__ double red[2 * 8];
+    const int w = blockIdx.x;
+    double a2[2] = {0, 0};
+    for (int e = threadIdx.x; e < s.ne; e += 256) {
+        a2[0] += wd.ebuf[((long)w * s.ne + e) * 2];
+        a2[1] += wd.ebuf[((long)w * s.ne + e) * 2 + 1];
+    }
+    block_sum<256, 2>(a2, red);
+    if (threadIdx.x == 0) {
+        const double K = -0.5 * a2[0];
+        wd.ekin[w] = K;
+        wd.eloc[w] = K + (a2[1] + s.e_nn);
+    }
+}
+
+cudaError_t launch_eloc(const SysDev& s, const WalkDev& wd, cudaStream_t st) {
+    dim3 grid((s.ne + 7) / 8, wd.W);
+    k_eloc_elec<<<grid, 256, 0, st>>>(s, wd);
+    COUNT_LAUNCH();
+    k_eloc_reduce<<<wd.W, 256, 0, st>>>(s, wd);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// walker creation helpers
+__global__ void k_gather_rp(WalkDev wd, int e) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= wd.W) return;
+    const double* Rw = wd.R + (long)w * 3 * wd.nep;
+    wd.rp[3 * w] = Rw[e]; wd.rp[3 * w + 1] = Rw[wd.nep + e]; wd.rp[3 * w + 2] = Rw[2 * wd.nep + e];
+}
+cudaError_t launch_gather_rp(const WalkDev& wd, int e, cudaStream_t st) {
+    k_gather_rp<<<(wd.W + 127) / 128, 128, 0, st>>>(wd, e);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// Orb[w][p][0..4][:] <- V[w][0..4][:], and the transposed Slater matrix T[j][p] = A[p][j] into AinvT
+__global__ void k_store_init_rows(SysDev s, WalkDev wd, int spin, int p) {
+    const int w = blockIdx.x, nsp = s.nsp[spin];
+    const double* v = wd.V + (long)w * 5 * wd.ldv;
+    double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
+    double* T = wd.AinvT[spin] + (long)w * nsp * nsp;
+    for (int j = threadIdx.x; j < nsp; j += blockDim.x) {
+        for (int c = 0; c < 5; c++) orb[c * nsp + j] = v[c * wd.ldv + j];
+        if (j < s.ns[spin]) T[(long)j * nsp + p] = v[j];
+    }
+}
+cudaError_t launch_store_init_rows(const SysDev& s, const WalkDev& wd, int spin, int p, cudaStream_t st) {
+    k_store_init_rows<<<wd.W, 256, 0, st>>>(s, wd, spin, p);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// In-place Gauss-Jordan inverse with partial (row) pivoting of the n x n leading block of each matrix;
+// one CTA per matrix.  logdet/sign accumulate over calls (one call per spin).
+template <int NT>
+__global__ void __launch_bounds__(NT) k_gj_inverse(double* Mall, long stride, int n, int ld, double* logdet, int* sign, int* status) {
+    extern __shared__ double gsm[];
+    double* rowk = gsm;               // [n]
+    double* colk = rowk + n;          // [n]
+    double* redv = colk + n;          // [NT/32]
+    int* redi = (int*)(redv + NT / 32);  // [NT/32]
+    int* perm = redi + NT / 32;       // [n]
+    __shared__ int s_piv;
+    __shared__ double s_pivval;
+    double* M = Mall + (long)blockIdx.x * stride;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double lad = 0.0;
+    int sg = 1;
+    for (int k = 0; k < n; k++) {
+        // pivot search: max |M[i][k]|, i >= k, lowest index on ties
+        double best = -1.0;
+        int bi = k;
+        for (int i = k + tid; i < n; i += NT) {
+            const double v = fabs(M[(long)i * ld + k]);
+            if (v > best) { best = v; bi = i; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+        }
+        if (lane == 0) { redv[warp] = best; redi[warp] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            double b = redv[0];
+            int r = redi[0];
+            for (int q = 1; q < NT / 32; q++)
+                if (redv[q] > b || (redv[q] == b && redi[q] < r)) { b = redv[q]; r = redi[q]; }
+            s_piv = r;
+            s_pivval = b;
+            perm[k] = r;
+        }
+        __syncthreads();
+        const int r = s_piv;
+        if (!(s_pivval > 0.0)) {  // singular (or NaN)
+            if (tid == 0) status[0] = -3;
+            return;
+        }
+        // swap rows k and r; build the scaled pivot row in shared memory
+        const double piv = M[(long)r * ld + k];
+        __syncthreads();  // everyone has read piv before row r is overwritten
+        const double pinv = 1.0 / piv;
+        for (int j = tid; j < n; j += NT) {
+            const double a = M[(long)r * ld + j];
+            if (r != k) M[(long)r * ld + j] = M[(long)k * ld + j];
+            const double v = (j == k ? 1.0 : a) * pinv;
+            rowk[j] = v;
+            M[(long)k * ld + j] = v;
+        }
+        __syncthreads();
+        for (int i = tid; i < n; i += NT) {
+            double f = 0.0;
+            if (i != k) { f = M[(long)i * ld + k]; M[(long)i * ld + k] = 0.0; }
+            colk[i] = f;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            lad += log(fabs(piv));
+            if (piv < 0.0) sg = -sg;
+            if (r != k) sg = -sg;
+        }
+        // eliminate: M[i][j] -= colk[i] * rowk[j], all i != k
+        for (int j = tid; j < n; j += NT) {
+            const double rk = rowk[j];
+#pragma unroll 4
+            for (int i = 0; i < n; i++) {
+                const double f = colk[i];
+                if (f != 0.0) M[(long)i * ld + j] -= f * rk;
+            }
+        }
+        __syncthreads();
+    }
+    // undo the row permutation as column swaps, in reverse order
+    for (int k = n - 1; k >= 0; k--) {
+        const int r = perm[k];
+        if (r != k) {
+            for (int i = tid; i < n; i += NT) {
+                const double a = M[(long)i * ld + k];
+                M[(long)i * ld + k] = M[(long)i * ld + r];
+                M[(long)i * ld + r] = a;
+            }
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        logdet[blockIdx.x] += lad;
+        sign[blockIdx.x] *= sg;
+    }
+}
+
+cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, cudaStream_t st) {
+    if (n == 0 || batch == 0) return cudaSuccess;
+    COUNT_LAUNCH();
+    if (n >= 512) {
+        constexpr int NT = 1024;
+        size_t smem = (size_t)(2 * n + NT / 32) * sizeof(double) + (size_t)(NT / 32 + n) * sizeof(int);
+        cudaFuncSetAttribute(k_gj_inverse<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        k_gj_inverse<NT><<<batch, NT, smem, st>>>(Mall, stride, n, ld, logdet, sign, status);
+    } else {
+        constexpr int NT = 256;
+        size_t smem = (size_t)(2 * n + NT / 32) * sizeof(double) + (size_t)(NT / 32 + n) * sizeof(int);
+        k_gj_inverse<NT><<<batch, NT, smem, st>>>(Mall, stride, n, ld, logdet, sign, status);
+    }
+    return cudaGetLastError();
+}
+
+// J(R) by direct sums (walker creation): one CTA per walker
+__global__ void __launch_bounds__(256) k_jastrow_total(SysDev s, WalkDev wd) {
+    __shared__ double red[8];
+    const int w = blockIdx.x, nep = wd.nep;
+    const double* Rw = wd.R + (long)w * 3 * nep;
+    const int npart = s.ne + s.n_atoms;
+    double a1[1] = {0.0};
+    for (long idx = threadIdx.x; idx < (long)s.ne * npart; idx += 256) {
+        const int i = (int)(idx / npart), k = (int)(idx % npart);
+        if (k < s.ne && k <= i) continue;
+        Partner P = partner(s, Rw, nep, i, k);
+        const double dx = Rw[i] - P.x, dy = Rw[nep + i] - P.y, dz = Rw[2 * nep + i] - P.z;
+        a1[0] += pade_u(P.a, P.b, sqrt(dx * dx + dy * dy + dz * dz));
+    }
+    block_sum<256, 1>(a1, red);
+    if (threadIdx.x == 0) wd.logpsi[w] += a1[0];
+}
+cudaError_t launch_jastrow_total(const SysDev& s, const WalkDev& wd, cudaStream_t st) {
+    k_jastrow_total<<<wd.W, 256, 0, st>>>(s, wd);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// nuclear repulsion sum_{I<J} Z_I Z_J / R_IJ (system constant), one CTA
+__global__ void __launch_bounds__(256) k_enn(SysDev s, double* out) {
+    __shared__ double red[8];
+    double a1[1] = {0.0};
+    const long n = (long)s.n_atoms * s.n_atoms;
+    for (long idx = threadIdx.x; idx < n; idx += 256) {
+        const int I = (int)(idx / s.n_atoms), J = (int)(idx % s.n_atoms);
+        if (J <= I) continue;
+        const double dx = s.atom_xyz[3 * I] - s.atom_xyz[3 * J], dy = s.atom_xyz[3 * I + 1] - s.atom_xyz[3 * J + 1],
+                     dz = s.atom_xyz[3 * I + 2] - s.atom_xyz[3 * J + 2];
+        a1[0] += s.atom_Z[I] * s.atom_Z[J] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+    block_sum<256, 1>(a1, red);
+    if (threadIdx.x == 0) out[0] = a1[0];
+}
+cudaError_t launch_enn(const SysDev& s, double* out, cudaStream_t st) {
+    k_enn<<<1, 256, 0, st>>>(s, out);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// layout conversion for the ABI
+__global__ void k_import_positions(WalkDev wd, const double* __restrict__ in /* [W][ne][3] */) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)wd.W * wd.ne) return;
+    const int w = (int)(idx / wd.ne), e = (int)(idx % wd.ne);
+    double* Rw = wd.R + (long)w * 3 * wd.nep;
+    Rw[e] = in[idx * 3]; Rw[wd.nep + e] = in[idx * 3 + 1]; Rw[2 * wd.nep + e] = in[idx * 3 + 2];
+}
+__global__ void k_export_positions(WalkDev wd, double* __restrict__ out) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)wd.W * wd.ne) return;
+    const int w = (int)(idx / wd.ne), e = (int)(idx % wd.ne);
+    const double* Rw = wd.R + (long)w * 3 * wd.nep;
+    out[idx * 3] = Rw[e]; out[idx * 3 + 1] = Rw[wd.nep + e]; out[idx * 3 + 2] = Rw[2 * wd.nep + e];
+}
+cudaError_t launch_import_positions(const WalkDev& wd, const double* in, cudaStream_t st) {
+    long n = (long)wd.W * wd.ne;
+    k_import_positions<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(wd, in);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_export_positions(const WalkDev& wd, double* out, cudaStream_t st) {
+    long n = (long)wd.W * wd.ne;
+    k_export_positions<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(wd, out);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_export_ainv(const double* __restrict__ AinvT, int W, int ns, int nsp, double* __restrict__ out) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long tot = (long)W * ns * ns;
+    if (idx >= tot) return;
+    const int j = (int)(idx % ns);
+    const long t = idx / ns;
+    const int p = (int)(t % ns), w = (int)(t / ns);
+    out[idx] = AinvT[((long)w * nsp + p) * nsp + j];
+}
+cudaError_t launch_export_ainv(const double* AinvT, int W, int ns, int nsp, double* out, cudaStream_t st) {
+    long n = (long)W * ns * ns;
+    if (n == 0) return cudaSuccess;
+    k_export_ainv<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(AinvT, W, ns, nsp, out);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_export_rows(const double* __restrict__ src, long n_rows, int width, long ld, double* __restrict__ out) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_rows * width) return;
+    out[idx] = src[(idx / width) * ld + idx % width];
+}
+cudaError_t launch_export_rows(const double* src, long n_rows, int width, long ld, double* out, cudaStream_t st) {
+    long n = n_rows * width;
+    if (n == 0) return cudaSuccess;
+    k_export_rows<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, n_rows, width, ld, out);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_pad_C(const double* __restrict__ in, int nb, int ns, double* __restrict__ out, int nsp) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)nb * ns) return;
+    out[(idx / ns) * nsp + idx % ns] = in[idx];
+}
+cudaError_t launch_pad_C(const double* in, int nb, int ns, double* out, int nsp, cudaStream_t st) {
+    long n = (long)nb * ns;
+    if (n == 0) return cudaSuccess;
+    k_pad_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, out, nsp);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_sign_to_i8(const int* __restrict__ in, int n, int8_t* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (int8_t)in[i];
+}
+cudaError_t launch_sign_to_i8(const int* in, int n, int8_t* out, cudaStream_t st) {
+    k_sign_to_i8<<<(n + 255) / 256, 256, 0, st>>>(in, n, out);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_fill_int(int* p, int n, int v) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+cudaError_t launch_fill_int(int* p, int n, int v, cudaStream_t st) {
+    k_fill_int<<<(n + 255) / 256, 256, 0, st>>>(p, n, v);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP64 ceiling: register-resident DMMA issue loop
+__global__ void k_dmma_peak(double* out, int iters, double a, double b) {
+    double c[8][2];
+#pragma unroll
+    for (int i = 0; i < 8; i++) { c[i][0] = threadIdx.x; c[i][1] = i; }
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++) dmma884(c[i][0], c[i][1], a, b);
+    }
+    double sacc = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) sacc += c[i][0] + c[i][1];
+    out[(long)blockIdx.x * blockDim.x + threadIdx.x] = sacc;
+}
+cudaError_t launch_dmma_peak(double* out, int grid, int threads, int iters, cudaStream_t st) {
+    k_dmma_peak<<<grid, threads, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+uint64_t launch_count() { return g_launches; }
+
+}  // namespace qmc

@@ -1,0 +1,29 @@
+// qmc_kernels.cuh -- launchers of the kernels in qmc_kernels.cu (host-side scheduler interface).
+#pragma once
+#include "qmc_internal.cuh"
+
+namespace qmc {
+
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* out, long ld, cudaStream_t st);
+cudaError_t launch_mo(const SysDev& s, int spin, const double* Phi, int rows, double* V, long ldv, cudaStream_t st);
+cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st);
+cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st);
+cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st);
+cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st);
+cudaError_t launch_eloc(const SysDev& s, const WalkDev& wd, cudaStream_t st);
+cudaError_t launch_gather_rp(const WalkDev& wd, int e, cudaStream_t st);
+cudaError_t launch_store_init_rows(const SysDev& s, const WalkDev& wd, int spin, int p, cudaStream_t st);
+cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, cudaStream_t st);
+cudaError_t launch_jastrow_total(const SysDev& s, const WalkDev& wd, cudaStream_t st);
+cudaError_t launch_import_positions(const WalkDev& wd, const double* in, cudaStream_t st);
+cudaError_t launch_export_positions(const WalkDev& wd, double* out, cudaStream_t st);
+cudaError_t launch_export_ainv(const double* AinvT, int W, int ns, int nsp, double* out, cudaStream_t st);
+cudaError_t launch_export_rows(const double* src, long n_rows, int width, long ld, double* out, cudaStream_t st);
+cudaError_t launch_pad_C(const double* in, int nb, int ns, double* out, int nsp, cudaStream_t st);
+cudaError_t launch_sign_to_i8(const int* in, int n, int8_t* out, cudaStream_t st);
+cudaError_t launch_fill_int(int* p, int n, int v, cudaStream_t st);
+cudaError_t launch_enn(const SysDev& s, double* out, cudaStream_t st);
+cudaError_t launch_dmma_peak(double* out, int grid, int threads, int iters, cudaStream_t st);
+uint64_t launch_count();
+
+}  // namespace qmc

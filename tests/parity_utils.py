@@ -1,0 +1,93 @@
+"""Comparison protocol GPU vs oracle (BASELINE.json north_star tolerances)."""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle
+import paper_2504_07948_b200 as qb
+
+TOL_RATIO = 1e-10      # ratios and log|Psi|, relative
+TOL_POS = 1e-10        # positions, absolute bohr (reading A27)
+TOL_AINV = 1e-9        # A^-1, relative Frobenius
+TOL_ELOC = 1e-9        # E_L, hartree
+
+
+def rel_frob(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def run_and_compare(wl, walker_ids, n_sweeps, delay_k, sweeps_per_call=1, threads=None, first_step=0, flags=qb.QMC_LOG_RATIOS,
+                    gsys=None, osys=None):
+    """Free-running comparison, walker by walker, sweep by sweep.
+
+    Returns a report dict; raises AssertionError on an unflagged accept/reject mismatch.  A decision that
+    differs with a tie flag on either side is flagged, not counted; the oracle walker is then re-seeded from
+    the GPU positions and the comparison continues."""
+    sysm = wl.system
+    walker_ids = list(walker_ids)
+    w0 = walker_ids[0]
+    assert walker_ids == list(range(w0, w0 + len(walker_ids)))
+    pos0 = wl.positions(w0, w0 + len(walker_ids))
+    gsys = gsys or qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(gsys, pos0, wl.seed, first_walker_id=w0, first_step=first_step, flags=flags)
+    osys = osys or oracle.OracleSystem(sysm)
+    ow = [osys.walker(p) for p in pos0]
+    rep = dict(n_moves=0, n_mismatch_flagged=0, n_resync=0, max_ratio_rel=0.0, max_pos_abs=0.0, max_logpsi_rel=0.0,
+               max_eloc_abs=0.0, max_ainv_rel=0.0, n_ties_gpu=0, n_ties_oracle=0, accept_frac=0.0, failures=[])
+    acc = 0
+    from concurrent.futures import ThreadPoolExecutor
+    nt = threads or oracle.default_threads()
+    for t in range(n_sweeps):
+        qb.qmc_sweep(gw, 1, wl.tau, delay_k)
+        gbits = qb.qmc_get_accept_log(gw).cpu().numpy()[0]          # [ne][W]
+        gratio, gpacc = [x.cpu().numpy()[0] for x in qb.qmc_get_ratio_log(gw)]
+        gpos = qb.qmc_get_positions(gw).cpu().numpy()
+        glog, gsign = [x.cpu().numpy() for x in qb.qmc_get_logpsi(gw)]
+        geloc, gekin = [x.cpu().numpy() for x in qb.qmc_get_eloc(gw)]
+
+        def one(n):
+            return ow[n].sweep(wl.seed, walker_ids[n], first_step + t, wl.tau)
+        if nt > 1 and len(ow) > 1:
+            with ThreadPoolExecutor(max_workers=nt) as ex:
+                res = list(ex.map(one, range(len(ow))))
+        else:
+            res = [one(n) for n in range(len(ow))]
+        for n, (obits, oratio, opacc) in enumerate(res):
+            gb = gbits[:, n]
+            rep["n_moves"] += len(gb)
+            rep["n_ties_gpu"] += int(((gb & 2) != 0).sum())
+            rep["n_ties_oracle"] += int(((obits & 2) != 0).sum())
+            acc += int((gb & 1).sum())
+            diff = np.nonzero((gb & 1) != (obits & 1))[0]
+            if len(diff):
+                i = int(diff[0])
+                if (gb[i] & 2) or (obits[i] & 2):
+                    rep["n_mismatch_flagged"] += 1
+                    rep["n_resync"] += 1
+                    ow[n].set_positions(gpos[n])   # re-seed the oracle from the GPU state
+                    continue
+                rep["failures"].append(dict(walker=walker_ids[n], sweep=t, electron=i, gpu_pacc=float(gpacc[i, n]),
+                                            oracle_pacc=float(opacc[i]), gpu_ratio=float(gratio[i, n]), oracle_ratio=float(oratio[i])))
+                ow[n].set_positions(gpos[n])
+                continue
+            m = oratio != 0
+            if m.any():
+                rep["max_ratio_rel"] = max(rep["max_ratio_rel"], float(np.max(np.abs(gratio[m, n] - oratio[m]) / np.abs(oratio[m]))))
+            rep["max_pos_abs"] = max(rep["max_pos_abs"], float(np.abs(gpos[n] - ow[n].positions()).max()))
+            ol, osg = ow[n].logpsi()
+            rep["max_logpsi_rel"] = max(rep["max_logpsi_rel"], abs(glog[n] - ol) / abs(ol))
+            assert int(gsign[n]) == osg
+            oe, ok = ow[n].eloc()
+            rep["max_eloc_abs"] = max(rep["max_eloc_abs"], abs(geloc[n] - oe))
+            rep.setdefault("eloc_scale", 0.0)
+            rep["eloc_scale"] = max(rep["eloc_scale"], abs(oe))
+    for spin in (0, 1):
+        if osys.ns(spin) == 0:
+            continue
+        ga = qb.qmc_get_Ainv(gw, spin).cpu().numpy()
+        for n in range(len(ow)):
+            rep["max_ainv_rel"] = max(rep["max_ainv_rel"], rel_frob(ga[n], ow[n].Ainv(spin)))
+    rep["accept_frac"] = acc / max(rep["n_moves"], 1)
+    rep["stats"] = qb.qmc_get_stats(gw)
+    rep["gw"], rep["gsys"], rep["ow"], rep["osys"] = gw, gsys, ow, osys
+    return rep
