@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- electron-moves/s of the batched Slater-Jastrow move on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands, on the host cores
+
+A "step" is ONE SWEEP of the whole hot path (rows a1-a9: drift, Philox proposal, basis, MO contraction,
+ratio + Jastrow, accept/reject, delayed-update flushes, local energy) over the crowd of the 256-water
+config (BASELINE.json configs[2]: 256 walkers x 2048 electrons, tau 0.005, delay_k 64) = 524,288 proposed
+moves per GPU.  N > 1: one process per GPU (torchrun), each with its own 256 walkers (global walker ids
+rank*256..) -- weak scaling, no data-path collective; time is the max over ranks.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the definitions of every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import qmc_inputs as qi  # noqa: E402
+
+METRIC, UNIT = "electron_moves_per_s", "moves/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--walkers", type=int, default=None, help="walkers per GPU (default: the config's)")
+    ap.add_argument("--delay-k", type=int, default=None)
+    ap.add_argument("--prof-stride", type=int, default=16, help="time the per-electron stages of every n-th electron")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-moves", type=int, default=96, help="electron moves per walker in the CPU-baseline sample")
+    return ap.parse_args()
+
+
+def workload_name(wl, walkers, k):
+    s = wl.system
+    return (f"configs[{wl.config}] {s.name}: {s.n_elec} electrons, {s.n_basis} GTOs, {walkers} walkers/GPU, "
+            f"tau {wl.tau}, delay_k {k}")
+
+
+def flop_model(sysm, n_moves, n_accepted):
+    """MO contraction 2*c*N_b*N_s per proposed move (c = 5) + 4*N_s^2 per accepted move."""
+    ns = sysm.n_up
+    return n_moves * 2.0 * 5 * sysm.n_basis * ns + n_accepted * 4.0 * ns * ns
+
+
+# ---------------------------------------------------------------------------------------- clocks
+
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "200"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---------------------------------------------------------------------------------------- CPU oracle legs
+
+def oracle_sample(wl, n_steps, n_warm, moves_per_step, walkers=None):
+    """Time the oracle (as it stands) on the host cores: `cores` walkers in parallel, each doing
+    moves_per_step electron moves of sweep 0 per step, continuing along the sweep.  Walker creation
+    (all orbital rows + LU inverse) is not timed."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    cores = oracle.default_threads()
+    nw = walkers or cores
+    osys = oracle.OracleSystem(wl.system)
+    pos = wl.positions(0, nw)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        ws = list(ex.map(lambda p: osys.walker(p), pos))
+    t_init = time.perf_counter() - t0
+    ne = wl.system.n_elec
+    times = []
+    e = 0
+    for s in range(n_warm + n_steps):
+        lo, hi = e % ne, min(e % ne + moves_per_step, ne)
+        t0 = time.perf_counter()
+        with ThreadPoolExecutor(max_workers=cores) as ex:
+            list(ex.map(lambda a: a[1].sweep_range(wl.seed, a[0], 0, wl.tau, lo, hi), enumerate(ws)))
+        dt = time.perf_counter() - t0
+        if s >= n_warm:
+            times.append((dt, (hi - lo) * nw))
+        e += hi - lo
+    tot_t = sum(t for t, _ in times)
+    tot_m = sum(m for _, m in times)
+    return dict(value=tot_m / tot_t, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{nw} walkers x {moves_per_step} electron moves x {n_steps} steps of sweep 0 "
+                       f"(walker creation, {t_init:.1f} s, not timed)"), tot_t / max(len(times), 1)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = qi.make_workload(args.config)
+    k = args.delay_k or wl.delay_k
+    cb, s_per_step = oracle_sample(wl, args.steps, args.warmup, args.cpu_moves)
+    line = dict(metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=s_per_step * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference",
+                config=dict(workload=workload_name(wl, args.walkers or wl.n_walkers, k),
+                            note="each step is a bounded sample of the workload, see cpu_baseline.sample"),
+                cpu_baseline=cb,
+                e2e=dict(value=cb["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------- this repo's arm
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2504_07948_b200 import build as qbuild
+    from paper_2504_07948_b200.sharding import dist_env, reduce_report, walker_slice
+    rank, local_rank, world = dist_env()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", init_method="env://", device_id=torch.device("cuda", local_rank))
+    if local_rank == 0:
+        qbuild.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2504_07948_b200 as qb
+    qb.load_library()
+
+    wl = qi.make_workload(args.config)
+    sysm = wl.system
+    W = args.walkers or wl.n_walkers
+    k = args.delay_k or wl.delay_k
+    lo, hi = walker_slice(W, rank)
+    pos_host = torch.from_numpy(qi.initial_positions(sysm, wl.config, range(lo, hi), wl.seed)).pin_memory()
+    gsys = qb.qmc_init_from(sysm)
+    peak = qb.qmc_measure_fp64_peak(300.0)
+
+    # ---- device-resident run: inputs already in HBM when the timed region starts
+    pos_dev = pos_host.cuda()
+    gw = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo)
+    for _ in range(args.warmup):
+        qb.qmc_sweep(gw, 1, wl.tau, k)
+    qb.qmc_synchronize(gw)
+    st0 = qb.qmc_get_stats(gw)
+    qb.qmc_set_profiling(gw, args.prof_stride)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = qb.qmc_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0.record()
+    qb.qmc_sweep(gw, args.steps, wl.tau, k)   # EXACTLY K steps (sweeps), enqueued on torch's current stream
+    ev1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = qb.qmc_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    stage = qb.qmc_get_stage_times(gw)
+    qb.qmc_set_profiling(gw, 0)
+    st1 = qb.qmc_get_stats(gw)
+    eloc = qb.qmc_get_eloc(gw)[0]
+    n_moves = st1["proposed"] - st0["proposed"]
+    n_acc = st1["accepted"] - st0["accepted"]
+    assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
+    assert st1["nonfinite"] == 0
+    red = reduce_report(ms, n_moves, float(eloc.sum()), float((eloc * eloc).sum()), W, backend_device="cuda")
+    qb.qmc_walkers_destroy(gw)
+
+    # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps
+    e2e = None
+    if not args.no_e2e:
+        ne = sysm.n_elec
+        out_pos = torch.empty((W, ne, 3), dtype=torch.float64).pin_memory()
+        out_e, out_k, out_l = [torch.empty(W, dtype=torch.float64).pin_memory() for _ in range(3)]
+        out_s = torch.empty(W, dtype=torch.int8).pin_memory()
+        out_b = torch.empty((args.steps, ne, W), dtype=torch.uint8).pin_memory()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        gw2 = qb.qmc_walkers_create(gsys, pos_host, wl.seed, first_walker_id=lo)     # H2D of the positions inside
+        qb.qmc_sweep(gw2, args.steps, wl.tau, k)
+        qb.qmc_get_positions(gw2, out=out_pos)                                        # D2H, synchronous
+        qb.qmc_get_eloc(gw2, out=out_e, out_kin=out_k)
+        qb.qmc_get_logpsi(gw2, out=out_l, out_sign=out_s)
+        qb.qmc_get_accept_log(gw2, out=out_b)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) * 1e3
+        qb.qmc_walkers_destroy(gw2)
+        red2 = reduce_report(t_e2e, W * ne * args.steps, 0.0, 0.0, W, backend_device="cuda")
+        d2h = out_pos.numel() * 8 + 3 * W * 8 + W + out_b.numel()
+        e2e = dict(value=red2["n_moves"] / (red2["elapsed_ms"] * 1e-3), unit=UNIT,
+                   h2d_bytes_per_step=pos_host.numel() * 8 // args.steps, d2h_bytes_per_step=d2h // args.steps,
+                   ms_total=red2["elapsed_ms"],
+                   what="qmc_walkers_create from pinned host positions (orbital rows + inverse of all Slater matrices) "
+                        f"+ qmc_sweep({args.steps}) + qmc_get_{{positions,eloc,logpsi,accept_log}} into pinned host buffers")
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    secs = red["elapsed_ms"] * 1e-3
+    value = red["n_moves"] / secs
+    ns, nb = sysm.n_up, sysm.n_basis
+    mo_ms, mo_n = stage["mo"]
+    mo_avg_ms = mo_ms / max(mo_n, 1)
+    mo_flop = 2.0 * 5 * W * nb * ns
+    achieved = mo_flop / (mo_avg_ms * 1e-3) * 1e-12 if mo_n else None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "mo_kernel_traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(f"config{wl.config}_W{W}")
+        except (OSError, ValueError):
+            traffic = None
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        pass
+    share = {s: stage[s][0] * (args.prof_stride if s in ("propose", "basis", "mo", "accept") else 1.0) for s in stage}
+    tot_share = sum(share.values()) or 1.0
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+        ms_per_step=red["elapsed_ms"] / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+        dtype="f64", data="synthetic",
+        config=dict(workload=workload_name(wl, W, k), step="one sweep = one proposed move per electron per walker",
+                    moves_per_step=W * sysm.n_elec * world, l2="per-step working set (A^-1 + row caches, ~25 GB/GPU) >> 126 MB L2; no flush needed",
+                    prof_stride=args.prof_stride),
+        clocks=clocks, e2e=e2e, gpu_launches=int(launches),
+        roofline=dict(kernel="gemm_f64_kernel (MO contraction V = Phi*C, DMMA m8n8k4)", bound="tensor", achieved=achieved,
+                      peak=peak, unit="TFLOP/s", frac=(achieved / peak) if achieved else None, traffic=traffic,
+                      peak_source="FP64 DMMA issue-rate loop measured in this run (qmc_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                      peak_alt_bf16_scaled=(peaks.get("bf16_tflops_sustained", 0) * 37.2 / 2250.0) or None,
+                      flop_per_launch=mo_flop, ms_per_launch=mo_avg_ms, launches_timed=int(mo_n),
+                      share_of_step=share["mo"] / tot_share),
+        fp64_tflops_model=flop_model(sysm, red["n_moves"], n_acc * world) / secs * 1e-12,
+        accept_frac=n_acc / max(n_moves, 1),
+        stage_ms_per_launch={s: (stage[s][0] / stage[s][1] if stage[s][1] else None) for s in stage},
+        stage_share={s: share[s] / tot_share for s in share},
+        eloc_mean=red["e_sum"] / red["n_walkers"],
+    )
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_sample(wl, 3, 1, args.cpu_moves)[0]
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -86,6 +86,8 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_get_logpsi.argtypes = [C.c_void_p, _dp, _ip]
     lib.oracle_walker_sweep.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                         _u8p, _dp, _dp]
+    lib.oracle_walker_sweep_range.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
+                                              C.c_int, C.c_int, _u8p, _dp, _dp]
     lib.oracle_walker_eloc.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
     lib.oracle_delayed_update.restype = C.c_int
     lib.oracle_delayed_update.argtypes = [C.c_int, _dp, C.c_int, _ip, _dp, _dp, _dp]
@@ -235,6 +237,16 @@ class OracleWalker:
         pacc = np.zeros(ne)
         self.lib.oracle_walker_sweep(self.sys.h, self.h, seed, walker_id, step, tau, bits.ctypes.data_as(_u8p),
                                      _d(ratio), _d(pacc))
+        return bits, ratio, pacc
+
+    def sweep_range(self, seed, walker_id, step, tau, e_begin, e_end):
+        """Electrons e_begin..e_end-1 of a sweep only (bounded sample for timing)."""
+        ne = self.sys.n_elec
+        bits = np.zeros(ne, np.uint8)
+        ratio = np.zeros(ne)
+        pacc = np.zeros(ne)
+        self.lib.oracle_walker_sweep_range(self.sys.h, self.h, seed, walker_id, step, tau, int(e_begin), int(e_end),
+                                           bits.ctypes.data_as(_u8p), _d(ratio), _d(pacc))
         return bits, ratio, pacc
 
     def eloc(self):

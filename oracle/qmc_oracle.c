@@ -243,13 +243,13 @@ void oracle_basis_eval(const oracle_system *s, const double r[3], double *phi, d
  * v_j = sum_l C_lj Phi_l(r), same for the three gradient components and the Laplacian
  * (PAPER.md L127).  out = [5][n_s]: value, d/dx, d/dy, d/dz, laplacian. */
 
-static void mo_rows(const oracle_system *s, int spin, const real r[3], real *out, real *scratch /*[5*n_basis]*/) {
+static void mo_rows(const oracle_system *s, int spin, const real r[3], real *restrict out, real *restrict scratch /*[5*n_basis]*/) {
     int nb = s->n_basis, ns = spin == 0 ? s->n_up : s->n_dn;
-    const real *C = s->C[spin];
+    const real *restrict C = s->C[spin];
     basis_eval(s, r, scratch, scratch + nb, scratch + 4 * nb);
     for (int i = 0; i < 5 * ns; i++) out[i] = 0;
     for (int l = 0; l < nb; l++) {
-        const real *Cl = C + (size_t)l * ns;
+        const real *restrict Cl = C + (size_t)l * ns;
         real b0 = scratch[l], b1 = scratch[nb + l], b2 = scratch[2 * nb + l], b3 = scratch[3 * nb + l], b4 = scratch[4 * nb + l];
         for (int j = 0; j < ns; j++) {
             out[j] += Cl[j] * b0;
@@ -303,8 +303,8 @@ static int lu_inverse(int n, const real *A, real *Ainv, real *logabsdet, int *si
         for (int i = k + 1; i < n; i++) {
             real f = LU[(size_t)i * n + k] / d;
             LU[(size_t)i * n + k] = f;
-            real *ri = LU + (size_t)i * n;
-            const real *rk = LU + (size_t)k * n;
+            real *restrict ri = LU + (size_t)i * n;
+            const real *restrict rk = LU + (size_t)k * n;
             for (int j = k + 1; j < n; j++) ri[j] -= f * rk[j];
         }
     }
@@ -316,16 +316,16 @@ static int lu_inverse(int n, const real *A, real *Ainv, real *logabsdet, int *si
         for (int k = 0; k < i; k++) {
             real f = LU[(size_t)i * n + k];
             if (f != 0) {
-                real *xi = X + (size_t)i * n;
-                const real *xk = X + (size_t)k * n;
+                real *restrict xi = X + (size_t)i * n;
+                const real *restrict xk = X + (size_t)k * n;
                 for (int j = 0; j < n; j++) xi[j] -= f * xk[j];
             }
         }
     for (int i = n - 1; i >= 0; i--) { /* backward */
-        real *xi = X + (size_t)i * n;
+        real *restrict xi = X + (size_t)i * n;
         for (int k = i + 1; k < n; k++) {
             real f = LU[(size_t)i * n + k];
-            const real *xk = X + (size_t)k * n;
+            const real *restrict xk = X + (size_t)k * n;
             for (int j = 0; j < n; j++) xi[j] -= f * xk[j];
         }
         real d = LU[(size_t)i * n + i];
@@ -517,13 +517,15 @@ void oracle_walker_get_logpsi(const oracle_walker *w, double *logabs, int *sign)
 
 /* ------------------------------------------------------------------ one sweep
  * bits[i]: 1 = accepted, 2 = tie-flagged (A19).  ratio[i] = rho_D * exp(dJ), pacc[i] = p_acc
- * (0 when rejected by the fixed-node test).  Any of the log pointers may be NULL. */
+ * (0 when rejected by the fixed-node test).  Any of the log pointers may be NULL.
+ * The _range form runs electrons e_begin..e_end-1 only (a full sweep is 0..n_e); it exists so that a
+ * bounded sample of a sweep can be timed. */
 
-void oracle_walker_sweep(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
-                         uint32_t step, double tau_d, uint8_t *bits, double *ratio, double *pacc) {
+void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                               uint32_t step, double tau_d, int e_begin, int e_end, uint8_t *bits, double *ratio,
+                               double *pacc) {
     real tau = (real)tau_d, sqrt_tau = R_SQRT(tau);
-    int ne = w->ne;
-    for (int i = 0; i < ne; i++) {
+    for (int i = e_begin; i < e_end; i++) {
         int sp = spin_of(s, i), ns = sp == 0 ? s->n_up : s->n_dn, p = sp == 0 ? i : i - s->n_up;
         real *Ainv = w->Ainv[sp];
         real *orbp = w->orb[sp] + (size_t)p * 5 * ns;
@@ -597,6 +599,11 @@ void oracle_walker_sweep(const oracle_system *s, oracle_walker *w, uint64_t seed
         if (ratio) ratio[i] = (double)jr;
         if (pacc) pacc[i] = (double)pa;
     }
+}
+
+void oracle_walker_sweep(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                         uint32_t step, double tau_d, uint8_t *bits, double *ratio, double *pacc) {
+    oracle_walker_sweep_range(s, w, seed, walker_id, step, tau_d, 0, w->ne, bits, ratio, pacc);
 }
 
 /* ------------------------------------------------------------------ local energy (A9)

@@ -332,3 +332,7 @@ def qmc_launch_count() -> int:
 
 def qmc_version() -> str:
     return load_library().qmc_version().decode()
+
+
+def qmc_last_error() -> str:
+    return load_library().qmc_last_error().decode()

@@ -1,0 +1,224 @@
+// mo_streamk.cuh -- the MO contraction V = Phi * C_s as a persistent, warp-specialised, stream-K FP64
+// tensor-core GEMM for sm_100a (BASELINE.json north_star item 2).
+//
+// Why this shape.  The contraction is skinny (M = 5 W rows, N = N_s, K = N_b): 128x128 output tiles give
+// 80 CTAs at the 256-water config, 54 % of 148 SMs.  Stream-K instead cuts the flattened (tile, k-block)
+// iteration space into 148 equal contiguous ranges, one persistent CTA per SM; a tile whose k-range is
+// split over 2-3 CTAs is summed by the CTA that holds its first k-block, in ascending k order
+// (deterministic: no atomics), from partial accumulators parked in an L2-resident workspace.
+//
+// Operand staging.  Both operands live in HBM already in the shape of a shared-memory stage:
+//   PhiT [MT][KB][128][36]   (A tile of 128 rows x 32 k, rows padded to 36 doubles)
+//   CT   [NT][KB][32][132]   (B tile of 32 k x 128 n, rows padded to 132 doubles)
+// so one stage is two contiguous blocks (36,864 B + 33,792 B) that a single producer thread fetches with
+// two TMA bulk copies (cp.async.bulk -> SASS UBLKCP) completing on an mbarrier; the row padding makes
+// every DMMA fragment load conflict free (a half warp covers 4 rows x 32 B = one 128 B wavefront).
+// Eight consumer warps (2 x 4, warp tile 64 x 32 = 32 DMMA m8n8k4 accumulators) never meet a block-wide
+// barrier in the main loop: full/empty mbarriers only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gemm_f64.cuh"
+
+namespace qmc {
+
+constexpr int MO_BM = 128, MO_BN = 128, MO_BK = 32;
+constexpr int MO_ALD = 36, MO_BLD = 132;
+constexpr int MO_A_STAGE = MO_BM * MO_ALD;   // doubles
+constexpr int MO_B_STAGE = MO_BK * MO_BLD;   // doubles
+constexpr int MO_STAGES = 3;
+constexpr int MO_CONSUMER_WARPS = 8;
+constexpr int MO_THREADS = (MO_CONSUMER_WARPS + 1) * 32;
+constexpr size_t MO_SMEM_BYTES = (size_t)MO_STAGES * (MO_A_STAGE + MO_B_STAGE) * 8 + 2 * MO_STAGES * 8 + 16;
+constexpr int MO_TM = 8, MO_TN = 4;  // DMMA tiles per warp (64 x 32)
+constexpr int MO_WS_DOUBLES = MO_BM * MO_BN;  // workspace per CTA
+
+__host__ __device__ inline long phiT_index(long row, int f, int KB) {
+    return (((row >> 7) * KB + (f >> 5)) * MO_BM + (row & 127)) * MO_ALD + (f & 31);
+}
+__host__ __device__ inline long cT_index(int l, int j, int KB) {
+    return ((((long)(j >> 7)) * KB + (l >> 5)) * MO_BK + (l & 31)) * MO_BLD + (j & 127);
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;\n" ::"n"(MO_CONSUMER_WARPS * 32) : "memory"); }
+
+struct MoArgs {
+    const double* PhiT;  // [MT][KB][128][36]
+    const double* CT;    // [NT][KB][32][132]
+    double* V;           // [M][ldv] row-major
+    long ldv;
+    int M, N;            // valid rows / columns of V
+    int MT, NT, KB;
+    double* ws;          // [grid][128*128] partial accumulators
+    unsigned* flags;     // [grid] epoch stamps
+    unsigned epoch;
+};
+
+__global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
+    extern __shared__ __align__(128) unsigned char mo_smem_raw[];
+    double* stages = reinterpret_cast<double*>(mo_smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(stages + (size_t)MO_STAGES * (MO_A_STAGE + MO_B_STAGE));
+    uint64_t* empty = full + MO_STAGES;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < MO_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], MO_CONSUMER_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+
+    const long total = (long)g.MT * g.NT * g.KB;
+    const long it0 = total * blockIdx.x / gridDim.x, it1 = total * (blockIdx.x + 1) / gridDim.x;
+    constexpr uint32_t STAGE_BYTES = (MO_A_STAGE + MO_B_STAGE) * 8;
+
+    if (warp == MO_CONSUMER_WARPS) {
+        // ===== producer: one thread streams the stages of this CTA's iteration range =====
+        if (lane == 0) {
+            uint32_t n = 0;
+            for (long it = it0; it < it1; it++, n++) {
+                const int s = n % MO_STAGES;
+                const uint32_t round = n / MO_STAGES;
+                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
+                const long tile = it / g.KB;
+                const int kb = (int)(it - tile * g.KB);
+                const int tm = (int)(tile / g.NT), tn = (int)(tile - (long)tm * g.NT);
+                double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
+                mbar_expect_tx(&full[s], STAGE_BYTES);
+                bulk_g2s(As, g.PhiT + ((long)tm * g.KB + kb) * MO_A_STAGE, MO_A_STAGE * 8, &full[s]);
+                bulk_g2s(As + MO_A_STAGE, g.CT + ((long)tn * g.KB + kb) * MO_B_STAGE, MO_B_STAGE * 8, &full[s]);
+            }
+        }
+        return;
+    }
+
+    // ===== consumers =====
+    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * 32;
+    const int lr = lane >> 2, lc = lane & 3;
+    uint32_t n = 0;
+    long it = it0;
+    while (it < it1) {
+        const long tile = it / g.KB;
+        const int ka = (int)(it - tile * g.KB);
+        const long rem = it1 - it;
+        const int kb_end = (rem < (long)(g.KB - ka)) ? (int)(ka + rem) : g.KB;
+        const int tm = (int)(tile / g.NT), tn = (int)(tile - (long)tm * g.NT);
+        double acc[MO_TM][MO_TN][2];
+#pragma unroll
+        for (int i = 0; i < MO_TM; i++)
+#pragma unroll
+            for (int j = 0; j < MO_TN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int kb = ka; kb < kb_end; kb++, n++) {
+            const int s = n % MO_STAGES;
+            mbar_wait(&full[s], (n / MO_STAGES) & 1);
+            const double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
+            const double* Bs = As + MO_A_STAGE;
+#pragma unroll
+            for (int kk = 0; kk < MO_BK / 4; kk++) {
+                double af[MO_TM], bf[MO_TN];
+#pragma unroll
+                for (int i = 0; i < MO_TM; i++) af[i] = As[(wm0 + i * 8 + lr) * MO_ALD + kk * 4 + lc];
+#pragma unroll
+                for (int j = 0; j < MO_TN; j++) bf[j] = Bs[(kk * 4 + lc) * MO_BLD + wn0 + j * 8 + lr];
+#pragma unroll
+                for (int i = 0; i < MO_TM; i++)
+#pragma unroll
+                    for (int j = 0; j < MO_TN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+        it += kb_end - ka;
+
+        // ---- epilogue of this segment
+        const bool head = (ka == 0), whole = head && (kb_end == g.KB);
+        if (!head) {
+            // park the partial tile for the owner (CTA with the tile's first k-block), then publish
+            double* ws = g.ws + (size_t)blockIdx.x * MO_WS_DOUBLES;
+#pragma unroll
+            for (int i = 0; i < MO_TM; i++)
+#pragma unroll
+                for (int j = 0; j < MO_TN; j++) {
+                    ws[((i * MO_TN + j) * 2 + 0) * 256 + tid] = acc[i][j][0];
+                    ws[((i * MO_TN + j) * 2 + 1) * 256 + tid] = acc[i][j][1];
+                }
+            __threadfence();
+            consumer_bar();
+            if (tid == 0) {
+                asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(g.flags + blockIdx.x), "r"(g.epoch) : "memory");
+            }
+        } else {
+            if (!whole) {
+                // owner: add the partials of the CTAs that hold the rest of this tile, in ascending k order
+                long covered = (tile * g.KB + kb_end);  // first iteration not yet summed
+                const long tile_end = (tile + 1) * g.KB;
+                int peer = blockIdx.x + 1;
+                while (covered < tile_end) {
+                    if (tid == 0) {
+                        unsigned v;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(g.flags + peer) : "memory");
+                            if (v != g.epoch) __nanosleep(64);
+                        } while (v != g.epoch);
+                    }
+                    consumer_bar();
+                    const double* ws = g.ws + (size_t)peer * MO_WS_DOUBLES;
+#pragma unroll
+                    for (int i = 0; i < MO_TM; i++)
+#pragma unroll
+                        for (int j = 0; j < MO_TN; j++) {
+                            acc[i][j][0] += __ldcg(ws + ((i * MO_TN + j) * 2 + 0) * 256 + tid);
+                            acc[i][j][1] += __ldcg(ws + ((i * MO_TN + j) * 2 + 1) * 256 + tid);
+                        }
+                    const long peer_end = total * (peer + 1) / gridDim.x;
+                    covered = peer_end < tile_end ? peer_end : tile_end;
+                    peer++;
+                }
+            }
+            const int m0 = tm * MO_BM, n0 = tn * MO_BN;
+#pragma unroll
+            for (int i = 0; i < MO_TM; i++) {
+                const int row = m0 + wm0 + i * 8 + lr;
+#pragma unroll
+                for (int j = 0; j < MO_TN; j++) {
+                    const int col = n0 + wn0 + j * 8 + lc * 2;
+                    if (row < g.M && col < g.N) *reinterpret_cast<double2*>(g.V + (long)row * g.ldv + col) = make_double2(acc[i][j][0], acc[i][j][1]);
+                }
+            }
+        }
+    }
+}
+
+}  // namespace qmc

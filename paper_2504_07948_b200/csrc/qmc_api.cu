@@ -57,6 +57,7 @@ struct qmc_system {
     DevPool pool;
     cudaStream_t stream;
     int device;
+    int n_sm;
 };
 
 struct StageTimer {
@@ -76,6 +77,7 @@ struct qmc_walkers {
     uint32_t flags;
     int T_last;          // sweeps in the most recent qmc_sweep call
     int* d_status;
+    unsigned mo_epoch;   // stream-K launch counter (flag stamps)
     int prof_stride;     // 0 = off
     StageTimer timer;
     double stage_ms[8];
@@ -147,9 +149,11 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     cudaGetDevice(&S->device);
     SysDev& d = S->d;
     memset(&d, 0, sizeof(d));
-    d.n_atoms = atoms->n_atoms; d.n_shells = basis->n_shells; d.n_basis = mo->n_basis; d.nbp = round_up(mo->n_basis, 16);
+    d.n_atoms = atoms->n_atoms; d.n_shells = basis->n_shells; d.n_basis = mo->n_basis; d.nbp = round_up(mo->n_basis, 32); d.kb = d.nbp / 32;
     d.ns[0] = mo->n_up; d.ns[1] = mo->n_dn; d.nsp[0] = round_up(mo->n_up, 16); d.nsp[1] = round_up(mo->n_dn, 16);
+    d.nt[0] = (d.nsp[0] + 127) / 128; d.nt[1] = (d.nsp[1] + 127) / 128;
     d.ne = mo->n_up + mo->n_dn;
+    cudaDeviceGetAttribute(&S->n_sm, cudaDevAttrMultiProcessorCount, S->device);
     d.a_anti = jas->a_anti; d.a_para = jas->a_para; d.b_ee = jas->b_ee; d.b_en = jas->b_en;
     auto cleanup = [&](int code, const std::string& m) { S->pool.free_all(); delete S; return fail(code, m); };
 #define CUS(call)                                                                                       \
@@ -173,15 +177,15 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     d.atom_xyz = dxyz; d.atom_Z = dZ; d.alpha = dal; d.coef = dco; d.shells = drec;
     for (int sp = 0; sp < 2; sp++) {
         double* dC;
-        CUS(S->pool.alloc((void**)&dC, (size_t)d.nbp * d.nsp[sp] * 8, st));
-        d.C[sp] = dC;
+        CUS(S->pool.alloc((void**)&dC, (size_t)d.nt[sp] * d.kb * 32 * 132 * 8, st));
+        d.CT[sp] = dC;
         const double* src = sp == 0 ? mo->C_up : mo->C_dn;
         if (d.ns[sp] > 0) {
-            double* tmp;  // stage (host or device source) -> device, then pad on the device
+            double* tmp;  // stage (host or device source) -> device, then tile on the device
             size_t bytes = (size_t)d.n_basis * d.ns[sp] * 8;
             CUS(cudaMalloc((void**)&tmp, bytes));
             cudaError_t e = cudaMemcpyAsync(tmp, src, bytes, cudaMemcpyDefault, st);
-            if (e == cudaSuccess) e = launch_pad_C(tmp, d.n_basis, d.ns[sp], dC, d.nsp[sp], st);
+            if (e == cudaSuccess) e = launch_tile_C(tmp, d.n_basis, d.ns[sp], dC, d.kb, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             cudaFree(tmp);
             CUS(e);
@@ -274,7 +278,12 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         CUW(w->pool.alloc((void**)&d.AinvT[sp], W * s.nsp[sp] * s.nsp[sp] * 8, st));
         CUW(w->pool.alloc((void**)&d.Orb[sp], W * s.nsp[sp] * 5 * s.nsp[sp] * 8, st));
     }
-    CUW(w->pool.alloc((void**)&d.Phi, W * 5 * s.nbp * 8, st));
+    d.mt = (5 * n_walkers + 127) / 128;
+    CUW(w->pool.alloc((void**)&d.Phi, phiT_bytes(s, 5 * n_walkers), st));
+    d.mo_grid = sys->n_sm;
+    CUW(w->pool.alloc((void**)&d.mo_ws, mo_ws_bytes(sys->n_sm), st));
+    CUW(w->pool.alloc((void**)&d.mo_flags, (size_t)sys->n_sm * 4, st));
+    w->mo_epoch = 0;
     CUW(w->pool.alloc((void**)&d.V, W * 5 * d.ldv * 8, st));
     CUW(w->pool.alloc((void**)&d.xcol, W * d.ldv * 8, st));
     CUW(w->pool.alloc((void**)&d.mcount, W * 4, st));
@@ -311,8 +320,8 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         const int e0 = sp == 0 ? 0 : s.ns[0];
         for (int p = 0; p < s.ns[sp]; p++) {
             CUW(launch_gather_rp(d, e0 + p, st));
-            CUW(launch_basis(s, d.rp, n_walkers, d.Phi, s.nbp, st));
-            CUW(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, st));
+            CUW(launch_basis(s, d.rp, n_walkers, d.Phi, st));
+            CUW(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * n_walkers, d.mo_grid), ++w->mo_epoch, st));
             CUW(launch_store_init_rows(s, d, sp, p, st));
         }
         CUW(launch_gj_inverse(d.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp], s.ns[sp], s.nsp[sp], n_walkers, d.logpsi, d.sign, w->d_status, st));
@@ -423,10 +432,10 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
                 CU(launch_propose(s, d, sp, p, e, w->step, tau, st));
                 prof_end(w, prof);
                 prof_begin(w, 1, prof);
-                CU(launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st));
+                CU(launch_basis(s, d.rp, d.W, d.Phi, st));
                 prof_end(w, prof);
                 prof_begin(w, 2, prof);
-                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, st));
+                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch, st));
                 prof_end(w, prof);
                 prof_begin(w, 3, prof);
                 CU(launch_accept(s, d, sp, p, e, log_off, tau, 1, st));
@@ -546,35 +555,41 @@ extern "C" int qmc_synchronize(const qmc_walkers* w) {
 // ------------------------------------------------------------------------------------------------ stage-level entry points
 
 static int eval_common(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream, bool mo) {
-    if (!sys || !xyz || !out || n_points < 0 || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_eval_*: bad argument");
+    if (!sys || n_points < 0 || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_eval_*: bad argument");
+    if (n_points == 0) return QMC_OK;
+    if (!xyz || !out) return fail(QMC_ERR_ARG, "qmc_eval_*: null buffer");
     int rc = check_device();
     if (rc) return rc;
-    if (n_points == 0) return QMC_OK;
     const SysDev& s = sys->d;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    double *pts = nullptr, *Phi = nullptr, *V = nullptr, *stage = nullptr;
+    double *pts = nullptr, *Phi = nullptr, *V = nullptr, *stage = nullptr, *ws = nullptr;
+    unsigned* flags = nullptr;
+    const int grid = mo ? mo_grid_for(s, spin, 5 * n_points, sys->n_sm) : 0;
     const int width = mo ? s.ns[spin] : s.n_basis;
     const size_t out_bytes = (size_t)n_points * 5 * width * 8;
     cudaError_t e = cudaMalloc((void**)&pts, (size_t)n_points * 3 * 8);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&Phi, (size_t)n_points * 5 * s.nbp * 8);
-    if (e == cudaSuccess) e = cudaMemsetAsync(Phi, 0, (size_t)n_points * 5 * s.nbp * 8, st);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&Phi, phiT_bytes(s, 5 * n_points));
+    if (e == cudaSuccess) e = cudaMemsetAsync(Phi, 0, phiT_bytes(s, 5 * n_points), st);
     if (e == cudaSuccess && mo) e = cudaMalloc((void**)&V, (size_t)n_points * 5 * s.nsp[spin] * 8 + 16);
+    if (e == cudaSuccess && mo) e = cudaMalloc((void**)&ws, mo_ws_bytes(grid) + 16);
+    if (e == cudaSuccess && mo) e = cudaMalloc((void**)&flags, (size_t)grid * 4 + 16);
+    if (e == cudaSuccess && mo) e = cudaMemsetAsync(flags, 0, (size_t)grid * 4 + 16, st);
     const bool dev_out = is_device_ptr(out);
     if (e == cudaSuccess && !dev_out) e = cudaMalloc((void**)&stage, out_bytes + 16);
     if (e == cudaSuccess) e = cudaMemcpyAsync(pts, xyz, (size_t)n_points * 3 * 8, cudaMemcpyDefault, st);
-    if (e == cudaSuccess) e = launch_basis(s, pts, n_points, Phi, s.nbp, st);
+    if (e == cudaSuccess) e = launch_basis(s, pts, n_points, Phi, st);
     double* dst = dev_out ? out : stage;
     if (e == cudaSuccess) {
         if (mo) {
-            e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], st);
+            e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], ws, flags, grid, 1u, st);
             if (e == cudaSuccess) e = launch_export_rows(V, (long)n_points * 5, width, s.nsp[spin], dst, st);
         } else {
-            e = launch_export_rows(Phi, (long)n_points * 5, width, s.nbp, dst, st);
+            e = launch_export_phi(Phi, (long)n_points * 5, width, s.kb, dst, st);
         }
     }
     if (e == cudaSuccess && !dev_out) e = cudaMemcpyAsync(out, stage, out_bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(pts); cudaFree(Phi); cudaFree(V); cudaFree(stage);
+    cudaFree(pts); cudaFree(Phi); cudaFree(V); cudaFree(stage); cudaFree(ws); cudaFree(flags);
     CU(e);
     return QMC_OK;
 }
@@ -605,8 +620,9 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
     CU(cudaEventCreate(&e1));
     // make the inputs of the later stages valid
     CU(launch_propose(s, d, spin, p, e, w->step, 0.005, st));
-    CU(launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st));
-    CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, st));
+    const int mgrid = mo_grid_for(s, spin, 5 * d.W, d.mo_grid);
+    CU(launch_basis(s, d.rp, d.W, d.Phi, st));
+    CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st));
     if (stage == 4) CU(launch_fill_int(d.mcount, d.W, delay_k, st));  // full window, S^-1 = 0: zero correction
     cudaError_t err = cudaSuccess;
     for (int r = -2; r < reps && err == cudaSuccess; r++) {
@@ -614,8 +630,8 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
         if (err != cudaSuccess) break;
         switch (stage) {
             case 0: err = launch_propose(s, d, spin, p, e, w->step, 0.005, st); break;
-            case 1: err = launch_basis(s, d.rp, d.W, d.Phi, s.nbp, st); break;
-            case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, st); break;
+            case 1: err = launch_basis(s, d.rp, d.W, d.Phi, st); break;
+            case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st); break;
             case 3: err = launch_accept(s, d, spin, p, e, 0, 0.005, 0, st); break;
             case 4:
                 err = launch_flush(s, d, spin, st);

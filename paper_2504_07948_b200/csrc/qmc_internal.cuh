@@ -1,13 +1,15 @@
 // qmc_internal.cuh -- device-side data layout shared by the kernels and the host scheduler.
 //
-// HBM layout (all FP64 unless noted; "NSP" = n_s rounded up to 16, "NBP" = n_basis rounded up to 16,
+// HBM layout (all FP64 unless noted; "NSP" = n_s rounded up to 16, "NBP" = n_basis rounded up to 32 = 32 KB,
 // padding is zero and stays zero, so padded orbitals/functions contribute nothing):
-//   C[s]      [NBP][NSP]            MO coefficients of spin s (GEMM B operand, N contiguous)
+//   CT[s]     [NT][KB][32][132]     MO coefficients of spin s, pre-tiled as the B stages of the stream-K GEMM
+//                                   (tile = 32 basis functions x 128 orbitals, rows padded to 132 doubles)
 //   R         [W][3][NEP]           positions, walker-major SoA (coalesced over electrons inside a walker)
 //   AinvT[s]  [W][NSP][NSP]         AinvT[p][j] = (A^-1)[j][p]: row p is the column the ratio needs (A18)
 //   Orb[s]    [W][NSP(p)][5][NSP]   value / d/dx / d/dy / d/dz / laplacian of the orbitals at the CURRENT
 //                                   position of electron p (row cache: drift and E_L cost O(N_s) per electron)
-//   Phi       [W*5][NBP]            basis functions at the proposed positions (GEMM A operand)
+//   PhiT      [MT][KB][128][36]     basis functions at the proposed positions, pre-tiled as the A stages
+//                                   (row = walker*5 + component, tile = 128 rows x 32 functions, padded to 36)
 //   V         [W*5][LDV]            orbital rows at the proposed positions (GEMM output)
 //   window    Vbuf,Wbuf,W2 [W][KP][NSP], SinvT [W][KP][KP], YT [W][NSP][KP], plist [W][KP] int, mcount [W] int
 #pragma once
@@ -22,14 +24,15 @@ struct ShellRec {
 };
 
 struct SysDev {
-    int n_atoms, n_shells, n_basis, nbp;
+    int n_atoms, n_shells, n_basis, nbp, kb;  // kb = nbp / 32
     int ns[2], nsp[2], ne;
     const double* atom_xyz;  // [n_atoms][3]
     const double* atom_Z;
     const ShellRec* shells;
     const double* alpha;
     const double* coef;
-    const double* C[2];
+    const double* CT[2];  // tiled, see mo_streamk.cuh
+    int nt[2];            // 128-column tiles per spin
     double a_anti, a_para, b_ee, b_en;
     double e_nn;  // nuclear repulsion
 };
@@ -39,8 +42,12 @@ struct WalkDev {
     double* R;
     double* AinvT[2];
     double* Orb[2];
-    double* Phi;
+    double* Phi;  // tiled PhiT
+    int mt;       // 128-row tiles of Phi
     double* V;
+    double* mo_ws;       // stream-K partial tiles [n_sm][128*128]
+    unsigned* mo_flags;  // [n_sm]
+    int mo_grid;
     double *Vbuf, *Wbuf, *W2, *SinvT, *YT, *bvec, *cvec, *xcol;
     int *plist, *mcount;
     double *rp, *G, *u, *dJ, *gJn;  // per-walker proposal scalars: [W][3], [W][3], [W], [W], [W][3]

@@ -5,6 +5,7 @@
 #include <math.h>
 
 #include "gemm_f64.cuh"
+#include "mo_streamk.cuh"
 
 namespace qmc {
 
@@ -64,8 +65,9 @@ __device__ __forceinline__ double u01(uint32_t we, uint32_t wo) {
 
 // ------------------------------------------------------------------------------------------------
 // a3: basis functions (value, gradient, laplacian) at one point per blockIdx.y        [north_star item 1]
-// out[(pt*5 + c)*ld + f].  One thread per shell; the shell table is read through the read-only path.
-__global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restrict__ pts, double* __restrict__ out, long ld) {
+// Written straight into the pre-tiled A-operand layout PhiT (row = pt*5 + component).  One thread per shell;
+// the shell table is read through the read-only path.
+__global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restrict__ pts, double* __restrict__ out) {
     const int pt = blockIdx.y;
     const int sh = blockIdx.x * blockDim.x + threadIdx.x;
     if (sh >= s.n_shells) return;
@@ -81,15 +83,17 @@ __global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restric
         g1 -= al * e;
         g2 += al * al * e;
     }
-    double* o = out + (long)pt * 5 * ld + rec.f0;
+    const long row0 = (long)pt * 5;
+    const int kb = s.kb;
     const double lapfac = (double)(4 * rec.l + 6) * g1 + 4.0 * t * g2;
     const double tg1 = 2.0 * g1;
     auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
-        o[m] = S * g;
-        o[ld + m] = g * Sx + tg1 * S * x;
-        o[2 * ld + m] = g * Sy + tg1 * S * y;
-        o[3 * ld + m] = g * Sz + tg1 * S * z;
-        o[4 * ld + m] = S * lapfac;
+        const int f = rec.f0 + m;
+        out[phiT_index(row0, f, kb)] = S * g;
+        out[phiT_index(row0 + 1, f, kb)] = g * Sx + tg1 * S * x;
+        out[phiT_index(row0 + 2, f, kb)] = g * Sy + tg1 * S * y;
+        out[phiT_index(row0 + 3, f, kb)] = g * Sz + tg1 * S * z;
+        out[phiT_index(row0 + 4, f, kb)] = S * lapfac;
     };
     const double s3 = 1.7320508075688772;
     if (rec.l == 0) {
@@ -107,26 +111,40 @@ __global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restric
     }
 }
 
-cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* out, long ld, cudaStream_t st) {
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
     dim3 grid((s.n_shells + 127) / 128, n_points);
-    k_basis<<<grid, 128, 0, st>>>(s, pts, out, ld);
+    k_basis<<<grid, 128, 0, st>>>(s, pts, PhiT);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------
-// a4: MO rows V = Phi * C_s  (FP64 DMMA GEMM)                                          [north_star item 2]
-using CfgMO = GemmCfg<128, 128, 64, 32, false, 4>;
+// a4: MO rows V = Phi * C_s: persistent stream-K FP64 DMMA GEMM (mo_streamk.cuh)       [north_star item 2]
+size_t phiT_bytes(const SysDev& s, int rows) { return (size_t)((rows + MO_BM - 1) / MO_BM) * s.kb * MO_A_STAGE * sizeof(double); }
+size_t mo_ws_bytes(int grid) { return (size_t)grid * MO_WS_DOUBLES * sizeof(double); }
+int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm) {
+    const long total = (long)((rows + MO_BM - 1) / MO_BM) * s.nt[spin] * s.kb;
+    return (int)(total < n_sm ? total : n_sm);
+}
 
-cudaError_t launch_mo(const SysDev& s, int spin, const double* Phi, int rows, double* V, long ldv, cudaStream_t st) {
-    GemmArgs g;
-    g.A = Phi; g.lda = s.nbp; g.strideA = 0;
-    g.B = s.C[spin]; g.ldb = s.nsp[spin]; g.strideB = 0;
-    g.C = V; g.ldc = ldv; g.strideC = 0;
-    g.M = rows; g.N = s.nsp[spin]; g.K = s.nbp;
+cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
+                      int grid, unsigned epoch, cudaStream_t st) {
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    MoArgs g;
+    g.PhiT = PhiT; g.CT = s.CT[spin]; g.V = V; g.ldv = ldv;
+    g.M = rows; g.N = s.nsp[spin];
+    g.MT = (rows + MO_BM - 1) / MO_BM; g.NT = s.nt[spin]; g.KB = s.kb;
+    g.ws = ws; g.flags = flags; g.epoch = epoch;
+    if (grid < 1) return cudaSuccess;
+    k_mo_streamk<<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
     COUNT_LAUNCH();
-    return gemm_f64_launch<CfgMO>(g, 1, EpiStore{}, st);
+    return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -815,15 +833,28 @@ cudaError_t launch_export_rows(const double* src, long n_rows, int width, long l
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
-__global__ void k_pad_C(const double* __restrict__ in, int nb, int ns, double* __restrict__ out, int nsp) {
+__global__ void k_tile_C(const double* __restrict__ in, int nb, int ns, double* __restrict__ CT, int kb) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long)nb * ns) return;
-    out[(idx / ns) * nsp + idx % ns] = in[idx];
+    const int l = (int)(idx / ns), j = (int)(idx % ns);
+    CT[cT_index(l, j, kb)] = in[idx];
 }
-cudaError_t launch_pad_C(const double* in, int nb, int ns, double* out, int nsp, cudaStream_t st) {
+cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, cudaStream_t st) {
     long n = (long)nb * ns;
     if (n == 0) return cudaSuccess;
-    k_pad_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, out, nsp);
+    k_tile_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, CT, kb);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+__global__ void k_export_phi(const double* __restrict__ PhiT, long n_rows, int width, int kb, double* __restrict__ out) {
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_rows * width) return;
+    out[idx] = PhiT[phiT_index(idx / width, (int)(idx % width), kb)];
+}
+cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, double* out, cudaStream_t st) {
+    long n = n_rows * width;
+    if (n == 0) return cudaSuccess;
+    k_export_phi<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(PhiT, n_rows, width, kb, out);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

@@ -4,8 +4,14 @@
 
 namespace qmc {
 
-cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* out, long ld, cudaStream_t st);
-cudaError_t launch_mo(const SysDev& s, int spin, const double* Phi, int rows, double* V, long ldv, cudaStream_t st);
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st);
+cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
+                      int grid, unsigned epoch, cudaStream_t st);
+int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm);
+size_t mo_ws_bytes(int grid);
+size_t phiT_bytes(const SysDev& s, int rows);
+cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, cudaStream_t st);
+cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, double* out, cudaStream_t st);
 cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st);
 cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st);
 cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st);
@@ -19,7 +25,6 @@ cudaError_t launch_import_positions(const WalkDev& wd, const double* in, cudaStr
 cudaError_t launch_export_positions(const WalkDev& wd, double* out, cudaStream_t st);
 cudaError_t launch_export_ainv(const double* AinvT, int W, int ns, int nsp, double* out, cudaStream_t st);
 cudaError_t launch_export_rows(const double* src, long n_rows, int width, long ld, double* out, cudaStream_t st);
-cudaError_t launch_pad_C(const double* in, int nb, int ns, double* out, int nsp, cudaStream_t st);
 cudaError_t launch_sign_to_i8(const int* in, int n, int8_t* out, cudaStream_t st);
 cudaError_t launch_fill_int(int* p, int n, int v, cudaStream_t st);
 cudaError_t launch_enn(const SysDev& s, double* out, cudaStream_t st);

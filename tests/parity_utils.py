@@ -6,7 +6,9 @@ import numpy as np
 import oracle
 import paper_2504_07948_b200 as qb
 
-TOL_RATIO = 1e-10      # ratios and log|Psi|, relative
+TOL_RATIO = 1e-10      # ratios and log|Psi|, relative (ratios: for |rho_D e^dJ| >= RATIO_SMALL)
+RATIO_SMALL = 1e-2     # below this the ratio is a cancelling dot product (proposal next to a node): its
+TOL_RATIO_ABS = 1e-12  # rounding error is absolute, ~eps * sum_j |v_j x_j|, so it is held to this absolute bound
 TOL_POS = 1e-10        # positions, absolute bohr (reading A27)
 TOL_AINV = 1e-9        # A^-1, relative Frobenius
 TOL_ELOC = 1e-9        # E_L, hartree
@@ -32,7 +34,7 @@ def run_and_compare(wl, walker_ids, n_sweeps, delay_k, sweeps_per_call=1, thread
     gw = qb.qmc_walkers_create(gsys, pos0, wl.seed, first_walker_id=w0, first_step=first_step, flags=flags)
     osys = osys or oracle.OracleSystem(sysm)
     ow = [osys.walker(p) for p in pos0]
-    rep = dict(n_moves=0, n_mismatch_flagged=0, n_resync=0, max_ratio_rel=0.0, max_pos_abs=0.0, max_logpsi_rel=0.0,
+    rep = dict(n_moves=0, n_mismatch_flagged=0, n_resync=0, max_ratio_rel=0.0, max_small_ratio_abs=0.0, max_pos_abs=0.0, max_logpsi_rel=0.0,
                max_eloc_abs=0.0, max_ainv_rel=0.0, n_ties_gpu=0, n_ties_oracle=0, accept_frac=0.0, failures=[])
     acc = 0
     from concurrent.futures import ThreadPoolExecutor
@@ -70,9 +72,11 @@ def run_and_compare(wl, walker_ids, n_sweeps, delay_k, sweeps_per_call=1, thread
                                             oracle_pacc=float(opacc[i]), gpu_ratio=float(gratio[i, n]), oracle_ratio=float(oratio[i])))
                 ow[n].set_positions(gpos[n])
                 continue
-            m = oratio != 0
+            m = np.abs(oratio) >= RATIO_SMALL
             if m.any():
                 rep["max_ratio_rel"] = max(rep["max_ratio_rel"], float(np.max(np.abs(gratio[m, n] - oratio[m]) / np.abs(oratio[m]))))
+            if (~m).any():
+                rep["max_small_ratio_abs"] = max(rep["max_small_ratio_abs"], float(np.max(np.abs(gratio[~m, n] - oratio[~m]))))
             rep["max_pos_abs"] = max(rep["max_pos_abs"], float(np.abs(gpos[n] - ow[n].positions()).max()))
             ol, osg = ow[n].logpsi()
             rep["max_logpsi_rel"] = max(rep["max_logpsi_rel"], abs(glog[n] - ol) / abs(ol))

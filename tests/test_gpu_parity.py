@@ -1,0 +1,252 @@
+"""Parity of the CUDA path against the CPU oracle, element by element, through the C ABI (-m gpu).
+
+Tolerances are BASELINE.json north_star's: accept/reject decisions identical (ties within 1e-12 flagged,
+not counted), ratios and log|Psi| 1e-10 relative, A^-1 1e-9 relative Frobenius, E_L 1e-9 Ha, positions
+1e-10 bohr (reading A27)."""
+import numpy as np
+import pytest
+
+import oracle
+import qmc_inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+qb = pytest.importorskip("paper_2504_07948_b200")
+from parity_utils import (RATIO_SMALL, TOL_AINV, TOL_ELOC, TOL_POS, TOL_RATIO, TOL_RATIO_ABS, rel_frob,  # noqa: E402
+                          run_and_compare)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    qb.load_library()  # fails loudly if the extension is missing: no CPU fallback
+
+
+def _assert_report(rep, eloc_tol=TOL_ELOC, max_flagged=2):
+    assert rep["failures"] == [], rep["failures"][:3]
+    assert rep["n_mismatch_flagged"] <= max_flagged
+    assert rep["max_ratio_rel"] < TOL_RATIO
+    assert rep["max_small_ratio_abs"] < TOL_RATIO_ABS
+    assert rep["max_logpsi_rel"] < TOL_RATIO
+    assert rep["max_pos_abs"] < TOL_POS
+    assert rep["max_ainv_rel"] < TOL_AINV
+    assert rep["max_eloc_abs"] < eloc_tol
+    assert rep["stats"]["nonfinite"] == 0
+    assert rep["stats"]["proposed"] == rep["n_moves"]
+
+
+# ------------------------------------------------------------------ stages
+
+@pytest.mark.parametrize("cfg,npts", [(0, 37), (1, 19)])
+def test_basis_and_mo_rows(cfg, npts):
+    s = qi.make_system(cfg)
+    g = qb.qmc_init_from(s)
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(cfg)
+    pts = s.atoms_xyz[rng.integers(0, s.n_atoms, npts)] + rng.standard_normal((npts, 3)) * 1.2
+    B = qb.qmc_eval_basis(g, pts).cpu().numpy()
+    for n in range(npts):
+        phi, gr, lap = o.basis_eval(pts[n])
+        ref = np.concatenate([phi[None], gr, lap[None]])
+        assert np.abs(B[n] - ref).max() <= 1e-13 * np.abs(ref).max()
+    for spin in (0, 1):
+        M = qb.qmc_eval_mo(g, spin, pts).cpu().numpy()
+        for n in range(npts):
+            ref = o.mo_rows(spin, pts[n])
+            assert np.abs(M[n] - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_mo_contraction_ragged_tiles():
+    # 300 points x 5 rows = 1500 rows: several 128-row tiles and a ragged tail; N_s = 128, K = 768
+    s = qi.make_system(1)
+    g = qb.qmc_init_from(s)
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(5)
+    pts = s.atoms_xyz[rng.integers(0, s.n_atoms, 300)] + rng.standard_normal((300, 3))
+    M = qb.qmc_eval_mo(g, 1, pts).cpu().numpy()
+    for n in (0, 1, 127, 128, 255, 256, 257, 299):
+        ref = o.mo_rows(1, pts[n])
+        assert np.abs(M[n] - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert qb.qmc_eval_mo(g, 0, pts[:0]).shape[0] == 0  # empty input
+
+
+def test_walker_creation_state():
+    for cfg, nw in ((0, 16), (1, 6)):
+        wl = qi.make_workload(cfg)
+        pos = wl.positions(0, nw)
+        g = qb.qmc_init_from(wl.system)
+        gw = qb.qmc_walkers_create(g, pos, wl.seed)
+        o = oracle.OracleSystem(wl.system)
+        lp, sg = [x.cpu().numpy() for x in qb.qmc_get_logpsi(gw)]
+        el, ek = [x.cpu().numpy() for x in qb.qmc_get_eloc(gw)]
+        np.testing.assert_array_equal(qb.qmc_get_positions(gw).cpu().numpy(), pos)
+        for n in range(nw):
+            w = o.walker(pos[n])
+            ol, os_ = w.logpsi()
+            assert abs(lp[n] - ol) < TOL_RATIO * abs(ol) and sg[n] == os_
+            oe, ok = w.eloc()
+            assert abs(el[n] - oe) < TOL_ELOC and abs(ek[n] - ok) < TOL_ELOC
+            for spin in (0, 1):
+                assert rel_frob(qb.qmc_get_Ainv(gw, spin).cpu().numpy()[n], w.Ainv(spin)) < TOL_AINV
+
+
+def test_hydrogen_atom_eloc_on_gpu():
+    h = qi.hydrogen_atom()
+    g = qb.qmc_init_from(h)
+    rng = np.random.default_rng(3)
+    pos = rng.standard_normal((32, 1, 3))
+    gw = qb.qmc_walkers_create(g, pos, 5)
+    qb.qmc_sweep(gw, 25, 0.05, 1)
+    el, ek = [x.cpu().numpy() for x in qb.qmc_get_eloc(gw)]
+    assert np.abs(el + 0.5).max() < 1e-12  # E_L = -1/2 with zero variance
+    lp, sg = [x.cpu().numpy() for x in qb.qmc_get_logpsi(gw)]
+    r = np.linalg.norm(qb.qmc_get_positions(gw).cpu().numpy()[:, 0], axis=1)
+    np.testing.assert_allclose(lp, -r, atol=1e-12)
+    res = oracle.run_crowd(h, pos, 5, range(32), 0, 25, 0.05, threads=1)
+    assert np.array_equal(qb.qmc_get_accept_log(gw).cpu().numpy() & 1, res["bits"] & 1)
+    np.testing.assert_allclose(qb.qmc_get_positions(gw).cpu().numpy(), res["positions"], atol=TOL_POS)
+
+
+# ------------------------------------------------------------------ trajectories
+
+def test_config0_full_trajectories():
+    # config 0 as BASELINE.json states it: 64 walkers, tau 0.01, 100 sweeps, delay_k 1
+    wl = qi.make_workload(0)
+    rep = run_and_compare(wl, range(wl.n_walkers), wl.n_sweeps, wl.delay_k)
+    _assert_report(rep)
+    assert rep["n_moves"] == wl.n_moves and 0.5 < rep["accept_frac"] < 1.0
+
+
+@pytest.mark.parametrize("k", [4, 5])
+def test_config0_delayed(k):
+    wl = qi.make_workload(0)
+    _assert_report(run_and_compare(wl, range(16), 20, k))
+
+
+def test_config1_trajectories_subset_delay32():
+    # config 1 system and run parameters (tau 0.005, delay_k 32); the GPU runs a 24-walker slice of the crowd,
+    # every walker compared with the oracle for 4 sweeps (the full 512 x 50 run is bench territory)
+    wl = qi.make_workload(1)
+    rep = run_and_compare(wl, range(100, 124), 4, wl.delay_k)
+    _assert_report(rep)
+
+
+def test_config1_full_crowd_sampled_walkers():
+    # full config-1 crowd (512 walkers) on the GPU in the bench launch configuration; sampled walkers are
+    # compared with the oracle (walkers are independent: A20)
+    wl = qi.make_workload(1)
+    g = qb.qmc_init_from(wl.system)
+    T = 3
+    gw = qb.qmc_walkers_create(g, wl.positions(), wl.seed, flags=qb.QMC_LOG_RATIOS)
+    qb.qmc_sweep(gw, T, wl.tau, wl.delay_k)
+    bits = qb.qmc_get_accept_log(gw).cpu().numpy()
+    ratio = qb.qmc_get_ratio_log(gw)[0].cpu().numpy()
+    pos = qb.qmc_get_positions(gw).cpu().numpy()
+    el = qb.qmc_get_eloc(gw)[0].cpu().numpy()
+    sample = [0, 1, 77, 255, 256, 400, 511]
+    res = oracle.run_crowd(wl.system, wl.positions()[sample], wl.seed, sample, 0, T, wl.tau)
+    n_div = 0
+    for n, w in enumerate(sample):
+        same = np.array_equal(bits[:, :, w] & 1, res["bits"][:, :, n] & 1)
+        if not same:
+            d = np.argwhere((bits[:, :, w] & 1) != (res["bits"][:, :, n] & 1))[0]
+            assert (bits[d[0], d[1], w] | res["bits"][d[0], d[1], n]) & 2, f"unflagged mismatch walker {w} at {d}"
+            n_div += 1
+            continue
+        m = np.abs(res["ratio"][:, :, n]) >= RATIO_SMALL
+        assert np.max(np.abs(ratio[:, :, w][m] - res["ratio"][:, :, n][m]) / np.abs(res["ratio"][:, :, n][m])) < TOL_RATIO
+        assert np.all(np.abs(ratio[:, :, w][~m] - res["ratio"][:, :, n][~m]) < TOL_RATIO_ABS)
+        assert np.abs(pos[w] - res["positions"][n]).max() < TOL_POS
+        assert abs(el[w] - res["eloc"][-1, n]) < TOL_ELOC
+    assert n_div <= 1
+    st = qb.qmc_get_stats(gw)
+    assert st["proposed"] == 512 * 256 * T and st["nonfinite"] == 0
+
+
+# ------------------------------------------------------------------ invariants on the GPU
+
+def _run_gpu(wl, w0, w1, T, k, calls=1, flags=0):
+    g = qb.qmc_init_from(wl.system)
+    gw = qb.qmc_walkers_create(g, wl.positions(w0, w1), wl.seed, first_walker_id=w0, flags=flags)
+    bits = []
+    for _ in range(calls):
+        qb.qmc_sweep(gw, T // calls, wl.tau, k)
+        bits.append(qb.qmc_get_accept_log(gw).cpu().numpy())
+    return (np.concatenate(bits), qb.qmc_get_positions(gw).cpu().numpy(), qb.qmc_get_eloc(gw)[0].cpu().numpy(),
+            qb.qmc_get_Ainv(gw, 0).cpu().numpy())
+
+
+def test_resume_is_bitwise():
+    wl = qi.make_workload(1)
+    a = _run_gpu(wl, 0, 12, 4, 16, calls=1)
+    b = _run_gpu(wl, 0, 12, 4, 16, calls=2)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)  # qmc_sweep(2) twice == qmc_sweep(4) once, bit for bit
+
+
+def test_delay_invariance_and_walker_prefix():
+    wl = qi.make_workload(1)
+    ref = _run_gpu(wl, 0, 16, 3, 1)
+    for k in (4, 16, 32, 64, 128):
+        got = _run_gpu(wl, 0, 16, 3, k)
+        assert np.array_equal(got[0] & 1, ref[0] & 1), f"accept bits differ at delay_k={k}"
+        assert np.abs(got[1] - ref[1]).max() < TOL_POS
+        assert np.abs(got[2] - ref[2]).max() < TOL_ELOC
+        assert max(rel_frob(got[3][n], ref[3][n]) for n in range(16)) < TOL_AINV
+    sub = _run_gpu(wl, 5, 11, 3, 32)  # walkers 5..10 alone == the same walkers inside the larger crowd (A20)
+    big = _run_gpu(wl, 0, 16, 3, 32)
+    assert np.array_equal(sub[0], big[0][:, :, 5:11])
+    assert np.array_equal(sub[1], big[1][5:11])
+
+
+# ------------------------------------------------------------------ ABI behaviour
+
+def test_error_codes():
+    s = qi.make_system(0)
+    g = qb.qmc_init_from(s)
+    wl = qi.make_workload(0)
+    gw = qb.qmc_walkers_create(g, wl.positions(0, 2), 1)
+    for bad in (dict(nsteps=1, tau=0.0, delay_k=1), dict(nsteps=1, tau=0.01, delay_k=0), dict(nsteps=1, tau=0.01, delay_k=129),
+                dict(nsteps=-1, tau=0.01, delay_k=1)):
+        with pytest.raises(qb.QmcError) as ei:
+            qb.qmc_sweep(gw, **bad)
+        assert ei.value.code == qb.QMC_ERR_ARG
+    with pytest.raises(qb.QmcError) as ei:
+        qb.qmc_get_ratio_log(gw)  # not created with QMC_LOG_RATIOS
+    assert ei.value.code == qb.QMC_ERR_STATE
+    with pytest.raises(qb.QmcError):
+        qb.qmc_walkers_create(g, np.zeros((2, 3, 3)), 1)  # wrong electron count
+    # two electrons of the same spin at the same point: singular Slater matrix
+    pos = wl.positions(0, 1).copy()
+    pos[0, 1] = pos[0, 0]
+    with pytest.raises(qb.QmcError) as ei:
+        qb.qmc_walkers_create(g, pos, 1)
+    assert ei.value.code == qb.QMC_ERR_SINGULAR
+    s_bad = qi.make_system(0)
+    l_bad = s_bad.shell_l.copy()
+    l_bad[0] = 3
+    with pytest.raises(qb.QmcError) as ei:
+        qb.qmc_init(s_bad.atoms_xyz, s_bad.Z, s_bad.shell_atom, l_bad, s_bad.shell_nprim, s_bad.shell_prim_offset,
+                    s_bad.alpha, s_bad.coef, s_bad.n_basis, 5, 5, s_bad.C_up, s_bad.C_dn)
+    assert ei.value.code == qb.QMC_ERR_ARG
+    # zero sweeps is legal and leaves the state untouched
+    qb.qmc_sweep(gw, 0, 0.01, 1)
+    assert qb.qmc_get_accept_log(gw).numel() == 0
+
+
+def test_device_and_host_buffers_agree():
+    import torch
+    wl = qi.make_workload(0)
+    g = qb.qmc_init_from(wl.system)
+    pos_dev = torch.from_numpy(wl.positions(0, 4)).cuda()
+    gw = qb.qmc_walkers_create(g, pos_dev, wl.seed)  # device input
+    qb.qmc_sweep(gw, 3, wl.tau, 2)
+    dev = qb.qmc_get_positions(gw)
+    host = torch.empty(dev.shape, dtype=torch.float64).pin_memory()
+    qb.qmc_get_positions(gw, out=host)  # host output (synchronous)
+    assert torch.equal(dev.cpu(), host)
+    e_host = torch.empty(4, dtype=torch.float64)
+    qb.qmc_get_eloc(gw, out=e_host, out_kin=torch.empty(4, dtype=torch.float64))
+    assert torch.equal(qb.qmc_get_eloc(gw)[0].cpu(), e_host)
