@@ -524,8 +524,9 @@ extern "C" int qmc_get_accept_log(const qmc_walkers* w, uint8_t* bits) {
 }
 
 extern "C" int qmc_get_ratio_log(const qmc_walkers* w, double* ratio, double* pacc) {
-    if (!w || !ratio) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null argument");
+    if (!w) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null walkers");
     if (!(w->flags & QMC_LOG_RATIOS) || !w->d.ratio_log) return fail(QMC_ERR_STATE, "qmc_get_ratio_log: walkers were not created with QMC_LOG_RATIOS, or no sweep has run");
+    if (!ratio) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null argument");
     size_t n = (size_t)w->T_last * w->d.ne * w->d.W * 8;
     if (n == 0) return QMC_OK;
     CU(cudaMemcpyAsync(ratio, w->d.ratio_log, n, cudaMemcpyDefault, w->stream));
