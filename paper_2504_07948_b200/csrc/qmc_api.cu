@@ -333,6 +333,17 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         destroy_walkers(w);
         return fail(QMC_ERR_SINGULAR, "qmc_walkers_create: singular Slater matrix (zero pivot)");
     }
+    {   // one Newton-Schulz refinement step of every inverse (temporary buffers, freed right after)
+        const size_t mat_max = (size_t)d.ldv * d.ldv * 8;
+        double *E = nullptr, *Z = nullptr;
+        CUW(cudaMalloc((void**)&E, W * mat_max + 16));
+        cudaError_t e = cudaMalloc((void**)&Z, W * mat_max + 16);
+        for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) e = launch_refine_inverse(s, d, sp, E, Z, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(E);
+        cudaFree(Z);
+        CUW(e);
+    }
     CUW(launch_jastrow_total(s, d, st));
     CUW(launch_window_reset(d, st));
     CUW(launch_eloc(s, d, st));
