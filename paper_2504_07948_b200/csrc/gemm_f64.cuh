@@ -155,8 +155,11 @@ struct GemmArgs {
     int M, N, K;
 };
 
-// Epilogues.  Each has: bool skip(int b) const; void operator()(int b, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const
+// Epilogues.  Each has: static constexpr bool preload (true: the accumulators start from the C tile, i.e. the
+// kernel computes C += A*B with the C loads issued before the main loop so their latency hides behind the
+// operand staging); bool skip(int b) const; void operator()(int b, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const
 struct EpiStore {
+    static constexpr bool preload = false;
     __device__ bool skip(int) const { return false; }
     __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
         if (row < M && col < N) *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
@@ -177,8 +180,16 @@ __global__ void __launch_bounds__(Cfg::NTHREADS) gemm_f64_kernel(GemmArgs g, Epi
     const double* A = g.A + (long)b * g.strideA;
     const double* B = g.B + (long)b * g.strideB;
     double* C = g.C + (long)b * g.strideC;
+    if constexpr (Epi::preload) {
+        gemm_foreach_acc<Cfg>(acc, m0, n0, [&](int row, int col, double& v0, double& v1) {
+            if (row < g.M && col < g.N) {
+                const double2 c = *reinterpret_cast<const double2*>(C + (long)row * g.ldc + col);
+                v0 = c.x; v1 = c.y;
+            }
+        });
+    }
     gemm_mainloop<Cfg>(acc, gemm_smem, A, g.lda, B, g.ldb, g.M, g.N, g.K, m0, n0, 0, g.K / Cfg::BK);
-    gemm_foreach_acc<Cfg>(acc, m0, n0, [&](int row, int col, double v0, double v1) { epi(b, C, g.ldc, g.M, g.N, row, col, v0, v1); });
+    gemm_foreach_acc<Cfg>(acc, m0, n0, [&](int row, int col, double& v0, double& v1) { epi(b, C, g.ldc, g.M, g.N, row, col, v0, v1); });
 }
 
 template <class Cfg, class Epi>

@@ -4,6 +4,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -175,6 +176,32 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     CUS(cudaMemcpyAsync(dco, coef.data(), coef.size() * 8, cudaMemcpyHostToDevice, st));
     CUS(cudaMemcpyAsync(drec, recs.data(), recs.size() * sizeof(ShellRec), cudaMemcpyHostToDevice, st));
     d.atom_xyz = dxyz; d.atom_Z = dZ; d.alpha = dal; d.coef = dco; d.shells = drec;
+    {   // shells that own a function of each 32-function k-block (a shell may straddle two blocks)
+        std::vector<int2> kbs(d.kb);
+        int lo = 0;
+        for (int kb = 0; kb < d.kb; kb++) {
+            const int f_lo = kb * 32, f_hi = f_lo + 32;
+            while (lo < basis->n_shells && recs[lo].f0 + 2 * recs[lo].l + 1 <= f_lo) lo++;
+            int hi = lo;
+            while (hi < basis->n_shells && recs[hi].f0 < f_hi) hi++;
+            kbs[kb] = make_int2(lo, hi);
+        }
+        int2* dkbs;
+        CUS(S->pool.alloc((void**)&dkbs, kbs.size() * sizeof(int2), st));
+        CUS(cudaMemcpyAsync(dkbs, kbs.data(), kbs.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+        CUS(cudaStreamSynchronize(st));
+        d.kb_shells = dkbs;
+        d.max_kb_shells = 1;
+        for (const int2& r : kbs) d.max_kb_shells = std::max(d.max_kb_shells, r.y - r.x);
+        std::vector<int> ftab(d.nbp, -1);
+        for (int i = 0; i < basis->n_shells; i++)
+            for (int m = 0; m < 2 * recs[i].l + 1; m++) ftab[recs[i].f0 + m] = i | (m << 24);
+        int* dft;
+        CUS(S->pool.alloc((void**)&dft, ftab.size() * sizeof(int), st));
+        CUS(cudaMemcpyAsync(dft, ftab.data(), ftab.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+        CUS(cudaStreamSynchronize(st));
+        d.fun_tab = dft;
+    }
     for (int sp = 0; sp < 2; sp++) {
         double* dC;
         CUS(S->pool.alloc((void**)&dC, (size_t)d.nt[sp] * d.kb * 32 * 132 * 8, st));

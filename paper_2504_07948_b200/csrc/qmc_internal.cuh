@@ -29,6 +29,9 @@ struct SysDev {
     const double* atom_xyz;  // [n_atoms][3]
     const double* atom_Z;
     const ShellRec* shells;
+    const int2* kb_shells;  // [kb]: shells [x, y) that own a function of k-block kb (32 functions)
+    const int* fun_tab;     // [nbp]: shell | (m << 24) of every basis function, -1 for the zero padding
+    int max_kb_shells;      // max over k-blocks of y - x
     const double* alpha;
     const double* coef;
     const double* CT[2];  // tiled, see mo_streamk.cuh

@@ -7,6 +7,15 @@
 #include "gemm_f64.cuh"
 #include "mo_streamk.cuh"
 
+#ifndef QMC_UPD_BM
+#define QMC_UPD_BM 128
+#define QMC_UPD_BN 64
+#define QMC_UPD_STAGES 2
+#endif
+#ifndef QMC_Y_STAGES
+#define QMC_Y_STAGES 3
+#endif
+
 namespace qmc {
 
 thread_local uint64_t g_launches = 0;
@@ -64,57 +73,108 @@ __device__ __forceinline__ double u01(uint32_t we, uint32_t wo) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3: basis functions (value, gradient, laplacian) at one point per blockIdx.y        [north_star item 1]
-// Written straight into the pre-tiled A-operand layout PhiT (row = pt*5 + component).  One thread per shell;
-// the shell table is read through the read-only path.
-__global__ void __launch_bounds__(128) k_basis(SysDev s, const double* __restrict__ pts, double* __restrict__ out) {
-    const int pt = blockIdx.y;
-    const int sh = blockIdx.x * blockDim.x + threadIdx.x;
-    if (sh >= s.n_shells) return;
-    const double px = pts[3 * pt], py = pts[3 * pt + 1], pz = pts[3 * pt + 2];
-    const ShellRec rec = s.shells[sh];
-    const double x = px - rec.x, y = py - rec.y, z = pz - rec.z;
-    const double t = x * x + y * y + z * z;
-    double g = 0.0, g1 = 0.0, g2 = 0.0;
-    for (int p = 0; p < rec.nprim; p++) {
-        const double al = __ldg(s.alpha + rec.poff + p);
-        const double e = __ldg(s.coef + rec.poff + p) * exp(-al * t);
-        g += e;
-        g1 -= al * e;
-        g2 += al * al * e;
+// a3: basis functions (value, gradient, laplacian) at the proposed positions          [north_star item 1]
+// One CTA builds one A stage of the MO contraction -- 128 rows (row = point*5 + component) x 32 functions,
+// rows padded to 36 doubles -- in shared memory and hands it to the TMA engine as ONE contiguous 36,864 B
+// bulk store (cp.async.bulk.global.shared::cta, SASS UBLKCP), so HBM sees only full-line writes.  Threads
+// take (point, shell) pairs of the tile; a shell that straddles two k-blocks is evaluated by both.
+__device__ __forceinline__ void bulk_s2g(void* gmem_dst, const void* smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gmem_dst), "r"(smem_u32(smem_src)), "r"(bytes)
+                 : "memory");
+}
+
+constexpr int BASIS_THREADS = 256;
+constexpr int BASIS_MAXPT = (MO_BM + 4) / 5 + 1;  // points that can touch one 128-row tile (27)
+
+// Two phases per tile.  (1) one thread per (point, shell): the contracted radial part g, 2g', (4l+6)g' + 4t g''
+// (three FP64 exp per pair -- the expensive part, done once per shell, never per function);  (2) one thread per
+// (point, function): the five components from the radial triple and the angular polynomial, written to the
+// shared-memory tile with consecutive threads on consecutive columns (conflict free).
+__global__ void __launch_bounds__(BASIS_THREADS) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out) {
+    extern __shared__ __align__(128) double bsm[];
+    double* tile = bsm;                          // [128][36]
+    double* spt = tile + MO_A_STAGE;             // [BASIS_MAXPT][3]
+    double* rad = spt + 3 * BASIS_MAXPT + 3;     // [npt][nsh][3]
+    const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
+    for (int i = tid; i < MO_A_STAGE / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
+    const int row_lo = tm * MO_BM;
+    const int pt_lo = row_lo / 5;
+    int pt_hi = (row_lo + MO_BM + 4) / 5;
+    if (pt_hi > n_points) pt_hi = n_points;
+    const int npt = pt_hi - pt_lo;
+    const int2 shr = s.kb_shells[kb];
+    const int nsh = shr.y - shr.x, npair = npt * nsh;
+    if (tid < 3 * npt) spt[tid] = pts[3 * pt_lo + tid];
+    __syncthreads();
+    for (int q = tid; q < npair; q += BASIS_THREADS) {
+        const int pi = q / nsh, sh = shr.x + (q - pi * nsh);
+        const ShellRec rec = s.shells[sh];
+        const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
+        const double t = x * x + y * y + z * z;
+        double g = 0.0, g1 = 0.0, g2 = 0.0;
+        for (int p = 0; p < rec.nprim; p++) {
+            const double al = __ldg(s.alpha + rec.poff + p);
+            const double e = __ldg(s.coef + rec.poff + p) * exp(-al * t);
+            g += e;
+            g1 -= al * e;
+            g2 += al * al * e;
+        }
+        rad[3 * q] = g;
+        rad[3 * q + 1] = 2.0 * g1;
+        rad[3 * q + 2] = (double)(4 * rec.l + 6) * g1 + 4.0 * t * g2;
     }
-    const long row0 = (long)pt * 5;
-    const int kb = s.kb;
-    const double lapfac = (double)(4 * rec.l + 6) * g1 + 4.0 * t * g2;
-    const double tg1 = 2.0 * g1;
-    auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
-        const int f = rec.f0 + m;
-        out[phiT_index(row0, f, kb)] = S * g;
-        out[phiT_index(row0 + 1, f, kb)] = g * Sx + tg1 * S * x;
-        out[phiT_index(row0 + 2, f, kb)] = g * Sy + tg1 * S * y;
-        out[phiT_index(row0 + 3, f, kb)] = g * Sz + tg1 * S * z;
-        out[phiT_index(row0 + 4, f, kb)] = S * lapfac;
-    };
-    const double s3 = 1.7320508075688772;
-    if (rec.l == 0) {
-        emit(0, 1.0, 0.0, 0.0, 0.0);
-    } else if (rec.l == 1) {
-        emit(0, x, 1.0, 0.0, 0.0);
-        emit(1, y, 0.0, 1.0, 0.0);
-        emit(2, z, 0.0, 0.0, 1.0);
-    } else {
-        emit(0, s3 * x * y, s3 * y, s3 * x, 0.0);
-        emit(1, s3 * y * z, 0.0, s3 * z, s3 * y);
-        emit(2, z * z - 0.5 * (x * x + y * y), -x, -y, 2.0 * z);
-        emit(3, s3 * x * z, s3 * z, 0.0, s3 * x);
-        emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
+    __syncthreads();
+    const int f = kb * MO_BK + (tid & 31);
+    const int ft = s.fun_tab[f];  // shell | m << 24, or -1 for a padding function
+    if (ft >= 0) {
+        const int sh = ft & 0xFFFFFF, m = ft >> 24, c = tid & 31;
+        const ShellRec rec = s.shells[sh];
+        for (int pi = tid >> 5; pi < npt; pi += BASIS_THREADS / 32) {
+            const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
+            const double* rd = rad + 3 * (pi * nsh + (sh - shr.x));
+            const double g = rd[0], tg1 = rd[1], lapfac = rd[2];
+            const double s3 = 1.7320508075688772;
+            double S, Sx, Sy, Sz;
+            if (rec.l == 0) { S = 1.0; Sx = 0.0; Sy = 0.0; Sz = 0.0; }
+            else if (rec.l == 1) {
+                S = m == 0 ? x : (m == 1 ? y : z);
+                Sx = m == 0 ? 1.0 : 0.0; Sy = m == 1 ? 1.0 : 0.0; Sz = m == 2 ? 1.0 : 0.0;
+            } else {
+                switch (m) {
+                    case 0: S = s3 * x * y; Sx = s3 * y; Sy = s3 * x; Sz = 0.0; break;
+                    case 1: S = s3 * y * z; Sx = 0.0; Sy = s3 * z; Sz = s3 * y; break;
+                    case 2: S = z * z - 0.5 * (x * x + y * y); Sx = -x; Sy = -y; Sz = 2.0 * z; break;
+                    case 3: S = s3 * x * z; Sx = s3 * z; Sy = 0.0; Sz = s3 * x; break;
+                    default: S = (0.5 * s3) * (x * x - y * y); Sx = s3 * x; Sy = -s3 * y; Sz = 0.0; break;
+                }
+            }
+            const int r0 = (pt_lo + pi) * 5 - row_lo;  // local row of the value component (may be < 0 or > 123)
+            const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
+#pragma unroll
+            for (int k = 0; k < 5; k++)
+                if (r0 + k >= 0 && r0 + k < MO_BM) tile[(r0 + k) * MO_ALD + c] = v[k];
+        }
+    }
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // generic-proxy smem writes -> visible to the TMA engine
+    __syncthreads();
+    if (tid == 0) {
+        bulk_s2g(out + ((long)tm * s.kb + kb) * MO_A_STAGE, tile, MO_A_STAGE * sizeof(double));
+        asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory");  // smem must outlive the read
     }
 }
 
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
-    dim3 grid((s.n_shells + 127) / 128, n_points);
-    k_basis<<<grid, 128, 0, st>>>(s, pts, PhiT);
+    static int configured_smem = 0;
+    const size_t smem = (size_t)(MO_A_STAGE + 3 * BASIS_MAXPT + 3 + 3 * BASIS_MAXPT * s.max_kb_shells) * sizeof(double);
+    if ((int)smem > configured_smem) {
+        cudaError_t e = cudaFuncSetAttribute(k_basis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured_smem = (int)smem;
+    }
+    dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
+    k_basis<<<grid, BASIS_THREADS, smem, st>>>(s, pts, n_points, PhiT);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
@@ -175,62 +235,108 @@ __device__ __forceinline__ Partner partner(const SysDev& s, const double* __rest
 
 // ------------------------------------------------------------------------------------------------
 // a1 + a2 + a6: effective inverse column, drift, Philox proposal, Jastrow ratio and gradient at r'.
-// One CTA per walker.                                                           [north_star items 3, 4]
-constexpr int PT = 256;
+// One CTA of 512 threads per walker.  The two streaming passes over the delay window (b = Vbuf a_p, then
+// x = a_p - Wbuf^T c) are HBM-bound GEMVs: every thread keeps 8 independent 16-byte loads in flight.
+//                                                                               [north_star items 3, 4]
+constexpr int PT = 512;
+constexpr int PW = PT / 32;
+
+__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+
+// dot products of row[0..n) with xs[0..n) (n % 2 == 0), one warp, 8 loads in flight per lane
+__device__ __forceinline__ double warp_dot(const double* __restrict__ row, const double* xs, int n, int lane) {
+    double acc = 0.0;
+    const int n2 = n >> 1;
+    int j = lane;
+    for (; j + 7 * 32 < n2; j += 8 * 32) {
+        double2 a[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) a[u] = ldg2(row + 2 * (j + u * 32));
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const double2 x = *reinterpret_cast<const double2*>(xs + 2 * (j + u * 32));
+            acc += a[u].x * x.x + a[u].y * x.y;
+        }
+    }
+    for (; j < n2; j += 32) {
+        const double2 a = ldg2(row + 2 * j);
+        const double2 x = *reinterpret_cast<const double2*>(xs + 2 * j);
+        acc += a.x * x.x + a.y * x.y;
+    }
+    return warp_sum(acc);
+}
 
 __global__ void __launch_bounds__(PT) k_propose(SysDev s, WalkDev wd, int spin, int p, int e, uint32_t step, double tau,
                                                 double sqrt_tau) {
-    extern __shared__ double sm[];
+    extern __shared__ __align__(16) double sm[];
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
-    double* xs = sm;              // [nsp]
-    double* bs = xs + nsp;        // [kp]
-    double* cs = bs + kp;         // [kp]
-    double* red = cs + kp;        // [8 * PT/32]
-    double* bc = red + 8 * (PT / 32);  // [4] broadcast
+    const int kps = kp + 1;            // padded row stride of the S^-1 copy (conflict-free column walks)
+    double* xs = sm;                   // [nsp]
+    double* bs = xs + nsp;             // [kp]
+    double* cs = bs + kp;              // [kp]
+    double* red = cs + kp;             // [8 * PW]
+    double* bc = red + 8 * PW;         // [4] broadcast
+    double* Ss = bc + 4;               // [kp][kp + 1]
     const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
     const int m = wd.mcount[w];
-    for (int j = tid; j < nsp; j += PT) xs[j] = arow[j];
+    for (int j = tid; j < nsp / 2; j += PT) reinterpret_cast<double2*>(xs)[j] = ldg2(arow + 2 * j);
+    if (m > 0) {
+        const double* Si = wd.SinvT + (long)w * kp * kp;
+        for (int idx = tid; idx < m * kp; idx += PT) {
+            const int l = idx / kp, n = idx - l * kp;
+            if (n < m) Ss[l * kps + n] = Si[idx];
+        }
+    }
     __syncthreads();
     if (m > 0) {
         // b_n = v_n . a_p ;  c = S^-1 b ;  x = a_p - Wbuf^T c     (effective column of the delayed inverse)
         const double* Vb = wd.Vbuf + (long)w * kp * nsp;
         const double* Wb = wd.Wbuf + (long)w * kp * nsp;
-        const double* Si = wd.SinvT + (long)w * kp * kp;
-        for (int n = warp; n < m; n += PT / 32) {
-            double acc = 0.0;
-            for (int j = lane; j < nsp; j += 32) acc += Vb[(long)n * nsp + j] * xs[j];
-            acc = warp_sum(acc);
+        for (int n = warp; n < m; n += PW) {
+            const double acc = warp_dot(Vb + (long)n * nsp, xs, nsp, lane);
             if (lane == 0) bs[n] = acc;
         }
         __syncthreads();
         for (int n = tid; n < m; n += PT) {
             double acc = 0.0;
-            for (int l = 0; l < m; l++) acc += Si[l * kp + n] * bs[l];
+            for (int l = 0; l < m; l++) acc += Ss[l * kps + n] * bs[l];
             cs[n] = acc;
             wd.cvec[(long)w * kp + n] = acc;
         }
         __syncthreads();
-        for (int j = tid; j < nsp; j += PT) {
-            double acc = xs[j];
-            for (int l = 0; l < m; l++) acc -= cs[l] * Wb[(long)l * nsp + j];
-            xs[j] = acc;
+        for (int j = tid; j < nsp / 2; j += PT) {
+            double2 acc = reinterpret_cast<double2*>(xs)[j];
+            int l = 0;
+            for (; l + 8 <= m; l += 8) {
+                double2 wv[8];
+#pragma unroll
+                for (int u = 0; u < 8; u++) wv[u] = ldg2(Wb + (long)(l + u) * nsp + 2 * j);
+#pragma unroll
+                for (int u = 0; u < 8; u++) { acc.x -= cs[l + u] * wv[u].x; acc.y -= cs[l + u] * wv[u].y; }
+            }
+            for (; l < m; l++) {
+                const double2 wv = ldg2(Wb + (long)l * nsp + 2 * j);
+                acc.x -= cs[l] * wv.x; acc.y -= cs[l] * wv.y;
+            }
+            reinterpret_cast<double2*>(xs)[j] = acc;
         }
         __syncthreads();
     }
     double* xcol = wd.xcol + (long)w * nsp;
-    for (int j = tid; j < nsp; j += PT) xcol[j] = xs[j];
+    for (int j = tid; j < nsp / 2; j += PT) reinterpret_cast<double2*>(xcol)[j] = reinterpret_cast<double2*>(xs)[j];
 
     // drift: determinant part from the cached gradient rows, Jastrow part by direct sums
     const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
     const double* Rw = wd.R + (long)w * 3 * nep;
     const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
     double acc6[6] = {0, 0, 0, 0, 0, 0};
-    for (int j = tid; j < nsp; j += PT) {
-        const double xj = xs[j];
-        acc6[0] += orb[nsp + j] * xj;
-        acc6[1] += orb[2 * nsp + j] * xj;
-        acc6[2] += orb[3 * nsp + j] * xj;
+    for (int j = tid; j < nsp / 2; j += PT) {
+        const double2 xj = reinterpret_cast<double2*>(xs)[j];
+        const double2 o1 = ldg2(orb + nsp + 2 * j), o2 = ldg2(orb + 2 * nsp + 2 * j), o3 = ldg2(orb + 3 * nsp + 2 * j);
+        acc6[0] += o1.x * xj.x + o1.y * xj.y;
+        acc6[1] += o2.x * xj.x + o2.y * xj.y;
+        acc6[2] += o3.x * xj.x + o3.y * xj.y;
     }
     const int npart = s.ne + s.n_atoms;
     for (int k = tid; k < npart; k += PT) {
@@ -293,11 +399,18 @@ __global__ void __launch_bounds__(PT) k_propose(SysDev s, WalkDev wd, int spin, 
 }
 
 size_t propose_smem(const SysDev& s, const WalkDev& wd, int spin) {
-    return (size_t)(s.nsp[spin] + 2 * wd.kp + 8 * (PT / 32) + 4) * sizeof(double);
+    return (size_t)(s.nsp[spin] + 2 * wd.kp + 8 * PW + 4 + wd.kp * (wd.kp + 1)) * sizeof(double);
 }
 
 cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st) {
-    k_propose<<<wd.W, PT, propose_smem(s, wd, spin), st>>>(s, wd, spin, p, e, step, tau, sqrt(tau));
+    static size_t configured = 48 * 1024;
+    const size_t smem = propose_smem(s, wd, spin);
+    if (smem > configured) {
+        cudaError_t er = cudaFuncSetAttribute(k_propose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (er != cudaSuccess) return er;
+        configured = smem;
+    }
+    k_propose<<<wd.W, PT, smem, st>>>(s, wd, spin, p, e, step, tau, sqrt(tau));
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
@@ -306,23 +419,28 @@ cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, 
 // a5 + a7: determinant ratio and gradient from the effective column, accept/reject, commit.
 // One CTA per walker.  commit == 0 evaluates everything but changes no state (stage timing).
 __global__ void __launch_bounds__(PT) k_accept(SysDev s, WalkDev wd, int spin, int p, int e, long log_off, double tau, int commit) {
-    extern __shared__ double sm[];
+    extern __shared__ __align__(16) double sm[];
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
-    double* rs = sm;                   // [kp]
+    const int kps = kp + 1;
+    double* vs = sm;                   // [nsp] value row of the proposed position
+    double* rs = vs + nsp;             // [kp]
     double* ts = rs + kp;              // [kp]
     double* cs = ts + kp;              // [kp]
-    double* red = cs + kp;             // [8 * PT/32]
-    double* bc = red + 8 * (PT / 32);  // [4]
+    double* red = cs + kp;             // [8 * PW]
+    double* bc = red + 8 * PW;         // [4]
+    double* Ss = bc + 4;               // [kp][kp + 1]
     const double* v = wd.V + (long)w * 5 * wd.ldv;
     const double* xcol = wd.xcol + (long)w * nsp;
     double a4[4] = {0, 0, 0, 0};
-    for (int j = tid; j < nsp; j += PT) {
-        const double xj = xcol[j];
-        a4[0] += v[j] * xj;
-        a4[1] += v[wd.ldv + j] * xj;
-        a4[2] += v[2 * wd.ldv + j] * xj;
-        a4[3] += v[3 * wd.ldv + j] * xj;
+    for (int j = tid; j < nsp / 2; j += PT) {
+        const double2 xj = ldg2(xcol + 2 * j);
+        const double2 v0 = ldg2(v + 2 * j), v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j);
+        reinterpret_cast<double2*>(vs)[j] = v0;
+        a4[0] += v0.x * xj.x + v0.y * xj.y;
+        a4[1] += v1.x * xj.x + v1.y * xj.y;
+        a4[2] += v2.x * xj.x + v2.y * xj.y;
+        a4[3] += v3.x * xj.x + v3.y * xj.y;
     }
     block_sum<PT, 4>(a4, red);
     const double rho = a4[0];
@@ -373,36 +491,40 @@ __global__ void __launch_bounds__(PT) k_accept(SysDev s, WalkDev wd, int spin, i
     double* Wb = wd.Wbuf + (long)w * kp * nsp;
     double* Si = wd.SinvT + (long)w * kp * kp;
     const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
-    for (int j = tid; j < nsp; j += PT) {
-        const double vj = v[j];
-        orb[j] = vj;
-        orb[nsp + j] = v[wd.ldv + j];
-        orb[2 * nsp + j] = v[2 * wd.ldv + j];
-        orb[3 * nsp + j] = v[3 * wd.ldv + j];
-        orb[4 * nsp + j] = v[4 * wd.ldv + j];
-        Vb[(long)m * nsp + j] = vj;
-        Wb[(long)m * nsp + j] = arow[j];
-    }
-    // r_l = v . Wbuf[l]  (row m of S)
-    for (int l = warp; l < m; l += PT / 32) {
-        double acc = 0.0;
-        for (int j = lane; j < nsp; j += 32) acc += v[j] * Wb[(long)l * nsp + j];
-        acc = warp_sum(acc);
+    // r_l = v . Wbuf[l]  (row m of S): the streaming pass, issued first
+    for (int l = warp; l < m; l += PW) {
+        const double acc = warp_dot(Wb + (long)l * nsp, vs, nsp, lane);
         if (lane == 0) rs[l] = acc;
     }
+    for (int idx = tid; idx < m * kp; idx += PT) {
+        const int l = idx / kp, n = idx - l * kp;
+        if (n < m) Ss[l * kps + n] = Si[idx];
+    }
     for (int n = tid; n < m; n += PT) cs[n] = wd.cvec[(long)w * kp + n];
+    for (int j = tid; j < nsp / 2; j += PT) {
+        const double2 a = ldg2(arow + 2 * j);
+        const double2 v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j), v4 = ldg2(v + 4 * wd.ldv + 2 * j);
+        const double2 v0 = reinterpret_cast<double2*>(vs)[j];
+        reinterpret_cast<double2*>(orb)[j] = v0;
+        reinterpret_cast<double2*>(orb + nsp)[j] = v1;
+        reinterpret_cast<double2*>(orb + 2 * nsp)[j] = v2;
+        reinterpret_cast<double2*>(orb + 3 * nsp)[j] = v3;
+        reinterpret_cast<double2*>(orb + 4 * nsp)[j] = v4;
+        reinterpret_cast<double2*>(Vb + (long)m * nsp)[j] = v0;
+        reinterpret_cast<double2*>(Wb + (long)m * nsp)[j] = a;
+    }
     __syncthreads();
     // t_l = sum_n r_n Sinv[n][l] = sum_n r_n SinvT[l][n]
     for (int l = tid; l < m; l += PT) {
         double acc = 0.0;
-        for (int n = 0; n < m; n++) acc += rs[n] * Si[l * kp + n];
+        for (int n = 0; n < m; n++) acc += rs[n] * Ss[l * kps + n];
         ts[l] = acc;
     }
     __syncthreads();
     const double sinv = 1.0 / rho;
     for (int idx = tid; idx < m * m; idx += PT) {
         const int l = idx / m, n = idx % m;
-        Si[l * kp + n] += cs[n] * ts[l] * sinv;
+        Si[l * kp + n] = Ss[l * kps + n] + cs[n] * ts[l] * sinv;
     }
     for (int n = tid; n < m; n += PT) {
         Si[m * kp + n] = -cs[n] * sinv;
@@ -416,7 +538,13 @@ __global__ void __launch_bounds__(PT) k_accept(SysDev s, WalkDev wd, int spin, i
 }
 
 cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st) {
-    size_t smem = (size_t)(3 * wd.kp + 8 * (PT / 32) + 4) * sizeof(double);
+    static size_t configured = 48 * 1024;
+    const size_t smem = (size_t)(s.nsp[spin] + 3 * wd.kp + 8 * PW + 4 + wd.kp * (wd.kp + 1)) * sizeof(double);
+    if (smem > configured) {
+        cudaError_t er = cudaFuncSetAttribute(k_accept, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (er != cudaSuccess) return er;
+        configured = smem;
+    }
     k_accept<<<wd.W, PT, smem, st>>>(s, wd, spin, p, e, log_off, tau, commit);
     COUNT_LAUNCH();
     return cudaGetLastError();
@@ -424,47 +552,46 @@ cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, i
 
 // ------------------------------------------------------------------------------------------------
 // a8: delayed rank-k flush as FP64 GEMMs                                           [north_star item 5]
-//   YT[q][n] = AinvT0[q][:] . Vbuf[n][:] - delta(q, p_n)           (n < m; columns n >= m are zero)
+//   YT[q][n] = delta(q, p_n) - AinvT0[q][:] . Vbuf[n][:]           (n < m; columns n >= m are zero)
 //   W2[l][j] = sum_n SinvT[l][n] Wbuf[n][j]
-//   AinvT[q][j] -= sum_l YT[q][l] W2[l][j]
+//   AinvT[q][j] += sum_l YT[q][l] W2[l][j]
 struct EpiY {
+    static constexpr bool preload = false;
     const int* plist; const int* mcount; int kp;
     __device__ bool skip(int b) const { return mcount[b] == 0; }
     __device__ void operator()(int b, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
         if (row >= M || col >= N) return;
         const int m = mcount[b];
         const int* pl = plist + (long)b * kp;
-        v0 = (col < m) ? (v0 - ((pl[col] == row) ? 1.0 : 0.0)) : 0.0;
-        v1 = (col + 1 < m) ? (v1 - ((pl[col + 1] == row) ? 1.0 : 0.0)) : 0.0;
+        v0 = (col < m) ? (((pl[col] == row) ? 1.0 : 0.0) - v0) : 0.0;      // stored negated: the update is A^-T += YT * W2
+        v1 = (col + 1 < m) ? (((pl[col + 1] == row) ? 1.0 : 0.0) - v1) : 0.0;
         *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
     }
 };
 struct EpiStoreSkip {
+    static constexpr bool preload = false;
     const int* mcount;
     __device__ bool skip(int b) const { return mcount[b] == 0; }
     __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
         if (row < M && col < N) *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
     }
 };
-struct EpiSubSkip {
+struct EpiAccumSkip {  // C += A*B: accumulators preloaded from C, plain store
+    static constexpr bool preload = true;
     const int* mcount;
     __device__ bool skip(int b) const { return mcount[b] == 0; }
     __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
-        if (row < M && col < N) {
-            double2* ptr = reinterpret_cast<double2*>(Cb + (long)row * ldc + col);
-            double2 c = *ptr;
-            c.x -= v0; c.y -= v1;
-            *ptr = c;
-        }
+        if (row < M && col < N) *reinterpret_cast<double2*>(Cb + (long)row * ldc + col) = make_double2(v0, v1);
     }
 };
 
 using CfgY16 = GemmCfg<128, 16, 16, 16, true, 4>;
 using CfgY32 = GemmCfg<128, 32, 16, 32, true, 4>;
-using CfgY64 = GemmCfg<128, 64, 32, 32, true, 4>;
+using CfgY64 = GemmCfg<128, 64, 32, 32, true, QMC_Y_STAGES>;
 using CfgY128 = GemmCfg<128, 128, 64, 32, true, 4>;
 using CfgW2 = GemmCfg<64, 128, 32, 32, false, 3>;
-using CfgUpd = GemmCfg<128, 128, 64, 32, false, 3>;
+using CfgUpd = GemmCfg<128, 128, 64, 32, false, 3>;   // Newton-Schulz at creation
+using CfgAcc = GemmCfg<QMC_UPD_BM, QMC_UPD_BN, 64, 32, false, QMC_UPD_STAGES>;  // flush update: several CTAs per SM
 
 __global__ void k_window_reset(WalkDev wd) {
     const int w = blockIdx.x;
@@ -503,12 +630,12 @@ cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStrea
     e = gemm_f64_launch<CfgW2>(g, wd.W, EpiStoreSkip{wd.mcount}, st);
     COUNT_LAUNCH();
     if (e != cudaSuccess) return e;
-    // AinvT -= YT * W2
+    // AinvT += YT * W2
     g.A = wd.YT; g.lda = kp; g.strideA = (long)nsp * kp;
     g.B = wd.W2; g.ldb = nsp; g.strideB = (long)kp * nsp;
     g.C = wd.AinvT[spin]; g.ldc = nsp; g.strideC = (long)nsp * nsp;
     g.M = nsp; g.N = nsp; g.K = kp;
-    e = gemm_f64_launch<CfgUpd>(g, wd.W, EpiSubSkip{wd.mcount}, st);
+    e = gemm_f64_launch<CfgAcc>(g, wd.W, EpiAccumSkip{wd.mcount}, st);
     COUNT_LAUNCH();
     if (e != cudaSuccess) return e;
     return launch_window_reset(wd, st);
@@ -737,6 +864,7 @@ cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batc
 // A read from the value rows of the row cache.  Two batched DMMA GEMMs; brings the Gauss-Jordan result to the
 // accuracy of a backward-stable inverse (residual-limited) at ~4 N^3 flop per matrix.
 struct EpiEyeMinus {
+    static constexpr bool preload = false;
     int ns;
     __device__ bool skip(int) const { return false; }
     __device__ void operator()(int, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
@@ -746,6 +874,7 @@ struct EpiEyeMinus {
     }
 };
 struct EpiAddSrc {
+    static constexpr bool preload = false;
     const double* src; long stride;
     __device__ bool skip(int) const { return false; }
     __device__ void operator()(int b, double* Cb, long ldc, int M, int N, int row, int col, double v0, double v1) const {
