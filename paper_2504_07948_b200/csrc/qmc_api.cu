@@ -176,31 +176,40 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     CUS(cudaMemcpyAsync(dco, coef.data(), coef.size() * 8, cudaMemcpyHostToDevice, st));
     CUS(cudaMemcpyAsync(drec, recs.data(), recs.size() * sizeof(ShellRec), cudaMemcpyHostToDevice, st));
     d.atom_xyz = dxyz; d.atom_Z = dZ; d.alpha = dal; d.coef = dco; d.shells = drec;
-    {   // shells that own a function of each 32-function k-block (a shell may straddle two blocks)
-        std::vector<int2> kbs(d.kb);
+    {   // shells that own a function of each 32-function k-block (a shell may straddle two blocks), grouped by l
+        std::vector<int4> cnts(d.kb);
+        std::vector<KbShell> list;
         int lo = 0;
         for (int kb = 0; kb < d.kb; kb++) {
             const int f_lo = kb * 32, f_hi = f_lo + 32;
             while (lo < basis->n_shells && recs[lo].f0 + 2 * recs[lo].l + 1 <= f_lo) lo++;
             int hi = lo;
             while (hi < basis->n_shells && recs[hi].f0 < f_hi) hi++;
-            kbs[kb] = make_int2(lo, hi);
+            int c[3] = {0, 0, 0};
+            const int off = (int)list.size();
+            for (int l = 0; l < 3; l++)
+                for (int i = lo; i < hi; i++)
+                    if (recs[i].l == l) {
+                        KbShell k;
+                        memset(&k, 0, sizeof(k));
+                        k.x = recs[i].x; k.y = recs[i].y; k.z = recs[i].z;
+                        k.l = recs[i].l; k.f0 = recs[i].f0; k.nprim = recs[i].nprim; k.poff = recs[i].poff;
+                        for (int q = 0; q < 3 && q < recs[i].nprim; q++) { k.a[q] = alpha[recs[i].poff + q]; k.c[q] = coef[recs[i].poff + q]; }
+                        list.push_back(k);
+                        c[l]++;
+                    }
+            cnts[kb] = make_int4(c[0], c[1], c[2], off);
         }
-        int2* dkbs;
-        CUS(S->pool.alloc((void**)&dkbs, kbs.size() * sizeof(int2), st));
-        CUS(cudaMemcpyAsync(dkbs, kbs.data(), kbs.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+        if (list.empty()) { KbShell k; memset(&k, 0, sizeof(k)); list.push_back(k); }
+        int4* dcn;
+        KbShell* dli;
+        CUS(S->pool.alloc((void**)&dcn, cnts.size() * sizeof(int4), st));
+        CUS(S->pool.alloc((void**)&dli, list.size() * sizeof(KbShell), st));
+        CUS(cudaMemcpyAsync(dcn, cnts.data(), cnts.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
+        CUS(cudaMemcpyAsync(dli, list.data(), list.size() * sizeof(KbShell), cudaMemcpyHostToDevice, st));
         CUS(cudaStreamSynchronize(st));
-        d.kb_shells = dkbs;
-        d.max_kb_shells = 1;
-        for (const int2& r : kbs) d.max_kb_shells = std::max(d.max_kb_shells, r.y - r.x);
-        std::vector<int> ftab(d.nbp, -1);
-        for (int i = 0; i < basis->n_shells; i++)
-            for (int m = 0; m < 2 * recs[i].l + 1; m++) ftab[recs[i].f0 + m] = i | (m << 24);
-        int* dft;
-        CUS(S->pool.alloc((void**)&dft, ftab.size() * sizeof(int), st));
-        CUS(cudaMemcpyAsync(dft, ftab.data(), ftab.size() * sizeof(int), cudaMemcpyHostToDevice, st));
-        CUS(cudaStreamSynchronize(st));
-        d.fun_tab = dft;
+        d.kb_counts = dcn;
+        d.kb_list = dli;
     }
     for (int sp = 0; sp < 2; sp++) {
         double* dC;

@@ -23,15 +23,25 @@ struct ShellRec {
     int l, f0, nprim, poff;
 };
 
+// One shell as the basis kernel reads it: a self-contained 96-byte record (six 16-byte loads, no dependent
+// second load for the primitives).  Up to three primitives are inline (unused slots have coef 0, alpha 0 and
+// contribute exactly 0); primitives beyond three are read from alpha/coef at poff + 3.
+struct __align__(16) KbShell {
+    double x, y, z;
+    double a[3];
+    double c[3];
+    int l, f0, nprim, poff;
+    double pad;
+};
+
 struct SysDev {
     int n_atoms, n_shells, n_basis, nbp, kb;  // kb = nbp / 32
     int ns[2], nsp[2], ne;
     const double* atom_xyz;  // [n_atoms][3]
     const double* atom_Z;
     const ShellRec* shells;
-    const int2* kb_shells;  // [kb]: shells [x, y) that own a function of k-block kb (32 functions)
-    const int* fun_tab;     // [nbp]: shell | (m << 24) of every basis function, -1 for the zero padding
-    int max_kb_shells;      // max over k-blocks of y - x
+    const int4* kb_counts;  // [kb]: number of s, p, d shells owning a function of k-block kb (32 functions), list offset
+    const KbShell* kb_list; // shells of every k-block, grouped s | p | d (a shell may be in two blocks)
     const double* alpha;
     const double* coef;
     const double* CT[2];  // tiled, see mo_streamk.cuh

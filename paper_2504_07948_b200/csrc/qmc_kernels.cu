@@ -86,73 +86,79 @@ __device__ __forceinline__ void bulk_s2g(void* gmem_dst, const void* smem_src, u
 constexpr int BASIS_THREADS = 256;
 constexpr int BASIS_MAXPT = (MO_BM + 4) / 5 + 1;  // points that can touch one 128-row tile (27)
 
-// Two phases per tile.  (1) one thread per (point, shell): the contracted radial part g, 2g', (4l+6)g' + 4t g''
-// (three FP64 exp per pair -- the expensive part, done once per shell, never per function);  (2) one thread per
-// (point, function): the five components from the radial triple and the angular polynomial, written to the
-// shared-memory tile with consecutive threads on consecutive columns (conflict free).
-__global__ void __launch_bounds__(BASIS_THREADS) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out) {
-    extern __shared__ __align__(128) double bsm[];
-    double* tile = bsm;                          // [128][36]
-    double* spt = tile + MO_A_STAGE;             // [BASIS_MAXPT][3]
-    double* rad = spt + 3 * BASIS_MAXPT + 3;     // [npt][nsh][3]
+// Work items are (point, shell) pairs, ordered s-shells | p-shells | d-shells of the k-block, so a warp mixes
+// shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
+// stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
+// issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
+__global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out) {
+    __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
+    __shared__ double spt[3 * BASIS_MAXPT + 3];
     const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
-    for (int i = tid; i < MO_A_STAGE / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
     const int row_lo = tm * MO_BM;
     const int pt_lo = row_lo / 5;
     int pt_hi = (row_lo + MO_BM + 4) / 5;
     if (pt_hi > n_points) pt_hi = n_points;
     const int npt = pt_hi - pt_lo;
-    const int2 shr = s.kb_shells[kb];
-    const int nsh = shr.y - shr.x, npair = npt * nsh;
+    const int f_lo = kb * MO_BK;
+    if (row_lo + MO_BM <= 5 * n_points && f_lo + MO_BK <= s.n_basis) {
+        // every (row, function) of the tile gets written below: only the 4 padding columns need zeros
+        for (int i = tid; i < MO_BM * 2; i += BASIS_THREADS)
+            reinterpret_cast<double2*>(tile + (i >> 1) * MO_ALD + MO_BK)[i & 1] = make_double2(0.0, 0.0);
+    } else {
+        for (int i = tid; i < MO_A_STAGE / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
+    }
     if (tid < 3 * npt) spt[tid] = pts[3 * pt_lo + tid];
     __syncthreads();
-    for (int q = tid; q < npair; q += BASIS_THREADS) {
-        const int pi = q / nsh, sh = shr.x + (q - pi * nsh);
-        const ShellRec rec = s.shells[sh];
+    const int4 cnt = s.kb_counts[kb];  // x, y, z = number of s, p, d shells; w = offset of this block's list
+    const KbShell* __restrict__ list = s.kb_list + cnt.w;
+    const int r_base = pt_lo * 5 - row_lo;
+    const int n0 = npt * cnt.x, n1 = n0 + npt * cnt.y, n2 = n1 + npt * cnt.z;
+    for (int q = tid; q < n2; q += BASIS_THREADS) {
+        int L, qq, c, base;
+        if (q < n0) { L = 0; qq = q; c = cnt.x; base = 0; }
+        else if (q < n1) { L = 1; qq = q - n0; c = cnt.y; base = cnt.x; }
+        else { L = 2; qq = q - n1; c = cnt.z; base = cnt.x + cnt.y; }
+        const int pi = qq / c;
+        const KbShell rec = list[base + qq - pi * c];
         const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
         const double t = x * x + y * y + z * z;
-        double g = 0.0, g1 = 0.0, g2 = 0.0;
-        for (int p = 0; p < rec.nprim; p++) {
+        // accumulation order p = 0, 1, 2, ... as in the definition of g, g', g''
+        const double e0 = rec.c[0] * exp(-rec.a[0] * t), e1 = rec.c[1] * exp(-rec.a[1] * t), e2 = rec.c[2] * exp(-rec.a[2] * t);
+        double g = e0, g1 = -(rec.a[0] * e0), g2 = rec.a[0] * rec.a[0] * e0;
+        g += e1; g1 -= rec.a[1] * e1; g2 += rec.a[1] * rec.a[1] * e1;
+        g += e2; g1 -= rec.a[2] * e2; g2 += rec.a[2] * rec.a[2] * e2;
+        for (int p = 3; p < rec.nprim; p++) {
             const double al = __ldg(s.alpha + rec.poff + p);
             const double e = __ldg(s.coef + rec.poff + p) * exp(-al * t);
             g += e;
             g1 -= al * e;
             g2 += al * al * e;
         }
-        rad[3 * q] = g;
-        rad[3 * q + 1] = 2.0 * g1;
-        rad[3 * q + 2] = (double)(4 * rec.l + 6) * g1 + 4.0 * t * g2;
-    }
-    __syncthreads();
-    const int f = kb * MO_BK + (tid & 31);
-    const int ft = s.fun_tab[f];  // shell | m << 24, or -1 for a padding function
-    if (ft >= 0) {
-        const int sh = ft & 0xFFFFFF, m = ft >> 24, c = tid & 31;
-        const ShellRec rec = s.shells[sh];
-        for (int pi = tid >> 5; pi < npt; pi += BASIS_THREADS / 32) {
-            const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
-            const double* rd = rad + 3 * (pi * nsh + (sh - shr.x));
-            const double g = rd[0], tg1 = rd[1], lapfac = rd[2];
-            const double s3 = 1.7320508075688772;
-            double S, Sx, Sy, Sz;
-            if (rec.l == 0) { S = 1.0; Sx = 0.0; Sy = 0.0; Sz = 0.0; }
-            else if (rec.l == 1) {
-                S = m == 0 ? x : (m == 1 ? y : z);
-                Sx = m == 0 ? 1.0 : 0.0; Sy = m == 1 ? 1.0 : 0.0; Sz = m == 2 ? 1.0 : 0.0;
-            } else {
-                switch (m) {
-                    case 0: S = s3 * x * y; Sx = s3 * y; Sy = s3 * x; Sz = 0.0; break;
-                    case 1: S = s3 * y * z; Sx = 0.0; Sy = s3 * z; Sz = s3 * y; break;
-                    case 2: S = z * z - 0.5 * (x * x + y * y); Sx = -x; Sy = -y; Sz = 2.0 * z; break;
-                    case 3: S = s3 * x * z; Sx = s3 * z; Sy = 0.0; Sz = s3 * x; break;
-                    default: S = (0.5 * s3) * (x * x - y * y); Sx = s3 * x; Sy = -s3 * y; Sz = 0.0; break;
-                }
-            }
-            const int r0 = (pt_lo + pi) * 5 - row_lo;  // local row of the value component (may be < 0 or > 123)
+        const int r0 = r_base + pi * 5;  // local row of the value component (may be < 0 or > 123)
+        const int c0 = rec.f0 - f_lo;
+        const double lapfac = (double)(4 * L + 6) * g1 + 4.0 * t * g2;
+        const double tg1 = 2.0 * g1;
+        auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
+            const int col = c0 + m;
+            if (col < 0 || col >= MO_BK) return;
             const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
             for (int k = 0; k < 5; k++)
-                if (r0 + k >= 0 && r0 + k < MO_BM) tile[(r0 + k) * MO_ALD + c] = v[k];
+                if (r0 + k >= 0 && r0 + k < MO_BM) tile[(r0 + k) * MO_ALD + col] = v[k];
+        };
+        const double s3 = 1.7320508075688772;
+        if (L == 0) {
+            emit(0, 1.0, 0.0, 0.0, 0.0);
+        } else if (L == 1) {
+            emit(0, x, 1.0, 0.0, 0.0);
+            emit(1, y, 0.0, 1.0, 0.0);
+            emit(2, z, 0.0, 0.0, 1.0);
+        } else {
+            emit(0, s3 * x * y, s3 * y, s3 * x, 0.0);
+            emit(1, s3 * y * z, 0.0, s3 * z, s3 * y);
+            emit(2, z * z - 0.5 * (x * x + y * y), -x, -y, 2.0 * z);
+            emit(3, s3 * x * z, s3 * z, 0.0, s3 * x);
+            emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
         }
     }
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // generic-proxy smem writes -> visible to the TMA engine
@@ -166,15 +172,8 @@ __global__ void __launch_bounds__(BASIS_THREADS) k_basis(SysDev s, const double*
 
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
-    static int configured_smem = 0;
-    const size_t smem = (size_t)(MO_A_STAGE + 3 * BASIS_MAXPT + 3 + 3 * BASIS_MAXPT * s.max_kb_shells) * sizeof(double);
-    if ((int)smem > configured_smem) {
-        cudaError_t e = cudaFuncSetAttribute(k_basis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured_smem = (int)smem;
-    }
     dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
-    k_basis<<<grid, BASIS_THREADS, smem, st>>>(s, pts, n_points, PhiT);
+    k_basis<<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
@@ -266,7 +265,7 @@ __device__ __forceinline__ double warp_dot(const double* __restrict__ row, const
     return warp_sum(acc);
 }
 
-__global__ void __launch_bounds__(PT) k_propose(SysDev s, WalkDev wd, int spin, int p, int e, uint32_t step, double tau,
+__global__ void __launch_bounds__(PT, 2) k_propose(SysDev s, WalkDev wd, int spin, int p, int e, uint32_t step, double tau,
                                                 double sqrt_tau) {
     extern __shared__ __align__(16) double sm[];
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -418,7 +417,7 @@ cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, 
 // ------------------------------------------------------------------------------------------------
 // a5 + a7: determinant ratio and gradient from the effective column, accept/reject, commit.
 // One CTA per walker.  commit == 0 evaluates everything but changes no state (stage timing).
-__global__ void __launch_bounds__(PT) k_accept(SysDev s, WalkDev wd, int spin, int p, int e, long log_off, double tau, int commit) {
+__global__ void __launch_bounds__(PT, 2) k_accept(SysDev s, WalkDev wd, int spin, int p, int e, long log_off, double tau, int commit) {
     extern __shared__ __align__(16) double sm[];
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
