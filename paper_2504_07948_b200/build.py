@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmc_b200.so")
 SOURCES = ["qmc_api.cu", "qmc_kernels.cu"]
-HEADERS = ["qmc_kernels.cuh", "qmc_internal.cuh", "gemm_f64.cuh", "mo_streamk.cuh", os.path.join("..", "..", "include", "qmc.h")]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh")) + [os.path.join("..", "..", "include", "qmc.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr", "--expt-extended-lambda"]
 

@@ -424,7 +424,8 @@ static void prof_collect(qmc_walkers* w) {
     t.used = 0;
 }
 
-/* stage ids: 0 propose, 1 basis, 2 MO contraction, 3 accept, 4 flush, 5 local energy */
+/* stage ids: 0 step kernel with one half (first proposal / last accept of a delay window), 1 basis, 2 MO contraction,
+   3 fused step kernel (accept of p + proposal of p + 1), 4 flush, 5 local energy */
 extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
     if (!w || stride < 0) return fail(QMC_ERR_ARG, "qmc_set_profiling");
     prof_collect(w);
@@ -475,25 +476,32 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
                 const int e = e0 + p;
                 const long log_off = ((long)t * s.ne + e) * d.W;
                 const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
-                prof_begin(w, 0, prof);
-                CU(launch_propose(s, d, sp, p, e, w->step, tau, st));
-                prof_end(w, prof);
+                if (in_window == 0) {  // first proposal of a window: nothing to fuse it with
+                    prof_begin(w, 0, prof);
+                    CU(launch_step(s, d, sp, -1, p, 0, w->step, tau, 1, st));
+                    prof_end(w, prof);
+                }
                 prof_begin(w, 1, prof);
                 CU(launch_basis(s, d.rp, d.W, d.Phi, st));
                 prof_end(w, prof);
                 prof_begin(w, 2, prof);
                 CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch, st));
                 prof_end(w, prof);
-                prof_begin(w, 3, prof);
-                CU(launch_accept(s, d, sp, p, e, log_off, tau, 1, st));
-                prof_end(w, prof);
                 in_window++;
                 if (in_window == delay_k || p == ns - 1) {
+                    prof_begin(w, 0, prof);
+                    CU(launch_step(s, d, sp, p, -1, log_off, w->step, tau, 1, st));
+                    prof_end(w, prof);
                     const bool pf = w->prof_stride > 0;
                     prof_begin(w, 4, pf);
                     CU(launch_flush(s, d, sp, st));
                     prof_end(w, pf);
                     in_window = 0;
+                } else {  // accept/reject of p and proposal of p + 1 in one launch
+                    const bool prof2 = w->prof_stride > 0 && ((p + 1) % w->prof_stride) == 0;
+                    prof_begin(w, 3, prof2);
+                    CU(launch_step(s, d, sp, p, p + 1, log_off, w->step, tau, 1, st));
+                    prof_end(w, prof2);
                 }
             }
         }
@@ -667,7 +675,7 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
     CU(cudaEventCreate(&e0));
     CU(cudaEventCreate(&e1));
     // make the inputs of the later stages valid
-    CU(launch_propose(s, d, spin, p, e, w->step, 0.005, st));
+    CU(launch_step(s, d, spin, -1, p, 0, w->step, 0.005, 1, st));
     const int mgrid = mo_grid_for(s, spin, 5 * d.W, d.mo_grid);
     CU(launch_basis(s, d.rp, d.W, d.Phi, st));
     CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st));
@@ -677,10 +685,10 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
         if (r == 0) err = cudaEventRecord(e0, st);
         if (err != cudaSuccess) break;
         switch (stage) {
-            case 0: err = launch_propose(s, d, spin, p, e, w->step, 0.005, st); break;
+            case 0: err = launch_step(s, d, spin, -1, p, 0, w->step, 0.005, 1, st); break;
             case 1: err = launch_basis(s, d.rp, d.W, d.Phi, st); break;
             case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st); break;
-            case 3: err = launch_accept(s, d, spin, p, e, 0, 0.005, 0, st); break;
+            case 3: err = launch_step(s, d, spin, p, p, 0, w->step, 0.005, 0, st); break;
             case 4:
                 err = launch_flush(s, d, spin, st);
                 if (err == cudaSuccess) err = launch_fill_int(d.mcount, d.W, delay_k, st);

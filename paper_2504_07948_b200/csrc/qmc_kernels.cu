@@ -6,6 +6,8 @@
 
 #include "gemm_f64.cuh"
 #include "mo_streamk.cuh"
+#include "device_utils.cuh"
+#include "step_kernel.cuh"
 
 #ifndef QMC_UPD_BM
 #define QMC_UPD_BM 128
@@ -20,57 +22,6 @@ namespace qmc {
 
 thread_local uint64_t g_launches = 0;
 #define COUNT_LAUNCH() (++g_launches)
-
-// ------------------------------------------------------------------------------------------------
-// block reductions (fixed shape -> deterministic): NV sums at once over a block of NT threads
-template <int NT, int NV>
-__device__ __forceinline__ void block_sum(double (&v)[NV], double* red /* [NV * NT/32] */) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int i = 0; i < NV; i++) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
-    }
-    __syncthreads();  // protect red from a previous use
-    if (lane == 0) {
-#pragma unroll
-        for (int i = 0; i < NV; i++) red[i * (NT / 32) + warp] = v[i];
-    }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < NV; i++) {
-        double s = 0.0;
-#pragma unroll
-        for (int k = 0; k < NT / 32; k++) s += red[i * (NT / 32) + k];
-        v[i] = s;
-    }
-}
-
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// ------------------------------------------------------------------------------------------------
-// Philox4x32-10, key = (seed lo, seed hi), counter = (walker, step, electron, block)   [reading A11]
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
-                                              uint32_t (&out)[4]) {
-#pragma unroll
-    for (int r = 0; r < 10; r++) {
-        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
-    }
-    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
-}
-__device__ __forceinline__ double u01(uint32_t we, uint32_t wo) {
-    unsigned long long x = ((unsigned long long)we << 32) | (unsigned long long)wo;
-    return (double)(2ull * (x >> 12) + 1ull) * 0x1.0p-53;  // odd integer * 2^-53: exact, in (0,1)
-}
 
 // ------------------------------------------------------------------------------------------------
 // a3: basis functions (value, gradient, laplacian) at the proposed positions          [north_star item 1]
@@ -207,344 +158,17 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 }
 
 // ------------------------------------------------------------------------------------------------
-// Pade Jastrow pieces
-__device__ __forceinline__ double pade_u(double a, double b, double r) { return a * r / (1.0 + b * r); }
-__device__ __forceinline__ double pade_du(double a, double b, double r) { double q = 1.0 + b * r; return a / (q * q); }
-__device__ __forceinline__ double pade_d2u(double a, double b, double r) { double q = 1.0 + b * r; return -2.0 * a * b / (q * q * q); }
-
-// partner k of electron e: k < ne electrons (skip k == e), then atoms
-struct Partner { double x, y, z, a, b; bool ok; };
-__device__ __forceinline__ Partner partner(const SysDev& s, const double* __restrict__ Rw, int nep, int e, int k) {
-    Partner P;
-    if (k < s.ne) {
-        P.x = Rw[k]; P.y = Rw[nep + k]; P.z = Rw[2 * nep + k];
-        const bool same = (k < s.ns[0]) == (e < s.ns[0]);
-        P.a = same ? s.a_para : s.a_anti;
-        P.b = s.b_ee;
-        P.ok = (k != e);
-    } else {
-        const int I = k - s.ne;
-        P.x = s.atom_xyz[3 * I]; P.y = s.atom_xyz[3 * I + 1]; P.z = s.atom_xyz[3 * I + 2];
-        P.a = -s.atom_Z[I];
-        P.b = s.b_en;
-        P.ok = true;
-    }
-    return P;
-}
-
-// ------------------------------------------------------------------------------------------------
-// a1 + a2 + a6: effective inverse column, drift, Philox proposal, Jastrow ratio and gradient at r'.
-// One CTA of 512 threads per walker.  The two streaming passes over the delay window (b = Vbuf a_p, then
-// x = a_p - Wbuf^T c) are HBM-bound GEMVs: every thread keeps 8 independent 16-byte loads in flight.
-//                                                                               [north_star items 3, 4]
-constexpr int PT = 512;
-constexpr int PW = PT / 32;
-
-__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
-
-// dot products of row[0..n) with xs[0..n) (n % 2 == 0), one warp, 8 loads in flight per lane
-__device__ __forceinline__ double warp_dot(const double* __restrict__ row, const double* xs, int n, int lane) {
-    double acc = 0.0;
-    const int n2 = n >> 1;
-    int j = lane;
-    for (; j + 7 * 32 < n2; j += 8 * 32) {
-        double2 a[8];
-#pragma unroll
-        for (int u = 0; u < 8; u++) a[u] = ldg2(row + 2 * (j + u * 32));
-#pragma unroll
-        for (int u = 0; u < 8; u++) {
-            const double2 x = *reinterpret_cast<const double2*>(xs + 2 * (j + u * 32));
-            acc += a[u].x * x.x + a[u].y * x.y;
-        }
-    }
-    for (; j < n2; j += 32) {
-        const double2 a = ldg2(row + 2 * j);
-        const double2 x = *reinterpret_cast<const double2*>(xs + 2 * j);
-        acc += a.x * x.x + a.y * x.y;
-    }
-    return warp_sum(acc);
-}
-
-__global__ void __launch_bounds__(PT, 2) k_propose(SysDev s, WalkDev wd, int spin, int p, int e, uint32_t step, double tau,
-                                                double sqrt_tau) {
-    extern __shared__ __align__(16) double sm[];
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
-    const int kps = kp + 1;            // padded row stride of the S^-1 copy (conflict-free column walks)
-    double* xs = sm;                   // [nsp]
-    double* bs = xs + nsp;             // [kp]
-    double* cs = bs + kp;              // [kp]
-    double* red = cs + kp;             // [8 * PW]
-    double* bc = red + 8 * PW;         // [4] broadcast
-    double* Ss = bc + 4;               // [kp][kp + 1]
-    const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
-    const int m = wd.mcount[w];
-    for (int j = tid; j < nsp / 2; j += PT) reinterpret_cast<double2*>(xs)[j] = ldg2(arow + 2 * j);
-    if (m > 0) {
-        const double* Si = wd.SinvT + (long)w * kp * kp;
-        for (int idx = tid; idx < m * kp; idx += PT) {
-            const int l = idx / kp, n = idx - l * kp;
-            if (n < m) Ss[l * kps + n] = Si[idx];
-        }
-    }
-    __syncthreads();
-    if (m > 0) {
-        // b_n = v_n . a_p ;  c = S^-1 b ;  x = a_p - Wbuf^T c     (effective column of the delayed inverse)
-        const double* Vb = wd.Vbuf + (long)w * kp * nsp;
-        const double* Wb = wd.Wbuf + (long)w * kp * nsp;
-        for (int n = warp; n < m; n += PW) {
-            const double acc = warp_dot(Vb + (long)n * nsp, xs, nsp, lane);
-            if (lane == 0) bs[n] = acc;
-        }
-        __syncthreads();
-        for (int n = tid; n < m; n += PT) {
-            double acc = 0.0;
-            for (int l = 0; l < m; l++) acc += Ss[l * kps + n] * bs[l];
-            cs[n] = acc;
-            wd.cvec[(long)w * kp + n] = acc;
-        }
-        __syncthreads();
-        for (int j = tid; j < nsp / 2; j += PT) {
-            double2 acc = reinterpret_cast<double2*>(xs)[j];
-            int l = 0;
-            for (; l + 8 <= m; l += 8) {
-                double2 wv[8];
-#pragma unroll
-                for (int u = 0; u < 8; u++) wv[u] = ldg2(Wb + (long)(l + u) * nsp + 2 * j);
-#pragma unroll
-                for (int u = 0; u < 8; u++) { acc.x -= cs[l + u] * wv[u].x; acc.y -= cs[l + u] * wv[u].y; }
-            }
-            for (; l < m; l++) {
-                const double2 wv = ldg2(Wb + (long)l * nsp + 2 * j);
-                acc.x -= cs[l] * wv.x; acc.y -= cs[l] * wv.y;
-            }
-            reinterpret_cast<double2*>(xs)[j] = acc;
-        }
-        __syncthreads();
-    }
-    double* xcol = wd.xcol + (long)w * nsp;
-    for (int j = tid; j < nsp / 2; j += PT) reinterpret_cast<double2*>(xcol)[j] = reinterpret_cast<double2*>(xs)[j];
-
-    // drift: determinant part from the cached gradient rows, Jastrow part by direct sums
-    const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
-    const double* Rw = wd.R + (long)w * 3 * nep;
-    const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
-    double acc6[6] = {0, 0, 0, 0, 0, 0};
-    for (int j = tid; j < nsp / 2; j += PT) {
-        const double2 xj = reinterpret_cast<double2*>(xs)[j];
-        const double2 o1 = ldg2(orb + nsp + 2 * j), o2 = ldg2(orb + 2 * nsp + 2 * j), o3 = ldg2(orb + 3 * nsp + 2 * j);
-        acc6[0] += o1.x * xj.x + o1.y * xj.y;
-        acc6[1] += o2.x * xj.x + o2.y * xj.y;
-        acc6[2] += o3.x * xj.x + o3.y * xj.y;
-    }
-    const int npart = s.ne + s.n_atoms;
-    for (int k = tid; k < npart; k += PT) {
-        Partner P = partner(s, Rw, nep, e, k);
-        if (P.ok) {
-            const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
-            const double r = sqrt(dx * dx + dy * dy + dz * dz);
-            const double du = pade_du(P.a, P.b, r);
-            acc6[3] += du * dx / r;
-            acc6[4] += du * dy / r;
-            acc6[5] += du * dz / r;
-        }
-    }
-    block_sum<PT, 6>(acc6, red);
-    if (tid == 0) {
-        const double Gx = acc6[0] + acc6[3], Gy = acc6[1] + acc6[4], Gz = acc6[2] + acc6[5];
-        const uint32_t wid = wd.first_walker + (uint32_t)w;
-        const uint32_t k0 = (uint32_t)(wd.seed & 0xFFFFFFFFull), k1 = (uint32_t)(wd.seed >> 32);
-        uint32_t o[4];
-        philox4x32_10(wid, step, (uint32_t)e, 0u, k0, k1, o);
-        const double U1 = u01(o[0], o[1]), U2 = u01(o[2], o[3]);
-        philox4x32_10(wid, step, (uint32_t)e, 1u, k0, k1, o);
-        const double U3 = u01(o[0], o[1]), U4 = u01(o[2], o[3]);
-        philox4x32_10(wid, step, (uint32_t)e, 2u, k0, k1, o);
-        const double U5 = u01(o[0], o[1]);
-        const double TWO_PI = 6.283185307179586;
-        const double r1 = sqrt(-2.0 * log(U1)), r2 = sqrt(-2.0 * log(U3));
-        const double chx = r1 * cos(TWO_PI * U2), chy = r1 * sin(TWO_PI * U2), chz = r2 * cos(TWO_PI * U4);
-        const double qx = rx + tau * Gx + sqrt_tau * chx;
-        const double qy = ry + tau * Gy + sqrt_tau * chy;
-        const double qz = rz + tau * Gz + sqrt_tau * chz;
-        wd.rp[3 * w] = qx; wd.rp[3 * w + 1] = qy; wd.rp[3 * w + 2] = qz;
-        wd.G[3 * w] = Gx; wd.G[3 * w + 1] = Gy; wd.G[3 * w + 2] = Gz;
-        wd.u[w] = U5;
-        bc[0] = qx; bc[1] = qy; bc[2] = qz;
-    }
-    __syncthreads();
-    const double qx = bc[0], qy = bc[1], qz = bc[2];
-    // Jastrow ratio (term by term) and gradient at r'
-    double acc4[4] = {0, 0, 0, 0};
-    for (int k = tid; k < npart; k += PT) {
-        Partner P = partner(s, Rw, nep, e, k);
-        if (P.ok) {
-            const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
-            const double ex = qx - P.x, ey = qy - P.y, ez = qz - P.z;
-            const double r_old = sqrt(dx * dx + dy * dy + dz * dz);
-            const double r_new = sqrt(ex * ex + ey * ey + ez * ez);
-            acc4[0] += pade_u(P.a, P.b, r_new) - pade_u(P.a, P.b, r_old);
-            const double du = pade_du(P.a, P.b, r_new);
-            acc4[1] += du * ex / r_new;
-            acc4[2] += du * ey / r_new;
-            acc4[3] += du * ez / r_new;
-        }
-    }
-    block_sum<PT, 4>(acc4, red);
-    if (tid == 0) {
-        wd.dJ[w] = acc4[0];
-        wd.gJn[3 * w] = acc4[1]; wd.gJn[3 * w + 1] = acc4[2]; wd.gJn[3 * w + 2] = acc4[3];
-    }
-}
-
-size_t propose_smem(const SysDev& s, const WalkDev& wd, int spin) {
-    return (size_t)(s.nsp[spin] + 2 * wd.kp + 8 * PW + 4 + wd.kp * (wd.kp + 1)) * sizeof(double);
-}
-
-cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st) {
+// a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
+cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
+                        int commit, cudaStream_t st) {
     static size_t configured = 48 * 1024;
-    const size_t smem = propose_smem(s, wd, spin);
+    const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp);
     if (smem > configured) {
-        cudaError_t er = cudaFuncSetAttribute(k_propose, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t er = cudaFuncSetAttribute(k_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (er != cudaSuccess) return er;
         configured = smem;
     }
-    k_propose<<<wd.W, PT, smem, st>>>(s, wd, spin, p, e, step, tau, sqrt(tau));
-    COUNT_LAUNCH();
-    return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------------
-// a5 + a7: determinant ratio and gradient from the effective column, accept/reject, commit.
-// One CTA per walker.  commit == 0 evaluates everything but changes no state (stage timing).
-__global__ void __launch_bounds__(PT, 2) k_accept(SysDev s, WalkDev wd, int spin, int p, int e, long log_off, double tau, int commit) {
-    extern __shared__ __align__(16) double sm[];
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nsp = s.nsp[spin], kp = wd.kp, nep = wd.nep;
-    const int kps = kp + 1;
-    double* vs = sm;                   // [nsp] value row of the proposed position
-    double* rs = vs + nsp;             // [kp]
-    double* ts = rs + kp;              // [kp]
-    double* cs = ts + kp;              // [kp]
-    double* red = cs + kp;             // [8 * PW]
-    double* bc = red + 8 * PW;         // [4]
-    double* Ss = bc + 4;               // [kp][kp + 1]
-    const double* v = wd.V + (long)w * 5 * wd.ldv;
-    const double* xcol = wd.xcol + (long)w * nsp;
-    double a4[4] = {0, 0, 0, 0};
-    for (int j = tid; j < nsp / 2; j += PT) {
-        const double2 xj = ldg2(xcol + 2 * j);
-        const double2 v0 = ldg2(v + 2 * j), v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j);
-        reinterpret_cast<double2*>(vs)[j] = v0;
-        a4[0] += v0.x * xj.x + v0.y * xj.y;
-        a4[1] += v1.x * xj.x + v1.y * xj.y;
-        a4[2] += v2.x * xj.x + v2.y * xj.y;
-        a4[3] += v3.x * xj.x + v3.y * xj.y;
-    }
-    block_sum<PT, 4>(a4, red);
-    const double rho = a4[0];
-    if (tid == 0) {
-        double* Rw = wd.R + (long)w * 3 * nep;
-        const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
-        const double qx = wd.rp[3 * w], qy = wd.rp[3 * w + 1], qz = wd.rp[3 * w + 2];
-        const double Gx = wd.G[3 * w], Gy = wd.G[3 * w + 1], Gz = wd.G[3 * w + 2];
-        const double u = wd.u[w], dJ = wd.dJ[w];
-        unsigned bits = 0;
-        double pacc = 0.0, jr = 0.0;
-        bool accept = false;
-        if (fabs(rho) < 1e-12) bits |= 2u;
-        if (rho > 0.0) {  // fixed node: reject rho_D <= 0 (A7); NaN fails the comparison and rejects
-            const double Hx = a4[1] / rho + wd.gJn[3 * w], Hy = a4[2] / rho + wd.gJn[3 * w + 1], Hz = a4[3] / rho + wd.gJn[3 * w + 2];
-            const double ax = qx - rx - tau * Gx, ay = qy - ry - tau * Gy, az = qz - rz - tau * Gz;
-            const double cx = rx - qx - tau * Hx, cy = ry - qy - tau * Hy, cz = rz - qz - tau * Hz;
-            const double fwd = ax * ax + ay * ay + az * az, rev = cx * cx + cy * cy + cz * cz;
-            const double Delta = (fwd - rev) / (2.0 * tau);
-            pacc = rho * rho * exp(2.0 * dJ + Delta);  // A25: linear domain, one exp
-            jr = rho * exp(dJ);
-            if (fabs(u - pacc) < 1e-12) bits |= 2u;
-            accept = (u < pacc);
-        }
-        const bool nonfinite = isnan(rho) || isnan(pacc);
-        if (nonfinite) { bits |= 4u; accept = false; }
-        if (accept) bits |= 1u;
-        if (commit) {
-            wd.bits[log_off + w] = (uint8_t)bits;
-            if (wd.ratio_log) { wd.ratio_log[log_off + w] = jr; wd.pacc_log[log_off + w] = pacc; }
-            atomicAdd(&wd.stats[0], 1ull);
-            if (accept) atomicAdd(&wd.stats[1], 1ull);
-            if (bits & 2u) atomicAdd(&wd.stats[2], 1ull);
-            if (nonfinite) { atomicAdd(&wd.stats[3], 1ull); wd.flags[w] = 1u; }
-            if (accept) {
-                Rw[e] = qx; Rw[nep + e] = qy; Rw[2 * nep + e] = qz;
-                wd.logpsi[w] += log(rho) + dJ;
-            }
-        }
-        bc[0] = (accept && commit) ? 1.0 : 0.0;
-    }
-    __syncthreads();
-    if (bc[0] == 0.0) return;
-    // ---- commit: row caches, delay window (Vbuf, Wbuf, bordered update of S^-1)
-    const int m = wd.mcount[w];
-    double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
-    double* Vb = wd.Vbuf + (long)w * kp * nsp;
-    double* Wb = wd.Wbuf + (long)w * kp * nsp;
-    double* Si = wd.SinvT + (long)w * kp * kp;
-    const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
-    // r_l = v . Wbuf[l]  (row m of S): the streaming pass, issued first
-    for (int l = warp; l < m; l += PW) {
-        const double acc = warp_dot(Wb + (long)l * nsp, vs, nsp, lane);
-        if (lane == 0) rs[l] = acc;
-    }
-    for (int idx = tid; idx < m * kp; idx += PT) {
-        const int l = idx / kp, n = idx - l * kp;
-        if (n < m) Ss[l * kps + n] = Si[idx];
-    }
-    for (int n = tid; n < m; n += PT) cs[n] = wd.cvec[(long)w * kp + n];
-    for (int j = tid; j < nsp / 2; j += PT) {
-        const double2 a = ldg2(arow + 2 * j);
-        const double2 v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j), v4 = ldg2(v + 4 * wd.ldv + 2 * j);
-        const double2 v0 = reinterpret_cast<double2*>(vs)[j];
-        reinterpret_cast<double2*>(orb)[j] = v0;
-        reinterpret_cast<double2*>(orb + nsp)[j] = v1;
-        reinterpret_cast<double2*>(orb + 2 * nsp)[j] = v2;
-        reinterpret_cast<double2*>(orb + 3 * nsp)[j] = v3;
-        reinterpret_cast<double2*>(orb + 4 * nsp)[j] = v4;
-        reinterpret_cast<double2*>(Vb + (long)m * nsp)[j] = v0;
-        reinterpret_cast<double2*>(Wb + (long)m * nsp)[j] = a;
-    }
-    __syncthreads();
-    // t_l = sum_n r_n Sinv[n][l] = sum_n r_n SinvT[l][n]
-    for (int l = tid; l < m; l += PT) {
-        double acc = 0.0;
-        for (int n = 0; n < m; n++) acc += rs[n] * Ss[l * kps + n];
-        ts[l] = acc;
-    }
-    __syncthreads();
-    const double sinv = 1.0 / rho;
-    for (int idx = tid; idx < m * m; idx += PT) {
-        const int l = idx / m, n = idx % m;
-        Si[l * kp + n] = Ss[l * kps + n] + cs[n] * ts[l] * sinv;
-    }
-    for (int n = tid; n < m; n += PT) {
-        Si[m * kp + n] = -cs[n] * sinv;
-        Si[n * kp + m] = -ts[n] * sinv;
-    }
-    if (tid == 0) {
-        Si[m * kp + m] = sinv;
-        wd.plist[(long)w * kp + m] = p;
-        wd.mcount[w] = m + 1;
-    }
-}
-
-cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st) {
-    static size_t configured = 48 * 1024;
-    const size_t smem = (size_t)(s.nsp[spin] + 3 * wd.kp + 8 * PW + 4 + wd.kp * (wd.kp + 1)) * sizeof(double);
-    if (smem > configured) {
-        cudaError_t er = cudaFuncSetAttribute(k_accept, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (er != cudaSuccess) return er;
-        configured = smem;
-    }
-    k_accept<<<wd.W, PT, smem, st>>>(s, wd, spin, p, e, log_off, tau, commit);
+    k_step<<<wd.W, PT, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

@@ -12,8 +12,9 @@ size_t mo_ws_bytes(int grid);
 size_t phiT_bytes(const SysDev& s, int rows);
 cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, cudaStream_t st);
 cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, double* out, cudaStream_t st);
-cudaError_t launch_propose(const SysDev& s, const WalkDev& wd, int spin, int p, int e, uint32_t step, double tau, cudaStream_t st);
-cudaError_t launch_accept(const SysDev& s, const WalkDev& wd, int spin, int p, int e, long log_off, double tau, int commit, cudaStream_t st);
+// p_acc >= 0: ratio + accept/reject + commit of electron p_acc (spin-local index); p_prop >= 0: proposal of p_prop
+cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
+                        int commit, cudaStream_t st);
 cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st);
 cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_eloc(const SysDev& s, const WalkDev& wd, cudaStream_t st);
