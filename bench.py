@@ -61,6 +61,38 @@ def flop_model(sysm, n_moves, n_accepted):
     return n_moves * 2.0 * 5 * sysm.n_basis * ns + n_accepted * 4.0 * ns * ns
 
 
+def stage_rooflines(sysm, W, k, acc, ms, hbm_gbs, fp64_tflops):
+    """Per-stage roofline fractions: algorithmic bytes or flops of ONE launch of each stage over
+    its mean duration measured in the timed region.  acc = accepted fraction; the mean number of rows pending in the
+    delay window when a fused step kernel runs is acc*(k-1)/2."""
+    ns, nb, ne, na = sysm.n_up, sysm.n_basis, sysm.n_elec, sysm.n_atoms
+    mbar = acc * (k - 1) / 2.0
+    per_walker_step = (8.0 * ns * (5 + 1 + 1 + acc * (5 + 2) + 1 + 3 + 1)          # V rows, x column r/w, a_p rows, row caches, new window rows
+                       + 8.0 * ns * mbar * (acc * 1 + 2)                            # Wbuf (commit), Vbuf + Wbuf (proposal)
+                       + 8.0 * mbar * mbar * (acc * 2 + 1)                          # S^-1 update and use
+                       + 2 * 24.0 * (ne + na))                                      # partner coordinates, two Jastrow passes
+    m = acc * k
+    alg = {
+        "basis": ("hbm", 8.0 * 5 * W * nb),
+        "mo": ("tensor", 2.0 * 5 * W * nb * ns),
+        "step": ("hbm", W * per_walker_step),
+        "flush": ("tensor", W * (4.0 * m * ns * ns + 2.0 * m * m * ns)),
+        "eloc": ("hbm", W * (40.0 * ns * ne + 24.0 * ne)),
+    }
+    out = {}
+    for st, (bound, amount) in alg.items():
+        t = ms.get(st)
+        if not t:
+            continue
+        if bound == "hbm":
+            a = amount / (t * 1e-3) * 1e-9
+            out[st] = dict(bound="hbm", achieved=a, peak=hbm_gbs, unit="GB/s", frac=a / hbm_gbs, bytes_per_launch=amount)
+        else:
+            a = amount / (t * 1e-3) * 1e-12
+            out[st] = dict(bound="tensor", achieved=a, peak=fp64_tflops, unit="TFLOP/s", frac=a / fp64_tflops, flop_per_launch=amount)
+    return out
+
+
 # ---------------------------------------------------------------------------------------- clocks
 
 class ClockSampler:
@@ -272,8 +304,10 @@ def run_ours(args):
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except (OSError, ValueError):
         pass
-    share = {s: stage[s][0] * (args.prof_stride if s in ("propose", "basis", "mo", "accept") else 1.0) for s in stage}
+    share = {s: stage[s][0] * (args.prof_stride if s in ("step", "basis", "mo") else 1.0) for s in stage}
     tot_share = sum(share.values()) or 1.0
+    hbm_gbs = peaks.get("hbm_gbs") or 6650.0
+    stage_ms = {s: (stage[s][0] / stage[s][1] if stage[s][1] else None) for s in stage}
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=red["elapsed_ms"] / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
@@ -282,7 +316,7 @@ def run_ours(args):
                     moves_per_step=W * sysm.n_elec * world, l2="per-step working set (A^-1 + row caches, ~25 GB/GPU) >> 126 MB L2; no flush needed",
                     prof_stride=args.prof_stride),
         clocks=clocks, e2e=e2e, gpu_launches=int(launches),
-        roofline=dict(kernel="gemm_f64_kernel (MO contraction V = Phi*C, DMMA m8n8k4)", bound="tensor", achieved=achieved,
+        roofline=dict(kernel="k_mo_streamk (MO contraction V = Phi*C, persistent stream-K, DMMA m8n8k4)", bound="tensor", achieved=achieved,
                       peak=peak, unit="TFLOP/s", frac=(achieved / peak) if achieved else None, traffic=traffic,
                       peak_source="FP64 DMMA issue-rate loop measured in this run (qmc_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                       peak_alt_bf16_scaled=(peaks.get("bf16_tflops_sustained", 0) * 37.2 / 2250.0) or None,
@@ -290,7 +324,9 @@ def run_ours(args):
                       share_of_step=share["mo"] / tot_share),
         fp64_tflops_model=flop_model(sysm, red["n_moves"], n_acc * world) / secs * 1e-12,
         accept_frac=n_acc / max(n_moves, 1),
-        stage_ms_per_launch={s: (stage[s][0] / stage[s][1] if stage[s][1] else None) for s in stage},
+        stage_ms_per_launch=stage_ms,
+        stage_roofline=stage_rooflines(sysm, W, k, n_acc / max(n_moves, 1), stage_ms, hbm_gbs, peak),
+        hbm_peak_source="MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "6.65 TB/s of fallback (B200_PROFILING.md)",
         stage_share={s: share[s] / tot_share for s in share},
         eloc_mean=red["e_sum"] / red["n_walkers"],
     )

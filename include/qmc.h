@@ -134,15 +134,17 @@ int qmc_eval_basis(const qmc_system* sys, int n_points, const double* xyz /* [n]
 /* Orbital rows at n_points positions: out[n][5][n_s] (basis kernel + FP64 contraction kernel). */
 int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream);
 /* Time `reps` launches of one stage of the move on the walker set's current state with CUDA events on its
- * stream (no state is committed).  stage: 0 = propose (drift + RNG + Jastrow), 1 = basis, 2 = MO contraction,
- * 3 = ratio/accept (decision suppressed), 4 = delayed-update flush at full window (A^-1 unchanged: zero
- * correction), 5 = local energy.  Returns mean milliseconds per launch. */
+ * stream (no state is committed).  stage: 0 = step kernel, proposal half only (effective column + drift + RNG +
+ * Jastrow), 1 = basis, 2 = MO contraction, 3 = step kernel with both halves (ratio/accept with the decision
+ * suppressed + proposal), 4 = delayed-update flush at full window (A^-1 unchanged: zero correction),
+ * 5 = local energy.  Returns mean milliseconds per launch. */
 int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, double* ms_per_launch);
-/* In-situ stage timing: with stride > 0, qmc_sweep brackets the four per-electron stages of every
- * stride-th electron, every flush and every local-energy evaluation with CUDA events on the walker set's
- * stream.  qmc_get_stage_times synchronises and returns accumulated milliseconds and launch counts per
- * stage id (same ids as qmc_time_stage; a "launch" of stage 4 is the whole flush = 4 kernels, of stage 5
- * two kernels).  stride = 0 turns it off and clears the totals. */
+/* In-situ stage timing: with stride > 0, qmc_sweep brackets the three per-electron launches (fused step
+ * kernel = stage 3, basis, MO contraction) of every stride-th electron, and every half-step launch (stage 0:
+ * the first proposal and the last accept of a delay window), flush and local-energy evaluation, with CUDA
+ * events on the walker set's stream.  qmc_get_stage_times synchronises and returns accumulated milliseconds
+ * and launch counts per stage id (a "launch" of stage 4 is the whole flush = 4 kernels, of stage 5 two
+ * kernels).  stride = 0 turns it off and clears the totals. */
 int qmc_set_profiling(qmc_walkers* w, int stride);
 int qmc_get_stage_times(qmc_walkers* w, double* ms /* [6] */, uint64_t* counts /* [6] */);
 /* Register-resident DMMA issue-rate loop for `ms_target` milliseconds: the FP64 ceiling of this GPU as

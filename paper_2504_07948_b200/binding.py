@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libqmc_b200.so")
 
 QMC_OK, QMC_ERR_ARG, QMC_ERR_CUDA, QMC_ERR_SINGULAR, QMC_ERR_NOMEM, QMC_ERR_STATE = 0, -1, -2, -3, -4, -5
 QMC_LOG_RATIOS = 1
-STAGES = ("propose", "basis", "mo", "accept", "flush", "eloc")
+STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc")
 
 EXPORTED = [
     "qmc_init", "qmc_finalize", "qmc_walkers_create", "qmc_walkers_destroy", "qmc_sweep", "qmc_get_positions",

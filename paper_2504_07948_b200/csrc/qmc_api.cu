@@ -476,10 +476,11 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
                 const int e = e0 + p;
                 const long log_off = ((long)t * s.ne + e) * d.W;
                 const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
+                const bool pf = w->prof_stride > 0;
                 if (in_window == 0) {  // first proposal of a window: nothing to fuse it with
-                    prof_begin(w, 0, prof);
+                    prof_begin(w, 0, pf);
                     CU(launch_step(s, d, sp, -1, p, 0, w->step, tau, 1, st));
-                    prof_end(w, prof);
+                    prof_end(w, pf);
                 }
                 prof_begin(w, 1, prof);
                 CU(launch_basis(s, d.rp, d.W, d.Phi, st));
@@ -489,10 +490,9 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
                 prof_end(w, prof);
                 in_window++;
                 if (in_window == delay_k || p == ns - 1) {
-                    prof_begin(w, 0, prof);
+                    prof_begin(w, 0, pf);
                     CU(launch_step(s, d, sp, p, -1, log_off, w->step, tau, 1, st));
-                    prof_end(w, prof);
-                    const bool pf = w->prof_stride > 0;
+                    prof_end(w, pf);
                     prof_begin(w, 4, pf);
                     CU(launch_flush(s, d, sp, st));
                     prof_end(w, pf);

@@ -268,7 +268,7 @@ cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStrea
 // a9: local energy E_L = K + V                                                     [north_star item 6]
 // One warp per electron: 4 dots over the row caches, Jastrow gradient/laplacian and Coulomb sums over
 // partners with warp-shuffle reductions; then a fixed-order per-walker reduction.
-__global__ void __launch_bounds__(256) k_eloc_elec(SysDev s, WalkDev wd) {
+__global__ void __launch_bounds__(256, 4) k_eloc_elec(SysDev s, WalkDev wd) {
     const int w = blockIdx.y;
     const int e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
@@ -278,27 +278,48 @@ __global__ void __launch_bounds__(256) k_eloc_elec(SysDev s, WalkDev wd) {
     const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
     const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
     double gx = 0, gy = 0, gz = 0, lp = 0;
-    for (int j = lane; j < nsp; j += 32) {
-        const double a = arow[j];
-        gx += orb[nsp + j] * a;
-        gy += orb[2 * nsp + j] * a;
-        gz += orb[3 * nsp + j] * a;
-        lp += orb[4 * nsp + j] * a;
+    {   // 4 dot products over the row caches: 16-byte loads, 10 in flight per lane
+        const double2* a2 = reinterpret_cast<const double2*>(arow);
+        const double2* o1 = reinterpret_cast<const double2*>(orb + nsp);
+        const double2* o2 = reinterpret_cast<const double2*>(orb + 2 * nsp);
+        const double2* o3 = reinterpret_cast<const double2*>(orb + 3 * nsp);
+        const double2* o4 = reinterpret_cast<const double2*>(orb + 4 * nsp);
+        const int n2 = nsp >> 1;
+        int j = lane;
+        for (; j + 32 < n2; j += 64) {
+            const double2 a = __ldg(a2 + j), b = __ldg(a2 + j + 32);
+            const double2 p1 = __ldg(o1 + j), q1 = __ldg(o1 + j + 32), p2 = __ldg(o2 + j), q2 = __ldg(o2 + j + 32);
+            const double2 p3 = __ldg(o3 + j), q3 = __ldg(o3 + j + 32), p4 = __ldg(o4 + j), q4 = __ldg(o4 + j + 32);
+            gx += p1.x * a.x + p1.y * a.y + q1.x * b.x + q1.y * b.y;
+            gy += p2.x * a.x + p2.y * a.y + q2.x * b.x + q2.y * b.y;
+            gz += p3.x * a.x + p3.y * a.y + q3.x * b.x + q3.y * b.y;
+            lp += p4.x * a.x + p4.y * a.y + q4.x * b.x + q4.y * b.y;
+        }
+        for (; j < n2; j += 32) {
+            const double2 a = __ldg(a2 + j), p1 = __ldg(o1 + j), p2 = __ldg(o2 + j), p3 = __ldg(o3 + j), p4 = __ldg(o4 + j);
+            gx += p1.x * a.x + p1.y * a.y;
+            gy += p2.x * a.x + p2.y * a.y;
+            gz += p3.x * a.x + p3.y * a.y;
+            lp += p4.x * a.x + p4.y * a.y;
+        }
     }
     const double* Rw = wd.R + (long)w * 3 * nep;
     const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
     double jx = 0, jy = 0, jz = 0, jl = 0, pot = 0;
     const int npart = s.ne + s.n_atoms;
+    // u' = a / q^2, u'' = -2ab / q^3 with q = 1 + b r: one sqrt and two divisions (1/r, 1/q) per pair
     for (int k = lane; k < npart; k += 32) {
         Partner P = partner(s, Rw, nep, e, k);
         if (P.ok) {
             const double dx = rx - P.x, dy = ry - P.y, dz = rz - P.z;
             const double r = sqrt(dx * dx + dy * dy + dz * dz);
-            const double du = pade_du(P.a, P.b, r);
-            jx += du * dx / r; jy += du * dy / r; jz += du * dz / r;
-            jl += pade_d2u(P.a, P.b, r) + 2.0 * du / r;
-            if (k >= s.ne) pot += P.a / r;          // P.a = -Z_I
-            else if (k > e) pot += 1.0 / r;         // each pair once
+            const double ir = 1.0 / r, iq = 1.0 / (1.0 + P.b * r);
+            const double du = P.a * iq * iq;
+            const double wgt = du * ir;
+            jx += wgt * dx; jy += wgt * dy; jz += wgt * dz;
+            jl += 2.0 * wgt - 2.0 * P.b * du * iq;
+            if (k >= s.ne) pot += P.a * ir;         // P.a = -Z_I
+            else if (k > e) pot += ir;              // each pair once
         }
     }
     gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz); lp = warp_sum(lp);
