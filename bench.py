@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--walkers", type=int, default=None, help="walkers per GPU (default: the config's)")
     ap.add_argument("--delay-k", type=int, default=None)
     ap.add_argument("--prof-stride", type=int, default=16, help="time the per-electron stages of every n-th electron")
+    ap.add_argument("--config4-sweep", action="store_true",
+                    help="BASELINE.json configs[4]: delay_k x crowd-size sweep on the 256-water system, 5 sweeps per point; "
+                         "prints one JSON line per point and checks the accept bits against the config-2 trajectory")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-moves", type=int, default=96, help="electron moves per walker in the CPU-baseline sample")
@@ -337,9 +340,70 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_config4(args):
+    """configs[4]: W in {32,128,256,512} x delay_k in {1,4,16,64,128} on the config-2 system, 5 sweeps each from the
+    initial state.  Walkers w < 256 must reproduce the first 5 sweeps of the config-2 run (W = 256, k = 64) decision by
+    decision (delay invariance + walker-prefix invariance, readings A13/A20); the config-2 run itself is compared with
+    the oracle in tests/test_gpu_parity.py."""
+    import torch
+    from paper_2504_07948_b200 import build as qbuild
+    torch.cuda.set_device(0)
+    qbuild.build()
+    import paper_2504_07948_b200 as qb
+    qb.load_library()
+    wl = qi.make_workload(2)
+    sysm = wl.system
+    T = 5
+    gsys = qb.qmc_init_from(sysm)
+    peak = qb.qmc_measure_fp64_peak(300.0)
+    warm = qb.qmc_walkers_create(gsys, torch.from_numpy(qi.initial_positions(sysm, wl.config, range(8), wl.seed)).cuda(), wl.seed)
+    for k in (1, 4, 16, 64, 128):
+        qb.qmc_sweep(warm, 1, wl.tau, k)     # loads every kernel variant once
+    qb.qmc_synchronize(warm)
+    qb.qmc_walkers_destroy(warm)
+
+    def run(W, k):
+        pos = torch.from_numpy(qi.initial_positions(sysm, wl.config, range(W), wl.seed)).cuda()
+        gw = qb.qmc_walkers_create(gsys, pos, wl.seed)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record()
+        qb.qmc_sweep(gw, T, wl.tau, k)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1)
+        bits = qb.qmc_get_accept_log(gw).cpu().numpy()
+        st = qb.qmc_get_stats(gw)
+        eloc = qb.qmc_get_eloc(gw)[0].cpu().numpy()
+        qb.qmc_walkers_destroy(gw)
+        return ms, bits, st, eloc
+
+    _, ref_bits, _, ref_eloc = run(256, 64)
+    for W in (32, 128, 256, 512):
+        for k in (1, 4, 16, 64, 128):
+            ms, bits, st, eloc = run(W, k)
+            n = min(W, 256)
+            a, b = bits[:, :, :n], ref_bits[:, :, :n]
+            differ = (a & 1) != (b & 1)
+            flagged = ((a | b) & 2) != 0
+            walkers_off = int(np.any(differ, axis=(0, 1)).sum())
+            moves = W * sysm.n_elec * T
+            line = dict(metric=METRIC, value=moves / (ms * 1e-3), unit=UNIT, n_gpus=1, steps=T, warmup=0, ms_per_step=ms / T,
+                        dtype="f64", data="synthetic",
+                        config=dict(workload=f"configs[4] water256: {W} walkers, delay_k {k}, tau {wl.tau}, 5 sweeps from the initial state"),
+                        fp64_tflops_model=flop_model(sysm, moves, st["accepted"]) / (ms * 1e-3) * 1e-12, fp64_peak_tflops=peak,
+                        accept_frac=st["accepted"] / moves, ties=st["ties"], nonfinite=st["nonfinite"],
+                        vs_config2=dict(walkers_compared=n, decisions_compared=int(a.size), decisions_differing=int(differ.sum()),
+                                        first_differences_flagged_as_ties=int((differ & flagged).sum()), walkers_diverged=walkers_off,
+                                        max_abs_eloc_diff=float(np.abs(eloc[:n] - ref_eloc[:n]).max())))
+            print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
-    if args.impl == "reference":
+    if args.config4_sweep:
+        run_config4(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -10,9 +10,15 @@
 #include "step_kernel.cuh"
 
 #ifndef QMC_UPD_BM
-#define QMC_UPD_BM 128
+// flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
+// flush against 2.87 ms for 128x64 / 64x32 / 2 and 3.31 ms for 128x128 / 32x64 / 2 (small tiles, several CTAs per SM)
+#define QMC_UPD_BM 64
 #define QMC_UPD_BN 64
-#define QMC_UPD_STAGES 2
+#define QMC_UPD_STAGES 3
+#endif
+#ifndef QMC_UPD_WM
+#define QMC_UPD_WM 16
+#define QMC_UPD_WN 32
 #endif
 #ifndef QMC_Y_STAGES
 #define QMC_Y_STAGES 3
@@ -214,7 +220,7 @@ using CfgY64 = GemmCfg<128, 64, 32, 32, true, QMC_Y_STAGES>;
 using CfgY128 = GemmCfg<128, 128, 64, 32, true, 4>;
 using CfgW2 = GemmCfg<64, 128, 32, 32, false, 3>;
 using CfgUpd = GemmCfg<128, 128, 64, 32, false, 3>;   // Newton-Schulz at creation
-using CfgAcc = GemmCfg<QMC_UPD_BM, QMC_UPD_BN, 64, 32, false, QMC_UPD_STAGES>;  // flush update: several CTAs per SM
+using CfgAcc = GemmCfg<QMC_UPD_BM, QMC_UPD_BN, QMC_UPD_WM, QMC_UPD_WN, false, QMC_UPD_STAGES>;  // flush update: several CTAs per SM
 
 __global__ void k_window_reset(WalkDev wd) {
     const int w = blockIdx.x;
