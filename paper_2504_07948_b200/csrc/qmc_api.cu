@@ -351,35 +351,44 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         CUW(e);
     }
     CUW(launch_fill_int(d.sign, n_walkers, 1, st));
+    // scratch for the blocked inversion and the Newton-Schulz step (freed before returning)
+    const size_t mat_max = (size_t)d.ldv * d.ldv * 8;
+    double *E = nullptr, *Z = nullptr;
+    CUW(cudaMalloc((void**)&E, W * mat_max + 16));
+    {
+        cudaError_t ez = cudaMalloc((void**)&Z, W * mat_max + 16);
+        if (ez != cudaSuccess) { cudaFree(E); CUW(ez); }
+    }
+#define CUF(call)                                                                                      \
+    do {                                                                                               \
+        cudaError_t _e = (call);                                                                       \
+        if (_e != cudaSuccess) { cudaStreamSynchronize(st); cudaFree(E); cudaFree(Z); CUW(_e); }       \
+    } while (0)
     // orbital rows of every electron: basis kernel + FP64 contraction, one electron index at a time
     for (int sp = 0; sp < 2; sp++) {
         const int e0 = sp == 0 ? 0 : s.ns[0];
         for (int p = 0; p < s.ns[sp]; p++) {
-            CUW(launch_gather_rp(d, e0 + p, st));
-            CUW(launch_basis(s, d.rp, n_walkers, d.Phi, st));
-            CUW(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * n_walkers, d.mo_grid), ++w->mo_epoch, st));
-            CUW(launch_store_init_rows(s, d, sp, p, st));
+            CUF(launch_gather_rp(d, e0 + p, st));
+            CUF(launch_basis(s, d.rp, n_walkers, d.Phi, st));
+            CUF(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * n_walkers, d.mo_grid), ++w->mo_epoch, st));
+            CUF(launch_store_init_rows(s, d, sp, p, st));
         }
-        CUW(launch_gj_inverse(d.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp], s.ns[sp], s.nsp[sp], n_walkers, d.logpsi, d.sign, w->d_status, st));
+        CUF(launch_gj_inverse(d.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp], s.ns[sp], s.nsp[sp], n_walkers, d.logpsi, d.sign, w->d_status, E, st));
     }
     int status = 0;
-    CUW(cudaMemcpyAsync(&status, w->d_status, 4, cudaMemcpyDeviceToHost, st));
-    CUW(cudaStreamSynchronize(st));
+    CUF(cudaMemcpyAsync(&status, w->d_status, 4, cudaMemcpyDeviceToHost, st));
+    CUF(cudaStreamSynchronize(st));
     if (status != 0) {
+        cudaFree(E);
+        cudaFree(Z);
         destroy_walkers(w);
         return fail(QMC_ERR_SINGULAR, "qmc_walkers_create: singular Slater matrix (zero pivot)");
     }
-    {   // one Newton-Schulz refinement step of every inverse (temporary buffers, freed right after)
-        const size_t mat_max = (size_t)d.ldv * d.ldv * 8;
-        double *E = nullptr, *Z = nullptr;
-        CUW(cudaMalloc((void**)&E, W * mat_max + 16));
-        cudaError_t e = cudaMalloc((void**)&Z, W * mat_max + 16);
-        for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) e = launch_refine_inverse(s, d, sp, E, Z, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        cudaFree(E);
-        cudaFree(Z);
-        CUW(e);
-    }
+    // one Newton-Schulz refinement step of every inverse
+    for (int sp = 0; sp < 2; sp++) CUF(launch_refine_inverse(s, d, sp, E, Z, st));
+    CUF(cudaStreamSynchronize(st));
+    cudaFree(E);
+    cudaFree(Z);
     CUW(launch_jastrow_total(s, d, st));
     CUW(launch_window_reset(d, st));
     CUW(launch_eloc(s, d, st));

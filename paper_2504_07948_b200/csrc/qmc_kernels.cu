@@ -8,6 +8,7 @@
 #include "mo_streamk.cuh"
 #include "device_utils.cuh"
 #include "step_kernel.cuh"
+#include "block_inverse.cuh"
 
 #ifndef QMC_UPD_BM
 // flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
@@ -494,8 +495,52 @@ __global__ void __launch_bounds__(NT) k_gj_inverse(double* Mall, long stride, in
     }
 }
 
-cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, cudaStream_t st) {
+using CfgGjb = GemmCfg<64, 64, 16, 32, false, 2>;
+
+// Blocked inversion (block_inverse.cuh) for n >= 256 when a panel fits in shared memory; tmp: scratch of batch * stride doubles.
+static cudaError_t launch_block_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status,
+                                        double* tmp, cudaStream_t st) {
+    const int nb = gjb_panel_width(n);
+    GjbArgs g;
+    g.M = Mall; g.stride = stride; g.n = n; g.ld = ld; g.logdet = logdet; g.sign = sign; g.status = status;
+    char* buf = nullptr;
+    const size_t bFn = (size_t)batch * ld * GJB_NB * 8, bT = bFn, bP = (size_t)batch * GJB_NB * GJB_NB * 8, bR = (size_t)batch * ld * 4,
+                 bU = (size_t)batch * ld;
+    cudaError_t e = cudaMalloc((void**)&buf, bFn + bT + bP + bR + bU + 256);
+    if (e != cudaSuccess) return e;
+    g.Fn = (double*)buf; g.T = (double*)(buf + bFn); g.Pinv = (double*)(buf + bFn + bT);
+    g.rowof = (int*)(buf + bFn + bT + bP); g.used = (unsigned char*)(buf + bFn + bT + bP + bR);
+    e = cudaMemsetAsync(buf, 0, bFn + bT + bP + bR + bU, st);
+    const size_t smem = gjb_panel_smem(n, nb);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gjb_panel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    GemmArgs ga;
+    ga.A = g.Fn; ga.lda = GJB_NB; ga.strideA = (long)ld * GJB_NB;
+    ga.B = g.T; ga.ldb = ld; ga.strideB = (long)GJB_NB * ld;
+    ga.C = Mall; ga.ldc = ld; ga.strideC = stride;
+    ga.M = ld; ga.N = ld; ga.K = GJB_NB;
+    for (int k0 = 0; k0 < n && e == cudaSuccess; k0 += nb) {
+        const int nbk = n - k0 < nb ? n - k0 : nb;
+        k_gjb_panel<<<batch, GJB_THREADS, smem, st>>>(g, k0, nbk, nb);
+        k_gjb_rows<<<dim3((ld + 255) / 256, batch), 256, 0, st>>>(g, k0, nbk);
+        e = gemm_f64_launch<CfgGjb>(ga, batch, EpiAccum{}, st);
+        g_launches += 3;
+    }
+    if (e == cudaSuccess) {
+        k_gjb_permute<<<dim3((n + 255) / 256, n, batch), 256, 0, st>>>(g, tmp);
+        k_gjb_copy_back<<<dim3((n + 255) / 256, n, batch), 256, 0, st>>>(g, tmp);
+        k_gjb_perm_sign<<<(batch + 63) / 64, 64, 0, st>>>(g, batch);
+        g_launches += 3;
+        e = cudaGetLastError();
+    }
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(buf);
+    return e != cudaSuccess ? e : e2;
+}
+
+cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, double* tmp,
+                              cudaStream_t st) {
     if (n == 0 || batch == 0) return cudaSuccess;
+    if (n >= 256 && tmp && gjb_panel_width(n) >= 4) return launch_block_inverse(Mall, stride, n, ld, batch, logdet, sign, status, tmp, st);
     COUNT_LAUNCH();
     if (n >= 512) {
         constexpr int NT = 1024;

@@ -20,7 +20,9 @@ cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_eloc(const SysDev& s, const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_gather_rp(const WalkDev& wd, int e, cudaStream_t st);
 cudaError_t launch_store_init_rows(const SysDev& s, const WalkDev& wd, int spin, int p, cudaStream_t st);
-cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, cudaStream_t st);
+// in-place inverse of the leading n x n blocks; tmp (batch * stride doubles, may be NULL) enables the blocked DMMA path
+cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batch, double* logdet, int* sign, int* status, double* tmp,
+                              cudaStream_t st);
 cudaError_t launch_refine_inverse(const SysDev& s, const WalkDev& wd, int spin, double* E, double* Z, cudaStream_t st);
 cudaError_t launch_jastrow_total(const SysDev& s, const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_import_positions(const WalkDev& wd, const double* in, cudaStream_t st);
