@@ -312,11 +312,9 @@ def test_config2_full_crowd_sampled_walkers():
     assert worst["eloc"] < 1e-6, worst
 
 
-@pytest.mark.slow
 def test_config3_full_crowd_first_electrons():
-    import os
-    if not os.environ.get("QMC_SLOW"):
-        pytest.skip("set QMC_SLOW=1 (oracle walker creation at 4096 electrons takes minutes per walker)")
+    # fragment config exactly as configs[3] states it (64 walkers, 4096 electrons, delay_k 128); three sampled walkers,
+    # first 192 electrons of sweep 0 against the oracle (about two minutes of oracle time on the GPU box's host cores)
     worst = _full_size_sampled(3, [0, 31, 63], 1, n_elec_checked=192)
     assert worst["ratio"] < 10 * TOL_RATIO, worst
 
