@@ -89,6 +89,12 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_sweep_range.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                               C.c_int, C.c_int, _u8p, _dp, _dp]
     lib.oracle_walker_eloc.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
+    lib.oracle_walker_dmc_generation.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
+                                                 C.c_double, C.c_double, _dp, _dp, _dp, _u8p]
+    lib.oracle_walker_sweep_limited.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
+                                                C.c_double, _u8p, _dp, _dp, _dp]
+    lib.oracle_drift_limiter_scale.restype = C.c_double
+    lib.oracle_drift_limiter_scale.argtypes = [C.c_double, C.c_double, C.c_double]
     lib.oracle_delayed_update.restype = C.c_int
     lib.oracle_delayed_update.argtypes = [C.c_int, _dp, C.c_int, _ip, _dp, _dp, _dp]
     lib.oracle_sherman_morrison.restype = C.c_double
@@ -249,6 +255,28 @@ class OracleWalker:
                                            bits.ctypes.data_as(_u8p), _d(ratio), _d(pacc))
         return bits, ratio, pacc
 
+    def sweep_limited(self, seed, walker_id, step, tau, lim_a):
+        """A sweep with the drift limiter of row f1; returns (bits, ratio, pacc, dr2[accepted, proposed])."""
+        ne = self.sys.n_elec
+        bits = np.zeros(ne, np.uint8)
+        ratio = np.zeros(ne)
+        pacc = np.zeros(ne)
+        dr2 = np.zeros(2)
+        self.lib.oracle_walker_sweep_limited(self.sys.h, self.h, seed, walker_id, step, tau, lim_a,
+                                             bits.ctypes.data_as(_u8p), _d(ratio), _d(pacc), _d(dr2))
+        return bits, ratio, pacc, dr2
+
+    def dmc_generation(self, seed, walker_id, step, tau, lim_a, e_trial, e_old, weight):
+        """One DMC generation (row f1): limited-drift sweep, E_L, tau_eff, weight update.
+        Returns (bits, e_new, weight_new, tau_eff)."""
+        bits = np.zeros(self.sys.n_elec, np.uint8)
+        e = C.c_double(e_old)
+        w = C.c_double(weight)
+        te = C.c_double()
+        self.lib.oracle_walker_dmc_generation(self.sys.h, self.h, seed, walker_id, step, tau, lim_a, e_trial,
+                                              C.byref(e), C.byref(w), C.byref(te), bits.ctypes.data_as(_u8p))
+        return bits, e.value, w.value, te.value
+
     def eloc(self):
         e = C.c_double()
         k = C.c_double()
@@ -285,6 +313,54 @@ class OracleWalker:
         if rc:
             raise ArithmeticError("oracle: singular Slater matrix")
         return la.value, sg.value
+
+
+# ------------------------------------------------------------------ DMC reconfiguration (row f1, reading A30)
+
+def drift_limiter_scale(v2, lim_a, tau, long_double=False):
+    return _lib(long_double).oracle_drift_limiter_scale(float(v2), float(lim_a), float(tau))
+
+
+def comb_uniform(seed, step):
+    """The one uniform of a reconfiguration: Philox block 3 of counter (0xFFFFFFFF, step, 0xFFFFFFFF, 3), first word
+    pair, mapped like every other uniform (A11)."""
+    out = philox4x32_10([0xFFFFFFFF, step & 0xFFFFFFFF, 0xFFFFFFFF, 3], [seed & 0xFFFFFFFF, seed >> 32])
+    x = (int(out[0]) << 32) | int(out[1])
+    return (2 * (x >> 12) + 1) * 2.0 ** -53
+
+
+def comb_reconfigure(weights, xi):
+    """Fixed-population "comb" reconfiguration, written out as its definition.
+
+    W teeth at t_j = (j + xi) * (W_tot / W), j = 0..W-1, are laid over the cumulative weights c_i = w_0 + ... + w_i
+    (summed in index order); walker i gets as many copies m_i as teeth fall in [c_{i-1}, c_i) (the last walker takes any
+    tooth at or beyond c_{W-1}, which rounding can produce).  Walkers with m_i >= 1 stay in their slot; the k-th slot
+    with m_i = 0 (ascending) receives the k-th extra copy, donors taken in ascending order, each m_i - 1 times.
+    Returns (source, multiplicity, new_weight): slot j now holds a copy of old walker source[j]; every weight becomes
+    W_tot / W."""
+    w = np.asarray(weights, dtype=np.float64)
+    W = len(w)
+    tot = 0.0
+    cum = np.zeros(W)
+    for i in range(W):
+        tot = tot + w[i]
+        cum[i] = tot
+    mult = np.zeros(W, dtype=np.int64)
+    i = 0
+    for j in range(W):
+        t = (j + xi) * (tot / W)
+        while i < W - 1 and not (t < cum[i]):
+            i += 1
+        mult[i] += 1
+    source = np.arange(W, dtype=np.int64)
+    dead = [k for k in range(W) if mult[k] == 0]
+    extra = []
+    for k in range(W):
+        extra += [k] * max(0, int(mult[k]) - 1)
+    assert len(dead) == len(extra)
+    for d, e in zip(dead, extra):
+        source[d] = e
+    return source, mult, tot / W
 
 
 # ------------------------------------------------------------------ crowd driver (threads over walkers)

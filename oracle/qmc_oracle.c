@@ -521,9 +521,27 @@ void oracle_walker_get_logpsi(const oracle_walker *w, double *logabs, int *sign)
  * The _range form runs electrons e_begin..e_end-1 only (a full sweep is 0..n_e); it exists so that a
  * bounded sample of a sweep can be timed. */
 
-void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
-                               uint32_t step, double tau_d, int e_begin, int e_end, uint8_t *bits, double *ratio,
-                               double *pacc) {
+/* Drift limiter of the DMC generation (row f1, reading A28; Umrigar, Nightingale, Runge 1993, eq. 35 with one
+ * constant a): vbar = v * (-1 + sqrt(1 + 2 a v^2 tau)) / (a v^2 tau).  Written as 2 / (1 + sqrt(1 + 2x)), x = a v^2 tau,
+ * which is the same number without the cancellation at small x ((sqrt(1+2x) - 1)(sqrt(1+2x) + 1) = 2x); a test pins it
+ * to the literal form.  lim_a <= 0: no limiter (A6), the drift is used as it is. */
+static void limit_drift(real G[3], real lim_a, real tau) {
+    if (!(lim_a > 0)) return;
+    real v2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+    real x = lim_a * v2 * tau;
+    real sc = 2 / (1 + R_SQRT(1 + 2 * x));
+    G[0] *= sc; G[1] *= sc; G[2] *= sc;
+}
+double oracle_drift_limiter_scale(double v2, double lim_a, double tau) {
+    real G[3] = {R_SQRT((real)v2), 0, 0};
+    limit_drift(G, (real)lim_a, (real)tau);
+    return v2 > 0 ? (double)(G[0] / R_SQRT((real)v2)) : 1.0;
+}
+
+/* lim_a, dr2: see oracle_walker_dmc_generation; the plain sweep passes lim_a = 0 and dr2 = NULL. */
+static void sweep_core(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                       uint32_t step, double tau_d, int e_begin, int e_end, uint8_t *bits, double *ratio,
+                       double *pacc, real lim_a, real *dr2 /* [2]: accepted, proposed */) {
     real tau = (real)tau_d, sqrt_tau = R_SQRT(tau);
     for (int i = e_begin; i < e_end; i++) {
         int sp = spin_of(s, i), ns = sp == 0 ? s->n_up : s->n_dn, p = sp == 0 ? i : i - s->n_up;
@@ -538,8 +556,11 @@ void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_
             for (int j = 0; j < ns; j++) acc += orbp[(1 + d) * ns + j] * Ainv[(size_t)j * ns + p];
             G[d] = acc + gJ[d];
         }
+        limit_drift(G, lim_a, tau);
         real chi[3], u;
         move_variates(seed, walker_id, step, (uint32_t)i, chi, &u);
+        real rr = tau * (chi[0] * chi[0] + chi[1] * chi[1] + chi[2] * chi[2]); /* |diffusive displacement|^2 */
+        if (dr2) dr2[1] += rr;
         real rp[3];
         for (int d = 0; d < 3; d++) rp[d] = r[d] + tau * G[d] + sqrt_tau * chi[d];
         /* orbital rows at r' */
@@ -562,6 +583,7 @@ void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_
                 for (int j = 0; j < ns; j++) acc += v[(1 + d) * ns + j] * Ainv[(size_t)j * ns + p];
                 Gp[d] = acc / rho + gJn[d];
             }
+            limit_drift(Gp, lim_a, tau);
             real fwd = 0, rev = 0;
             for (int d = 0; d < 3; d++) {
                 real a = rp[d] - r[d] - tau * G[d];
@@ -576,6 +598,7 @@ void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_
         }
         if (accept) {
             b |= 1;
+            if (dr2) dr2[0] += rr;
             r[0] = rp[0]; r[1] = rp[1]; r[2] = rp[2];
             /* Sherman-Morrison: Ainv[:,q] -= Ainv[:,p] (v.Ainv[:,q]) / rho (q != p); Ainv[:,p] /= rho */
             real *sq = w->tmp;
@@ -599,6 +622,12 @@ void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_
         if (ratio) ratio[i] = (double)jr;
         if (pacc) pacc[i] = (double)pa;
     }
+}
+
+void oracle_walker_sweep_range(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                               uint32_t step, double tau_d, int e_begin, int e_end, uint8_t *bits, double *ratio,
+                               double *pacc) {
+    sweep_core(s, w, seed, walker_id, step, tau_d, e_begin, e_end, bits, ratio, pacc, 0, NULL);
 }
 
 void oracle_walker_sweep(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
@@ -648,6 +677,39 @@ void oracle_walker_eloc(const oracle_system *s, const oracle_walker *w, double *
         }
     *eloc = (double)(K + V);
     if (ekin) *ekin = (double)K;
+}
+
+/* ------------------------------------------------------------------ one DMC generation (row f1 of SURVEY 8(f))
+ * The paper runs fixed-node DMC (eq. 1; tau = 0.01, 4096 walkers, L131) and says nothing about the
+ * weights, so this follows the textbook algorithm (Umrigar, Nightingale, Runge, J. Chem. Phys. 99, 2865 (1993)),
+ * readings A28-A30 of DESIGN.md:
+ *   1. the sweep above with the drift of every proposal (forward and reverse) limited by limit_drift;
+ *   2. tau_eff = tau * (sum over ACCEPTED moves of |sqrt(tau) chi|^2) / (sum over ALL proposed moves of it);
+ *      tau if nothing was proposed;
+ *   3. weight *= exp(-tau_eff * ((E_old + E_new) / 2 - E_T)),  E_old / E_new = E_L before / after the sweep.
+ * e_io: in E_old, out E_new.  weight_io: in/out.  bits: accept log of the sweep, may be NULL. */
+/* The sweep with the limited drift alone (no E_L, no weight), with its logs: lets a test recompute every p_acc of a
+ * limited-drift sweep from first principles.  dr2: [accepted, proposed] sums of |sqrt(tau) chi|^2, may be NULL. */
+void oracle_walker_sweep_limited(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                                 uint32_t step, double tau_d, double lim_a, uint8_t *bits, double *ratio, double *pacc,
+                                 double *dr2_out) {
+    real dr2[2] = {0, 0};
+    sweep_core(s, w, seed, walker_id, step, tau_d, 0, w->ne, bits, ratio, pacc, (real)lim_a, dr2);
+    if (dr2_out) { dr2_out[0] = (double)dr2[0]; dr2_out[1] = (double)dr2[1]; }
+}
+
+void oracle_walker_dmc_generation(const oracle_system *s, oracle_walker *w, uint64_t seed, uint32_t walker_id,
+                                  uint32_t step, double tau_d, double lim_a, double E_T, double *e_io,
+                                  double *weight_io, double *tau_eff_out, uint8_t *bits) {
+    real dr2[2] = {0, 0};
+    sweep_core(s, w, seed, walker_id, step, tau_d, 0, w->ne, bits, NULL, NULL, (real)lim_a, dr2);
+    double e_new, e_kin;
+    oracle_walker_eloc(s, w, &e_new, &e_kin);
+    real tau_eff = dr2[1] > 0 ? (real)tau_d * dr2[0] / dr2[1] : (real)tau_d;
+    real arg = -tau_eff * (((real)*e_io + (real)e_new) / 2 - (real)E_T);
+    *weight_io = (double)((real)*weight_io * R_EXP(arg));
+    *e_io = e_new;
+    if (tau_eff_out) *tau_eff_out = (double)tau_eff;
 }
 
 /* ------------------------------------------------------------------ delayed rank-k update
