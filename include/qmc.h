@@ -128,6 +128,27 @@ int qmc_get_stats(const qmc_walkers* w, uint64_t* n_proposed, uint64_t* n_accept
                   uint64_t* n_nonfinite);
 int qmc_synchronize(const qmc_walkers* w);
 
+/* ---- Row f1 of the scope table: the DMC generation (fixed-node DMC, eq. 1; the paper prints no
+ * weight or branching rule, so these follow Umrigar-Nightingale-Runge 1993 -- readings A28-A30 of DESIGN.md).
+ *
+ * qmc_dmc_step: n_generations times { one sweep exactly as qmc_sweep, except that the drift of every proposal (forward
+ * and reverse) is limited, vbar = v (-1 + sqrt(1 + 2 a v^2 tau)) / (a v^2 tau) with a = limiter_a (0: no limiter);
+ * E_L; tau_eff = tau * (sum over accepted moves of |sqrt(tau) chi|^2) / (sum over all proposals of it);
+ * weight *= exp(-tau_eff ((E_old + E_new) / 2 - e_trial)) }.  Weights start at 1 at creation and persist across calls;
+ * E_old of the first generation of a call is the current E_L.  Asynchronous on the stream; the accept log covers the
+ * call like qmc_sweep's.  Errors: QMC_ERR_ARG as qmc_sweep, or limiter_a < 0 / non-finite e_trial. */
+int qmc_dmc_step(qmc_walkers* w, int n_generations, double tau, int delay_k, double e_trial, double limiter_a);
+/* weights[W] (and tau_eff[W] of the last generation; may be NULL); host or device buffers. */
+int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff);
+/* Fixed-population "comb" reconfiguration: with c_i the cumulative weights (summed in index order) and one uniform xi
+ * (Philox counter (0xFFFFFFFF, step, 0xFFFFFFFF, 3), first word pair), walker i gets as many copies as teeth
+ * (j + xi) W_tot / W, j = 0..W-1, fall in [c_{i-1}, c_i).  Walkers with >= 1 copy keep their slot; the k-th slot with
+ * none (ascending) receives the k-th extra copy, donors in ascending order; every weight becomes W_tot / W.
+ * source[W] (int32, host or device, may be NULL): slot j now holds a copy of old walker source[j].  e_mixed (may be
+ * NULL): sum w E_L / sum w before the reconfiguration.  Must be called between sweeps (the delay window is empty then);
+ * synchronises the stream. */
+int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed);
+
 /* Stage-level entry points (used by the per-stage parity tests and the per-stage roofline bench).
  * Basis functions at n_points positions: out[n][5][n_basis] = value, d/dx, d/dy, d/dz, laplacian. */
 int qmc_eval_basis(const qmc_system* sys, int n_points, const double* xyz /* [n][3] */, double* out, void* cuda_stream);

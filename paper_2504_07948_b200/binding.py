@@ -23,6 +23,7 @@ EXPORTED = [
     "qmc_get_Ainv", "qmc_get_logpsi", "qmc_get_eloc", "qmc_get_accept_log", "qmc_get_ratio_log", "qmc_get_stats",
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
+    "qmc_dmc_step", "qmc_get_weights", "qmc_branch",
 ]
 
 
@@ -84,6 +85,9 @@ def load_library(path: str | None = None):
     lib.qmc_set_profiling.argtypes = [vp, i]
     lib.qmc_get_stage_times.argtypes = [vp, C.POINTER(d), C.POINTER(u64)]
     lib.qmc_measure_fp64_peak.argtypes = [d, C.POINTER(d), vp]
+    lib.qmc_dmc_step.argtypes = [vp, i, d, i, d, d]
+    lib.qmc_get_weights.argtypes = [vp, vp, vp]
+    lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
     lib.qmc_version.restype = C.c_char_p
@@ -214,6 +218,28 @@ def qmc_walkers_destroy(walkers: Walkers):
 def qmc_sweep(walkers: Walkers, nsteps, tau, delay_k):
     _check(load_library().qmc_sweep(walkers.handle, int(nsteps), float(tau), int(delay_k)))
     walkers.last_nsteps = int(nsteps)
+
+
+def qmc_dmc_step(walkers: Walkers, n_generations, tau, delay_k, e_trial, limiter_a=1.0):
+    _check(load_library().qmc_dmc_step(walkers.handle, int(n_generations), float(tau), int(delay_k), float(e_trial), float(limiter_a)))
+    walkers.last_nsteps = int(n_generations)
+
+
+def qmc_get_weights(walkers: Walkers, out=None, out_tau_eff=None):
+    import torch
+    out = _out((walkers.n_walkers,), torch.float64, out)
+    out_tau_eff = _out((walkers.n_walkers,), torch.float64, out_tau_eff)
+    _check(load_library().qmc_get_weights(walkers.handle, _ptr(out), _ptr(out_tau_eff)))
+    return out, out_tau_eff
+
+
+def qmc_branch(walkers: Walkers, out_source=None):
+    """Comb reconfiguration; returns (source [W] int32 tensor, e_mixed float)."""
+    import torch
+    out_source = _out((walkers.n_walkers,), torch.int32, out_source)
+    e = C.c_double()
+    _check(load_library().qmc_branch(walkers.handle, _ptr(out_source), C.byref(e)))
+    return out_source, e.value
 
 
 def _out(shape, dtype, out, device="cuda"):

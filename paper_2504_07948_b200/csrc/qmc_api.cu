@@ -30,6 +30,7 @@ static int fail(int code, const std::string& msg) {
     } while (0)
 
 static inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+static bool is_device_ptr(const void* p);
 
 struct DevPool {  // owns cudaMalloc'ed blocks
     std::vector<void*> blocks;
@@ -78,6 +79,8 @@ struct qmc_walkers {
     uint32_t flags;
     int T_last;          // sweeps in the most recent qmc_sweep call
     int* d_status;
+    int* d_comb;        // [4 W + 1] reconfiguration scratch: source, pair_dst, pair_src, mult, n_pairs
+    double* d_emixed;   // [1]
     unsigned mo_epoch;   // stream-K launch counter (flag stamps)
     int prof_stride;     // 0 = off
     StageTimer timer;
@@ -335,6 +338,14 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     CUW(w->pool.alloc((void**)&d.ekin, W * 8, st));
     CUW(w->pool.alloc((void**)&d.ebuf, W * s.ne * 2 * 8, st));
     CUW(w->pool.alloc((void**)&d.stats, 4 * 8, st));
+    CUW(w->pool.alloc((void**)&d.weight, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.eold, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.dr2, W * 2 * 8, st));
+    CUW(w->pool.alloc((void**)&d.dr2p, W * 8, st));
+    CUW(w->pool.alloc((void**)&d.tau_eff, W * 8, st));
+    CUW(w->pool.alloc((void**)&w->d_comb, (4 * W + 1) * 4, st));
+    CUW(w->pool.alloc((void**)&w->d_emixed, 8, st));
+    CUW(launch_fill_double(d.weight, n_walkers, 1.0, st));
     CUW(w->pool.alloc((void**)&w->d_status, 4, st));
     rc = alloc_window(w, 16);
     if (rc) { std::string m = g_err; destroy_walkers(w); return fail(rc, m); }
@@ -452,14 +463,17 @@ extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t*
 
 // ------------------------------------------------------------------------------------------------ qmc_sweep
 
-extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
+// dmc != 0: every sweep is a DMC generation (row f1): limited drift, then the weight update after E_L
+static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
     if (nsteps < 0) return fail(QMC_ERR_ARG, "qmc_sweep: nsteps < 0");
     if (!(tau > 0.0) || !isfinite(tau)) return fail(QMC_ERR_ARG, "qmc_sweep: tau must be > 0");
     if (delay_k < 1 || delay_k > 128) return fail(QMC_ERR_ARG, "qmc_sweep: delay_k must be in 1..128");
+    if (dmc && (!isfinite(e_trial) || !(lim_a >= 0.0) || !isfinite(lim_a))) return fail(QMC_ERR_ARG, "qmc_dmc_step: e_trial must be finite and limiter_a >= 0");
     const SysDev& s = w->sys->d;
     WalkDev& d = w->d;
     cudaStream_t st = w->stream;
+    d.lim_a = dmc ? lim_a : 0.0;
     const int kp = round_up(delay_k, 16);
     if (kp != d.kp) {
         int rc = alloc_window(w, kp);
@@ -477,6 +491,7 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
         CU(w->logpool.alloc((void**)&d.pacc_log, nlog * 8, st));
     }
     w->T_last = nsteps;
+    if (dmc) CU(launch_dmc_begin(d, st));
     for (int t = 0; t < nsteps; t++) {
         for (int sp = 0; sp < 2; sp++) {
             const int ns = s.ns[sp], e0 = sp == 0 ? 0 : s.ns[0];
@@ -518,9 +533,37 @@ extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) {
         prof_begin(w, 5, pf);
         CU(launch_eloc(s, d, st));
         prof_end(w, pf);
+        if (dmc) CU(launch_dmc_weight(d, tau, e_trial, st));
         w->step++;
         if (w->timer.used > 8192) prof_collect(w);
     }
+    return QMC_OK;
+}
+
+extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) { return sweep_impl(w, nsteps, tau, delay_k, 0, 0.0, 0.0); }
+
+extern "C" int qmc_dmc_step(qmc_walkers* w, int n_generations, double tau, int delay_k, double e_trial, double limiter_a) {
+    return sweep_impl(w, n_generations, tau, delay_k, 1, e_trial, limiter_a);
+}
+
+extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_branch: null walkers");
+    cudaStream_t st = w->stream;
+    CU(launch_branch(w->sys->d, w->d, w->d_comb, w->d_emixed, w->step, st));
+    if (source) {
+        CU(cudaMemcpyAsync(source, w->d_comb, (size_t)w->d.W * 4, cudaMemcpyDefault, st));
+    }
+    if (e_mixed) CU(cudaMemcpyAsync(e_mixed, w->d_emixed, 8, cudaMemcpyDefault, st));
+    CU(cudaStreamSynchronize(st));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff) {
+    if (!w || !weights) return fail(QMC_ERR_ARG, "qmc_get_weights: null argument");
+    const size_t n = (size_t)w->d.W * 8;
+    CU(cudaMemcpyAsync(weights, w->d.weight, n, cudaMemcpyDefault, w->stream));
+    if (tau_eff) CU(cudaMemcpyAsync(tau_eff, w->d.tau_eff, n, cudaMemcpyDefault, w->stream));
+    if (!is_device_ptr(weights) || (tau_eff && !is_device_ptr(tau_eff))) CU(cudaStreamSynchronize(w->stream));
     return QMC_OK;
 }
 

@@ -73,6 +73,10 @@ struct WalkDev {
     unsigned long long* stats;  // proposed, accepted, ties, nonfinite
     uint64_t seed;
     uint32_t first_walker;
+    // DMC generation (row f1): drift-limiter constant (<= 0: off), per-walker weight, E_L at the start of the generation,
+    // sums of |sqrt(tau) chi|^2 over accepted / all proposals [W][2], the pending proposal's value [W], tau_eff [W]
+    double lim_a;
+    double *weight, *eold, *dr2, *dr2p, *tau_eff;
 };
 
 }  // namespace qmc

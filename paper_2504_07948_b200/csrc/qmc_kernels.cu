@@ -9,6 +9,7 @@
 #include "device_utils.cuh"
 #include "step_kernel.cuh"
 #include "block_inverse.cuh"
+#include "dmc_kernels.cuh"
 
 #ifndef QMC_UPD_BM
 // flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
@@ -760,6 +761,51 @@ __global__ void k_dmma_peak(double* out, int iters, double a, double b) {
 }
 cudaError_t launch_dmma_peak(double* out, int grid, int threads, int iters, cudaStream_t st) {
     k_dmma_peak<<<grid, threads, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// row f1: DMC generation bookkeeping and reconfiguration (dmc_kernels.cuh)
+__global__ void k_fill_double(double* p, int n, double v) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+cudaError_t launch_fill_double(double* p, int n, double v, cudaStream_t st) {
+    k_fill_double<<<(n + 255) / 256, 256, 0, st>>>(p, n, v);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_dmc_begin(const WalkDev& wd, cudaStream_t st) {
+    k_dmc_begin<<<(wd.W + 255) / 256, 256, 0, st>>>(wd);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, cudaStream_t st) {
+    k_dmc_weight<<<(wd.W + 255) / 256, 256, 0, st>>>(wd, tau, e_trial);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf /* [4 W + 1] */, double* e_mixed, uint32_t step, cudaStream_t st) {
+    CombOut o;
+    o.source = ibuf; o.pair_dst = ibuf + wd.W; o.pair_src = ibuf + 2 * wd.W; o.mult = ibuf + 3 * wd.W; o.n_pairs = ibuf + 4 * wd.W;
+    o.e_mixed = e_mixed;
+    const size_t smem = (size_t)wd.W * 8 <= 40 * 1024 ? (size_t)wd.W * 8 : 0;
+    k_comb<<<1, 256, smem, st>>>(wd, o, step);
+    COUNT_LAUNCH();
+    CopyArgs a;
+    a.n_seg = 0;
+    a.seg[a.n_seg++] = CopySeg{wd.R, 3L * wd.nep};
+    for (int sp = 0; sp < 2; sp++) {
+        if (s.ns[sp] == 0) continue;
+        a.seg[a.n_seg++] = CopySeg{wd.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp]};
+        a.seg[a.n_seg++] = CopySeg{wd.Orb[sp], 5L * s.nsp[sp] * s.nsp[sp]};
+    }
+    const long biggest = 5L * wd.ldv * wd.ldv / 2;
+    int chunks = (int)((biggest + 256L * 16 - 1) / (256L * 16));
+    if (chunks < 1) chunks = 1;
+    if (chunks > 512) chunks = 512;
+    k_copy_walkers<<<dim3(chunks, wd.W), 256, 0, st>>>(wd, a, o);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

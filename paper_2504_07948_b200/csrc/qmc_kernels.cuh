@@ -33,6 +33,10 @@ cudaError_t launch_sign_to_i8(const int* in, int n, int8_t* out, cudaStream_t st
 cudaError_t launch_fill_int(int* p, int n, int v, cudaStream_t st);
 cudaError_t launch_enn(const SysDev& s, double* out, cudaStream_t st);
 cudaError_t launch_dmma_peak(double* out, int grid, int threads, int iters, cudaStream_t st);
+cudaError_t launch_fill_double(double* p, int n, double v, cudaStream_t st);
+cudaError_t launch_dmc_begin(const WalkDev& wd, cudaStream_t st);
+cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, cudaStream_t st);
+cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double* e_mixed, uint32_t step, cudaStream_t st);
 uint64_t launch_count();
 
 }  // namespace qmc

@@ -80,6 +80,17 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
     accB = warp_sum(sb);
 }
 
+// Drift limiter of the DMC generation (row f1, reading A28; Umrigar-Nightingale-Runge 1993 eq. 35 with one constant a):
+// vbar = v (-1 + sqrt(1 + 2 a v^2 tau)) / (a v^2 tau), evaluated as v * 2 / (1 + sqrt(1 + 2x)), x = a v^2 tau (the same
+// number without the cancellation at small x).  a <= 0: off (reading A6).
+__device__ __forceinline__ void limit_drift(double& gx, double& gy, double& gz, double lim_a, double tau) {
+    if (!(lim_a > 0.0)) return;
+    const double v2 = gx * gx + gy * gy + gz * gz;
+    const double x = lim_a * v2 * tau;
+    const double sc = 2.0 / (1.0 + sqrt(1.0 + 2.0 * x));
+    gx *= sc; gy *= sc; gz *= sc;
+}
+
 // p_acc >= 0: finish the move of electron p_acc of this spin (needs its MO rows in V);  p_prop >= 0: propose the
 // move of electron p_prop.  commit == 0 evaluates the decision but changes no state (stage timing only).
 __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
@@ -145,7 +156,8 @@ __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, 
             bool accept = false;
             if (fabs(rho) < 1e-12) bits |= 2u;
             if (rho > 0.0) {  // fixed node: reject rho_D <= 0 (A7); NaN fails the comparison and rejects
-                const double Hx = a4[1] / rho + wd.gJn[3 * w], Hy = a4[2] / rho + wd.gJn[3 * w + 1], Hz = a4[3] / rho + wd.gJn[3 * w + 2];
+                double Hx = a4[1] / rho + wd.gJn[3 * w], Hy = a4[2] / rho + wd.gJn[3 * w + 1], Hz = a4[3] / rho + wd.gJn[3 * w + 2];
+                limit_drift(Hx, Hy, Hz, wd.lim_a, tau);
                 const double ax = qx - rx - tau * Gx, ay = qy - ry - tau * Gy, az = qz - rz - tau * Gz;
                 const double cx = rx - qx - tau * Hx, cy = ry - qy - tau * Hy, cz = rz - qz - tau * Hz;
                 const double fwd = ax * ax + ay * ay + az * az, rev = cx * cx + cy * cy + cz * cz;
@@ -165,7 +177,10 @@ __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, 
                 if (accept) atomicAdd(&wd.stats[1], 1ull);
                 if (bits & 2u) atomicAdd(&wd.stats[2], 1ull);
                 if (nonfinite) { atomicAdd(&wd.stats[3], 1ull); wd.flags[w] = 1u; }
+                const double rr = wd.dr2p[w];  // |sqrt(tau) chi|^2 of this proposal (for tau_eff, row f1)
+                wd.dr2[2 * w + 1] += rr;
                 if (accept) {
+                    wd.dr2[2 * w] += rr;
                     Rw[e] = qx; Rw[nep + e] = qy; Rw[2 * nep + e] = qz;
                     wd.logpsi[w] += log(rho) + dJ;
                 }
@@ -313,7 +328,8 @@ __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, 
         }
     }
     block_sum<PT, 6>(acc6, red);
-    const double Gx = acc6[0] + acc6[3], Gy = acc6[1] + acc6[4], Gz = acc6[2] + acc6[5];
+    double Gx = acc6[0] + acc6[3], Gy = acc6[1] + acc6[4], Gz = acc6[2] + acc6[5];
+    limit_drift(Gx, Gy, Gz, wd.lim_a, tau);
     const double qx = rx + tau * Gx + sqrt_tau * bc[4];
     const double qy = ry + tau * Gy + sqrt_tau * bc[5];
     const double qz = rz + tau * Gz + sqrt_tau * bc[6];
@@ -321,6 +337,7 @@ __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, 
         wd.rp[3 * w] = qx; wd.rp[3 * w + 1] = qy; wd.rp[3 * w + 2] = qz;
         wd.G[3 * w] = Gx; wd.G[3 * w + 1] = Gy; wd.G[3 * w + 2] = Gz;
         wd.u[w] = bc[7];
+        wd.dr2p[w] = tau * (bc[4] * bc[4] + bc[5] * bc[5] + bc[6] * bc[6]);
     }
     // Jastrow ratio, term by term, and gradient at r'.  With q = 1 + b r:  u(r') - u(r) = a (r' - r) / (q' q)  (the same
     // term, written without the cancellation of two nearly equal quotients) and grad' = a / (q'^2 r') (r' - r_k);
