@@ -46,6 +46,7 @@ def parse():
     ap.add_argument("--config4-sweep", action="store_true",
                     help="BASELINE.json configs[4]: delay_k x crowd-size sweep on the 256-water system, 5 sweeps per point; "
                          "prints one JSON line per point and checks the accept bits against the config-2 trajectory")
+    ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-moves", type=int, default=96, help="electron moves per walker in the CPU-baseline sample")
@@ -253,6 +254,21 @@ def run_ours(args):
     assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
     assert st1["nonfinite"] == 0
     red = reduce_report(ms, n_moves, float(eloc.sum()), float((eloc * eloc).sum()), W, backend_device="cuda")
+    # row f1 (outside the timed region): one DMC generation + one comb reconfiguration on the same crowd
+    f1 = None
+    if not args.no_dmc:
+        e_t = float(eloc.mean())
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        evs[0].record()
+        qb.qmc_dmc_step(gw, 1, wl.tau, k, e_t, 1.0)
+        evs[1].record()
+        src, e_mixed = qb.qmc_branch(gw)
+        evs[2].record()
+        torch.cuda.synchronize()
+        f1 = dict(generation_ms=evs[0].elapsed_time(evs[1]), branch_ms=evs[1].elapsed_time(evs[2]),
+                  walkers_copied=int((src.cpu().numpy() != np.arange(W)).sum()), e_trial=e_t, e_mixed=e_mixed, limiter_a=1.0,
+                  what="qmc_dmc_step(1) = sweep with limited drift + weight update; qmc_branch = comb + copies of A^-1 and row caches")
     qb.qmc_walkers_destroy(gw)
 
     # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps
@@ -332,6 +348,7 @@ def run_ours(args):
         hbm_peak_source="MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "6.65 TB/s of fallback (B200_PROFILING.md)",
         stage_share={s: share[s] / tot_share for s in share},
         eloc_mean=red["e_sum"] / red["n_walkers"],
+        f1_dmc=f1,
     )
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = oracle_sample(wl, 3, 1, args.cpu_moves)[0]
