@@ -46,6 +46,10 @@ extern "C" {
 
 /* flags of qmc_walkers_create */
 #define QMC_LOG_RATIOS 1u /* also record rho_D*exp(dJ) and p_acc of every proposed move */
+#define QMC_LARGE_PATH 2u /* never use the one-launch small-system path (row f4): systems with <= 32 electrons per spin
+                             whose per-walker state fits in shared memory otherwise run a whole qmc_sweep / qmc_dmc_step
+                             call in one kernel, one warp per walker, with rank-1 updates (delay_k then only changes
+                             rounding, reading A13) */
 
 typedef struct qmc_system qmc_system;   /* immutable after qmc_init: atoms, basis, MO coefficients, Jastrow (device) */
 typedef struct qmc_walkers qmc_walkers; /* mutable crowd state */

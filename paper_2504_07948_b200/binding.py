@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libqmc_b200.so")
 
 QMC_OK, QMC_ERR_ARG, QMC_ERR_CUDA, QMC_ERR_SINGULAR, QMC_ERR_NOMEM, QMC_ERR_STATE = 0, -1, -2, -3, -4, -5
 QMC_LOG_RATIOS = 1
+QMC_LARGE_PATH = 2
 STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc")
 
 EXPORTED = [

@@ -491,6 +491,11 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
         CU(w->logpool.alloc((void**)&d.pacc_log, nlog * 8, st));
     }
     w->T_last = nsteps;
+    if (!(w->flags & QMC_LARGE_PATH) && small_path_ok(s, d)) {  // row f4: the whole call in one launch
+        if (nsteps > 0) CU(launch_sweep_small(s, d, nsteps, w->step, tau, dmc, e_trial, st));
+        w->step += (uint32_t)nsteps;
+        return QMC_OK;
+    }
     if (dmc) CU(launch_dmc_begin(d, st));
     for (int t = 0; t < nsteps; t++) {
         for (int sp = 0; sp < 2; sp++) {

@@ -10,6 +10,7 @@
 #include "step_kernel.cuh"
 #include "block_inverse.cuh"
 #include "dmc_kernels.cuh"
+#include "small_sweep.cuh"
 
 #ifndef QMC_UPD_BM
 // flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
@@ -806,6 +807,38 @@ cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf /* [4 W 
     if (chunks < 1) chunks = 1;
     if (chunks > 512) chunks = 512;
     k_copy_walkers<<<dim3(chunks, wd.W), 256, 0, st>>>(wd, a, o);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// row f4: whole call in one launch for small systems (small_sweep.cuh).  Returns false if the system does not qualify.
+bool small_path_ok(const SysDev& s, const WalkDev& wd) {
+    const int nsm = s.ns[0] > s.ns[1] ? s.ns[0] : s.ns[1];
+    if (nsm > 32 || s.n_basis > 512) return false;
+    const size_t per_block = small_block_doubles(s, nsm) * 8, per_walker = small_walker_doubles(s, wd.nep, nsm) * 8;
+    return per_block + per_walker <= 200 * 1024;
+}
+cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
+                               cudaStream_t st) {
+    SmallArgs a;
+    a.nsteps = nsteps; a.step0 = step0; a.tau = tau; a.sqrt_tau = sqrt(tau); a.dmc = dmc; a.e_trial = e_trial;
+    a.nsm = s.ns[0] > s.ns[1] ? s.ns[0] : s.ns[1];
+    const size_t per_block = small_block_doubles(s, a.nsm) * 8, per_walker = small_walker_doubles(s, wd.nep, a.nsm) * 8;
+    // warps per block: as many as fit in ~100 KB (two blocks per SM), at most 8, and no more than needed to give every SM a block
+    int wpb = (int)((100 * 1024 - per_block) / per_walker);
+    if (wpb < 1) wpb = 1;
+    if (wpb > 8) wpb = 8;
+    while (wpb > 1 && (wd.W + wpb - 1) / wpb < 148) wpb--;
+    a.wpb = wpb;
+    const size_t smem = per_block + (size_t)wpb * per_walker;
+    static size_t configured = 48 * 1024;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_sweep_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    k_sweep_small<<<(wd.W + wpb - 1) / wpb, wpb * 32, smem, st>>>(s, wd, a);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

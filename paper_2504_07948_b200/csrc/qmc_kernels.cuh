@@ -37,6 +37,9 @@ cudaError_t launch_fill_double(double* p, int n, double v, cudaStream_t st);
 cudaError_t launch_dmc_begin(const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, cudaStream_t st);
 cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double* e_mixed, uint32_t step, cudaStream_t st);
+bool small_path_ok(const SysDev& s, const WalkDev& wd);
+cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
+                               cudaStream_t st);
 uint64_t launch_count();
 
 }  // namespace qmc

@@ -50,14 +50,16 @@ def _compare(gw, bits_o, e_o, w_o, te_o, eloc_tol=1e-9):
     return ok
 
 
-@pytest.mark.parametrize("cfg,W,k,T,e_t", [(0, 48, 1, 12, -76.0), (0, 48, 4, 12, -76.0), (1, 12, 32, 2, -550.0)])
-def test_dmc_generations_match_oracle(cfg, W, k, T, e_t):
+@pytest.mark.parametrize("cfg,W,k,T,e_t,flags", [(0, 48, 1, 12, -76.0, 0), (0, 48, 1, 12, -76.0, 2), (0, 48, 4, 12, -76.0, 2),
+                                                 (1, 12, 32, 2, -550.0, 0)])
+def test_dmc_generations_match_oracle(cfg, W, k, T, e_t, flags):
+    # flags 0: config 0 takes the one-launch small-system path (row f4); 2 = QMC_LARGE_PATH: the per-electron kernels
     wl = qi.make_workload(cfg)
     sysm = wl.system
     a, tau = 1.0, wl.tau
     pos = wl.positions(0, W)
     g = qb.qmc_init_from(sysm)
-    gw = qb.qmc_walkers_create(g, pos, wl.seed)
+    gw = qb.qmc_walkers_create(g, pos, wl.seed, flags=flags)
     e0 = qb.qmc_get_eloc(gw)[0].cpu().numpy()
     qb.qmc_dmc_step(gw, T, tau, k, e_t, a)
     osys = oracle.OracleSystem(sysm)

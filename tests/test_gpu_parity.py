@@ -121,10 +121,34 @@ def test_config0_full_trajectories():
     assert rep["n_moves"] == wl.n_moves and 0.5 < rep["accept_frac"] < 1.0
 
 
-@pytest.mark.parametrize("k", [4, 5])
-def test_config0_delayed(k):
+@pytest.mark.parametrize("k", [1, 4, 5])
+def test_config0_large_system_path(k):
+    # config 0 qualifies for the one-launch small-system path (row f4), which the test above exercises; here the same
+    # system is forced through the per-electron kernels and the delayed update (QMC_LARGE_PATH)
     wl = qi.make_workload(0)
-    _assert_report(run_and_compare(wl, range(16), 20, k))
+    _assert_report(run_and_compare(wl, range(16), 20, k, flags=qb.QMC_LOG_RATIOS | qb.QMC_LARGE_PATH))
+
+
+def test_small_and_large_paths_agree_and_resume():
+    wl = qi.make_workload(0)
+    g = qb.qmc_init_from(wl.system)
+    out = {}
+    for name, flags, calls in (("small", 0, 1), ("small2", 0, 2), ("large", qb.QMC_LARGE_PATH, 1)):
+        gw = qb.qmc_walkers_create(g, wl.positions(0, 40), wl.seed, flags=flags)
+        bits = []
+        for _ in range(calls):
+            qb.qmc_sweep(gw, 6 // calls, wl.tau, 2)
+            bits.append(qb.qmc_get_accept_log(gw).cpu().numpy())
+        out[name] = (np.concatenate(bits), qb.qmc_get_positions(gw).cpu().numpy(), qb.qmc_get_eloc(gw)[0].cpu().numpy(),
+                     qb.qmc_get_logpsi(gw)[0].cpu().numpy(), qb.qmc_get_Ainv(gw, 1).cpu().numpy(), qb.qmc_get_stats(gw))
+    for x, y in zip(out["small"][:5], out["small2"][:5]):
+        assert np.array_equal(x, y)                      # 3 + 3 sweeps == 6 sweeps, bit for bit (A12)
+    a, b = out["small"], out["large"]
+    assert np.array_equal(a[0] & 1, b[0] & 1)
+    assert np.abs(a[1] - b[1]).max() < TOL_POS and np.abs(a[2] - b[2]).max() < TOL_ELOC
+    assert np.abs(a[3] - b[3]).max() < 1e-10 * np.abs(b[3]).max()
+    assert max(rel_frob(a[4][n], b[4][n]) for n in range(40)) < TOL_AINV
+    assert a[5]["proposed"] == b[5]["proposed"] and a[5]["accepted"] == b[5]["accepted"]
 
 
 def test_config1_trajectories_subset_delay32():
