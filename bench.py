@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--config4-sweep", action="store_true",
                     help="BASELINE.json configs[4]: delay_k x crowd-size sweep on the 256-water system, 5 sweeps per point; "
                          "prints one JSON line per point and checks the accept bits against the config-2 trajectory")
+    ap.add_argument("--paper-regime", action="store_true",
+                    help="row f4: the paper's own regime -- water clusters of 8/16/24/152 valence electrons, 4320 walkers per GPU "
+                         "(PAPER.md L279-302) -- on the one-launch small-system path and on the per-electron path; one JSON line each")
     ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -416,9 +419,61 @@ def run_config4(args):
             print(json.dumps(line), flush=True)
 
 
+def run_paper_regime(args):
+    """Second workload: synthetic valence-only water clusters of the sizes of the paper's Table I
+    (8, 16, 24, 152 electrons) with the paper's 4320 walkers per GPU rank and tau = 0.01.
+    Systems with <= 32 electrons per spin run a whole qmc_sweep call in one launch (small_sweep.cuh); every system is
+    also timed on the per-electron kernels (QMC_LARGE_PATH).  Four walkers of every run are checked against the oracle."""
+    import torch
+    import oracle
+    from paper_2504_07948_b200 import build as qbuild
+    torch.cuda.set_device(0)
+    qbuild.build()
+    import paper_2504_07948_b200 as qb
+    qb.load_library()
+    W, T, tau, seed = args.walkers or 4320, 10, 0.01, qi.MASTER_SEED
+    for n_water in (1, 2, 3, 19):
+        sysm = qi.water_cluster(n_water, seed, cfg=1)
+        pos = qi.initial_positions(sysm, 1, range(W), seed)
+        gsys = qb.qmc_init_from(sysm)
+        osys = oracle.OracleSystem(sysm)
+        ref = oracle.run_crowd(sysm, pos[:4], seed, range(4), 0, 2, tau, osys=osys)
+        k = min(16, sysm.n_up)
+        for path, flags in (("one-launch", 0), ("per-electron", qb.QMC_LARGE_PATH)):
+            if path == "one-launch" and sysm.n_up > 32:
+                continue
+            pos_dev = torch.from_numpy(pos).cuda()
+            gw = qb.qmc_walkers_create(gsys, pos_dev, seed, flags=flags)
+            qb.qmc_sweep(gw, 2, tau, k)                                   # warm-up, and the parity sample
+            bits = qb.qmc_get_accept_log(gw).cpu().numpy()[:, :, :4]
+            differ = int(((bits & 1) != (ref["bits"] & 1)).sum())
+            e_err = float(np.abs(qb.qmc_get_eloc(gw)[0].cpu().numpy()[:4] - ref["eloc"][-1]).max())
+            l0 = qb.qmc_launch_count()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            ev0.record()
+            qb.qmc_sweep(gw, T, tau, k)
+            ev1.record()
+            torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1)
+            launches = qb.qmc_launch_count() - l0
+            st = qb.qmc_get_stats(gw)
+            qb.qmc_walkers_destroy(gw)
+            moves = W * sysm.n_elec * T
+            print(json.dumps(dict(metric=METRIC, value=moves / (ms * 1e-3), unit=UNIT, n_gpus=1, steps=T, warmup=2, ms_per_step=ms / T,
+                                  dtype="f64", data="synthetic", path=path, gpu_launches=int(launches),
+                                  walkers_per_s=W * T / (ms * 1e-3),
+                                  config=dict(workload=f"{sysm.name}: {sysm.n_elec} valence electrons, {sysm.n_basis} GTOs, {W} walkers, tau {tau}, "
+                                                       f"delay_k {k if path == 'per-electron' else 1}"),
+                                  accept_frac=st["accepted"] / st["proposed"], nonfinite=st["nonfinite"],
+                                  oracle_check=dict(walkers=4, sweeps=2, decisions_differing=differ, max_abs_eloc_diff=e_err))), flush=True)
+
+
 def main():
     args = parse()
-    if args.config4_sweep:
+    if args.paper_regime:
+        run_paper_regime(args)
+    elif args.config4_sweep:
         run_config4(args)
     elif args.impl == "reference":
         run_reference(args)
