@@ -46,6 +46,13 @@ extern "C" {
 
 /* flags of qmc_walkers_create */
 #define QMC_LOG_RATIOS 1u /* also record rho_D*exp(dJ) and p_acc of every proposed move */
+#define QMC_SCREEN_MO 4u  /* optional screening of the MO contraction (off by default; SURVEY 8(d).1 allows it where the
+                             parity tolerances still hold): a 128-row x 32-function stage of the basis matrix Phi whose
+                             largest |entry| (value, gradient, Laplacian) is below QMC_SCREEN_THETA is not contracted.  With
+                             orthonormal MO columns the orbital rows change by at most sqrt(N_b) * theta ~ 1e-22 absolute,
+                             far below the rounding of the sums.  The work saved depends on how localised the crowd's
+                             electron is; qmc_get_mo_work reports it. */
+#define QMC_SCREEN_THETA 1e-24
 #define QMC_LARGE_PATH 2u /* never use the one-launch small-system path (row f4): systems with <= 32 electrons per spin
                              whose per-walker state fits in shared memory otherwise run a whole qmc_sweep / qmc_dmc_step
                              call in one kernel, one warp per walker, with rank-1 updates (delay_k then only changes
@@ -152,6 +159,10 @@ int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff);
  * NULL): sum w E_L / sum w before the reconfiguration.  Must be called between sweeps (the delay window is empty then);
  * synchronises the stream. */
 int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed);
+
+/* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
+ * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
+int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);
 
 /* Stage-level entry points (used by the per-stage parity tests and the per-stage roofline bench).
  * Basis functions at n_points positions: out[n][5][n_basis] = value, d/dx, d/dy, d/dz, laplacian. */

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libqmc_b200.so")
 QMC_OK, QMC_ERR_ARG, QMC_ERR_CUDA, QMC_ERR_SINGULAR, QMC_ERR_NOMEM, QMC_ERR_STATE = 0, -1, -2, -3, -4, -5
 QMC_LOG_RATIOS = 1
 QMC_LARGE_PATH = 2
+QMC_SCREEN_MO = 4
 STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc")
 
 EXPORTED = [
@@ -24,7 +25,7 @@ EXPORTED = [
     "qmc_get_Ainv", "qmc_get_logpsi", "qmc_get_eloc", "qmc_get_accept_log", "qmc_get_ratio_log", "qmc_get_stats",
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
-    "qmc_dmc_step", "qmc_get_weights", "qmc_branch",
+    "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work",
 ]
 
 
@@ -89,6 +90,7 @@ def load_library(path: str | None = None):
     lib.qmc_dmc_step.argtypes = [vp, i, d, i, d, d]
     lib.qmc_get_weights.argtypes = [vp, vp, vp]
     lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
+    lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
     lib.qmc_version.restype = C.c_char_p
@@ -232,6 +234,13 @@ def qmc_get_weights(walkers: Walkers, out=None, out_tau_eff=None):
     out_tau_eff = _out((walkers.n_walkers,), torch.float64, out_tau_eff)
     _check(load_library().qmc_get_weights(walkers.handle, _ptr(out), _ptr(out_tau_eff)))
     return out, out_tau_eff
+
+
+def qmc_get_mo_work(walkers: Walkers):
+    """(executed, dense) (tile, k-block) iterations of the MO contraction since creation (QMC_SCREEN_MO sets only)."""
+    a, b = C.c_uint64(), C.c_uint64()
+    _check(load_library().qmc_get_mo_work(walkers.handle, C.byref(a), C.byref(b)))
+    return a.value, b.value
 
 
 def qmc_branch(walkers: Walkers, out_source=None):

@@ -85,8 +85,34 @@ struct MoArgs {
     double* ws;          // [grid][128*128] partial accumulators
     unsigned* flags;     // [grid] epoch stamps
     unsigned epoch;
+    // optional screening plan (MoPlan below): NULL = every k-block of every tile (dense)
+    const int* plan_cnt;   // [MT]      kept k-blocks of row tile tm (>= 1)
+    const int* plan_pre;   // [MT + 1]  NT * (cnt[0] + ... + cnt[tm-1]); plan_pre[MT] = total iterations
+    const int* plan_kb;    // [MT][KB]  the kept k-blocks of tm, ascending
 };
 
+// Where a flattened iteration lies.  Dense: tiles of KB iterations.  Screened: the tiles of row tile tm have cnt[tm]
+// iterations each (only the A stages whose largest entry reaches the threshold), tiles ordered tm-major.
+struct MoLoc { int tm, tn, i, cnt; long tile_begin; };
+template <bool SCREEN>
+__device__ __forceinline__ MoLoc mo_locate(const MoArgs& g, long it) {
+    MoLoc L;
+    if (!SCREEN) {
+        const long tile = it / g.KB;
+        L.tm = (int)(tile / g.NT); L.tn = (int)(tile - (long)L.tm * g.NT);
+        L.cnt = g.KB; L.tile_begin = tile * g.KB; L.i = (int)(it - L.tile_begin);
+    } else {
+        int tm = 0;
+        while (tm + 1 < g.MT && it >= g.plan_pre[tm + 1]) tm++;
+        const int c = g.plan_cnt[tm];
+        const long r = it - g.plan_pre[tm];
+        L.tm = tm; L.tn = (int)(r / c); L.cnt = c; L.i = (int)(r - (long)L.tn * c);
+        L.tile_begin = g.plan_pre[tm] + (long)L.tn * c;
+    }
+    return L;
+}
+
+template <bool SCREEN>
 __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
     extern __shared__ __align__(128) unsigned char mo_smem_raw[];
     double* stages = reinterpret_cast<double*>(mo_smem_raw);
@@ -100,7 +126,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
     }
     __syncthreads();
 
-    const long total = (long)g.MT * g.NT * g.KB;
+    const long total = SCREEN ? (long)g.plan_pre[g.MT] : (long)g.MT * g.NT * g.KB;
     const long it0 = total * blockIdx.x / gridDim.x, it1 = total * (blockIdx.x + 1) / gridDim.x;
     constexpr uint32_t STAGE_BYTES = (MO_A_STAGE + MO_B_STAGE) * 8;
 
@@ -112,9 +138,8 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
                 const int s = n % MO_STAGES;
                 const uint32_t round = n / MO_STAGES;
                 if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
-                const long tile = it / g.KB;
-                const int kb = (int)(it - tile * g.KB);
-                const int tm = (int)(tile / g.NT), tn = (int)(tile - (long)tm * g.NT);
+                const MoLoc L = mo_locate<SCREEN>(g, it);
+                const int tm = L.tm, tn = L.tn, kb = SCREEN ? g.plan_kb[(long)tm * g.KB + L.i] : L.i;
                 double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
                 mbar_expect_tx(&full[s], STAGE_BYTES);
                 bulk_g2s(As, g.PhiT + ((long)tm * g.KB + kb) * MO_A_STAGE, MO_A_STAGE * 8, &full[s]);
@@ -130,11 +155,11 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
     uint32_t n = 0;
     long it = it0;
     while (it < it1) {
-        const long tile = it / g.KB;
-        const int ka = (int)(it - tile * g.KB);
+        const MoLoc L = mo_locate<SCREEN>(g, it);
+        const int ka = L.i, KBt = L.cnt;  // this segment starts at iteration ka of a tile of KBt iterations
         const long rem = it1 - it;
-        const int kb_end = (rem < (long)(g.KB - ka)) ? (int)(ka + rem) : g.KB;
-        const int tm = (int)(tile / g.NT), tn = (int)(tile - (long)tm * g.NT);
+        const int kb_end = (rem < (long)(KBt - ka)) ? (int)(ka + rem) : KBt;
+        const int tm = L.tm, tn = L.tn;
         double acc[MO_TM][MO_TN][2];
 #pragma unroll
         for (int i = 0; i < MO_TM; i++)
@@ -163,7 +188,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
         it += kb_end - ka;
 
         // ---- epilogue of this segment
-        const bool head = (ka == 0), whole = head && (kb_end == g.KB);
+        const bool head = (ka == 0), whole = head && (kb_end == KBt);
         if (!head) {
             // park the partial tile for the owner (CTA with the tile's first k-block), then publish
             double* ws = g.ws + (size_t)blockIdx.x * MO_WS_DOUBLES;
@@ -182,28 +207,30 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
         } else {
             if (!whole) {
                 // owner: add the partials of the CTAs that hold the rest of this tile, in ascending k order
-                long covered = (tile * g.KB + kb_end);  // first iteration not yet summed
-                const long tile_end = (tile + 1) * g.KB;
+                long covered = L.tile_begin + kb_end;  // first iteration not yet summed
+                const long tile_end = L.tile_begin + KBt;
                 int peer = blockIdx.x + 1;
                 while (covered < tile_end) {
-                    if (tid == 0) {
-                        unsigned v;
-                        do {
-                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(g.flags + peer) : "memory");
-                            if (v != g.epoch) __nanosleep(64);
-                        } while (v != g.epoch);
-                    }
-                    consumer_bar();
-                    const double* ws = g.ws + (size_t)peer * MO_WS_DOUBLES;
-#pragma unroll
-                    for (int i = 0; i < MO_TM; i++)
-#pragma unroll
-                        for (int j = 0; j < MO_TN; j++) {
-                            acc[i][j][0] += __ldcg(ws + ((i * MO_TN + j) * 2 + 0) * 256 + tid);
-                            acc[i][j][1] += __ldcg(ws + ((i * MO_TN + j) * 2 + 1) * 256 + tid);
+                    const long peer_begin = total * peer / gridDim.x, peer_end = total * (peer + 1) / gridDim.x;
+                    if (peer_end > peer_begin) {  // (a CTA whose range is empty never publishes)
+                        if (tid == 0) {
+                            unsigned v;
+                            do {
+                                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(g.flags + peer) : "memory");
+                                if (v != g.epoch) __nanosleep(64);
+                            } while (v != g.epoch);
                         }
-                    const long peer_end = total * (peer + 1) / gridDim.x;
-                    covered = peer_end < tile_end ? peer_end : tile_end;
+                        consumer_bar();
+                        const double* ws = g.ws + (size_t)peer * MO_WS_DOUBLES;
+#pragma unroll
+                        for (int i = 0; i < MO_TM; i++)
+#pragma unroll
+                            for (int j = 0; j < MO_TN; j++) {
+                                acc[i][j][0] += __ldcg(ws + ((i * MO_TN + j) * 2 + 0) * 256 + tid);
+                                acc[i][j][1] += __ldcg(ws + ((i * MO_TN + j) * 2 + 1) * 256 + tid);
+                            }
+                        covered = peer_end < tile_end ? peer_end : tile_end;
+                    }
                     peer++;
                 }
             }

@@ -346,6 +346,12 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     CUW(w->pool.alloc((void**)&w->d_comb, (4 * W + 1) * 4, st));
     CUW(w->pool.alloc((void**)&w->d_emixed, 8, st));
     CUW(launch_fill_double(d.weight, n_walkers, 1.0, st));
+    d.screen_theta = (flags & QMC_SCREEN_MO) ? QMC_SCREEN_THETA : -1.0;
+    CUW(w->pool.alloc((void**)&d.tilemax, (size_t)d.mt * s.kb * 8, st));
+    CUW(w->pool.alloc((void**)&d.plan_cnt, (size_t)d.mt * 4, st));
+    CUW(w->pool.alloc((void**)&d.plan_pre, (size_t)(d.mt + 1) * 4, st));
+    CUW(w->pool.alloc((void**)&d.plan_kb, (size_t)d.mt * s.kb * 4, st));
+    CUW(w->pool.alloc((void**)&d.mo_work, 2 * 8, st));
     CUW(w->pool.alloc((void**)&w->d_status, 4, st));
     rc = alloc_window(w, 16);
     if (rc) { std::string m = g_err; destroy_walkers(w); return fail(rc, m); }
@@ -380,8 +386,8 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         const int e0 = sp == 0 ? 0 : s.ns[0];
         for (int p = 0; p < s.ns[sp]; p++) {
             CUF(launch_gather_rp(d, e0 + p, st));
-            CUF(launch_basis(s, d.rp, n_walkers, d.Phi, st));
-            CUF(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * n_walkers, d.mo_grid), ++w->mo_epoch, st));
+            CUF(launch_basis(s, d.rp, n_walkers, d.Phi, nullptr, st));
+            CUF(launch_mo(s, sp, d.Phi, 5 * n_walkers, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * n_walkers, d.mo_grid), ++w->mo_epoch, nullptr, st));
             CUF(launch_store_init_rows(s, d, sp, p, st));
         }
         CUF(launch_gj_inverse(d.AinvT[sp], (long)s.nsp[sp] * s.nsp[sp], s.ns[sp], s.nsp[sp], n_walkers, d.logpsi, d.sign, w->d_status, E, st));
@@ -512,10 +518,13 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
                     prof_end(w, pf);
                 }
                 prof_begin(w, 1, prof);
-                CU(launch_basis(s, d.rp, d.W, d.Phi, st));
+                const bool screen = d.screen_theta >= 0.0;
+                CU(launch_basis(s, d.rp, d.W, d.Phi, screen ? d.tilemax : nullptr, st));
                 prof_end(w, prof);
                 prof_begin(w, 2, prof);
-                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch, st));
+                if (screen) CU(launch_mo_plan(s, sp, d, 5 * d.W, st));
+                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch,
+                             screen ? &d : nullptr, st));
                 prof_end(w, prof);
                 in_window++;
                 if (in_window == delay_k || p == ns - 1) {
@@ -560,6 +569,16 @@ extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
     }
     if (e_mixed) CU(cudaMemcpyAsync(e_mixed, w->d_emixed, 8, cudaMemcpyDefault, st));
     CU(cudaStreamSynchronize(st));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_get_mo_work: null walkers");
+    unsigned long long h[2];
+    CU(cudaMemcpyAsync(h, w->d.mo_work, sizeof(h), cudaMemcpyDeviceToHost, w->stream));
+    CU(cudaStreamSynchronize(w->stream));
+    if (executed) *executed = h[0];
+    if (dense) *dense = h[1];
     return QMC_OK;
 }
 
@@ -690,11 +709,11 @@ static int eval_common(const qmc_system* sys, int spin, int n_points, const doub
     const bool dev_out = is_device_ptr(out);
     if (e == cudaSuccess && !dev_out) e = cudaMalloc((void**)&stage, out_bytes + 16);
     if (e == cudaSuccess) e = cudaMemcpyAsync(pts, xyz, (size_t)n_points * 3 * 8, cudaMemcpyDefault, st);
-    if (e == cudaSuccess) e = launch_basis(s, pts, n_points, Phi, st);
+    if (e == cudaSuccess) e = launch_basis(s, pts, n_points, Phi, nullptr, st);
     double* dst = dev_out ? out : stage;
     if (e == cudaSuccess) {
         if (mo) {
-            e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], ws, flags, grid, 1u, st);
+            e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], ws, flags, grid, 1u, nullptr, st);
             if (e == cudaSuccess) e = launch_export_rows(V, (long)n_points * 5, width, s.nsp[spin], dst, st);
         } else {
             e = launch_export_phi(Phi, (long)n_points * 5, width, s.kb, dst, st);
@@ -734,8 +753,8 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
     // make the inputs of the later stages valid
     CU(launch_step(s, d, spin, -1, p, 0, w->step, 0.005, 1, st));
     const int mgrid = mo_grid_for(s, spin, 5 * d.W, d.mo_grid);
-    CU(launch_basis(s, d.rp, d.W, d.Phi, st));
-    CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st));
+    CU(launch_basis(s, d.rp, d.W, d.Phi, nullptr, st));
+    CU(launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, nullptr, st));
     if (stage == 4) CU(launch_fill_int(d.mcount, d.W, delay_k, st));  // full window, S^-1 = 0: zero correction
     cudaError_t err = cudaSuccess;
     for (int r = -2; r < reps && err == cudaSuccess; r++) {
@@ -743,8 +762,8 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
         if (err != cudaSuccess) break;
         switch (stage) {
             case 0: err = launch_step(s, d, spin, -1, p, 0, w->step, 0.005, 1, st); break;
-            case 1: err = launch_basis(s, d.rp, d.W, d.Phi, st); break;
-            case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, st); break;
+            case 1: err = launch_basis(s, d.rp, d.W, d.Phi, nullptr, st); break;
+            case 2: err = launch_mo(s, spin, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++w->mo_epoch, nullptr, st); break;
             case 3: err = launch_step(s, d, spin, p, p, 0, w->step, 0.005, 0, st); break;
             case 4:
                 err = launch_flush(s, d, spin, st);

@@ -77,6 +77,13 @@ struct WalkDev {
     // sums of |sqrt(tau) chi|^2 over accepted / all proposals [W][2], the pending proposal's value [W], tau_eff [W]
     double lim_a;
     double *weight, *eold, *dr2, *dr2p, *tau_eff;
+    // optional screening of the MO contraction (QMC_SCREEN_MO): A stages whose largest |entry| is below screen_theta are
+    // not contracted.  tilemax [MT][KB] from k_basis; plan_* from k_mo_plan (see mo_streamk.cuh); mo_work [2]: executed
+    // and dense (tile, k-block) iterations since creation.  screen_theta < 0: off, the plan is not used.
+    double screen_theta;
+    double* tilemax;
+    int *plan_cnt, *plan_pre, *plan_kb;
+    unsigned long long* mo_work;
 };
 
 }  // namespace qmc

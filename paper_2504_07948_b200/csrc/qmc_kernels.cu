@@ -50,9 +50,13 @@ constexpr int BASIS_MAXPT = (MO_BM + 4) / 5 + 1;  // points that can touch one 1
 // shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
 // stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
 // issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
-__global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out) {
+__global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
+                                                             double* __restrict__ tilemax /* [MT][KB] or NULL: max |entry| of every stage */) {
     __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
     __shared__ double spt[3 * BASIS_MAXPT + 3];
+    __shared__ unsigned long long smax;  // bit pattern of a non-negative double: integer order = numeric order
+    if (threadIdx.x == 0) smax = 0ull;
+    double vmax = 0.0;
     const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
     const int row_lo = tm * MO_BM;
     const int pt_lo = row_lo / 5;
@@ -104,7 +108,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
             for (int k = 0; k < 5; k++)
-                if (r0 + k >= 0 && r0 + k < MO_BM) tile[(r0 + k) * MO_ALD + col] = v[k];
+                if (r0 + k >= 0 && r0 + k < MO_BM) { tile[(r0 + k) * MO_ALD + col] = v[k]; vmax = fmax(vmax, fabs(v[k])); }
         };
         const double s3 = 1.7320508075688772;
         if (L == 0) {
@@ -121,19 +125,25 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
         }
     }
+    if (tilemax) {  // NaN entries count as +inf: such a stage is never screened out
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+        if ((tid & 31) == 0) atomicMax(&smax, (unsigned long long)__double_as_longlong(vmax));
+    }
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // generic-proxy smem writes -> visible to the TMA engine
     __syncthreads();
     if (tid == 0) {
+        if (tilemax) tilemax[tm * s.kb + kb] = __longlong_as_double((long long)smax);
         bulk_s2g(out + ((long)tm * s.kb + kb) * MO_A_STAGE, tile, MO_A_STAGE * sizeof(double));
         asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory");  // smem must outlive the read
     }
 }
 
-cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
     dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
-    k_basis<<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT);
+    k_basis<<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
@@ -147,11 +157,41 @@ int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm) {
     return (int)(total < n_sm ? total : n_sm);
 }
 
+// Screening plan of one contraction: a thread per row tile keeps the k-blocks whose largest entry reaches theta
+// (ascending; at least one, so every output tile is written), thread 0 builds the prefix of iterations.
+__global__ void __launch_bounds__(256) k_mo_plan(const double* __restrict__ tilemax, int MT, int KB, int NT, double theta, int* cnt, int* pre,
+                                                 int* kbl, unsigned long long* work) {
+    for (int tm = threadIdx.x; tm < MT; tm += blockDim.x) {
+        int c = 0;
+        for (int kb = 0; kb < KB; kb++)
+            if (!(tilemax[(long)tm * KB + kb] < theta)) kbl[(long)tm * KB + c++] = kb;
+        if (c == 0) { kbl[(long)tm * KB] = 0; c = 1; }
+        cnt[tm] = c;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int tm = 0; tm < MT; tm++) { pre[tm] = acc; acc += NT * cnt[tm]; }
+        pre[MT] = acc;
+        work[0] += (unsigned long long)acc;
+        work[1] += (unsigned long long)MT * NT * KB;
+    }
+}
+
+cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int rows, cudaStream_t st) {
+    const int MT = (rows + MO_BM - 1) / MO_BM;
+    k_mo_plan<<<1, 256, 0, st>>>(wd.tilemax, MT, s.kb, s.nt[spin], wd.screen_theta, wd.plan_cnt, wd.plan_pre, wd.plan_kb, wd.mo_work);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// plan: NULL for the dense contraction, else the walker set whose plan_* buffers launch_mo_plan has just filled
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
-                      int grid, unsigned epoch, cudaStream_t st) {
+                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st) {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -160,8 +200,10 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
     g.M = rows; g.N = s.nsp[spin];
     g.MT = (rows + MO_BM - 1) / MO_BM; g.NT = s.nt[spin]; g.KB = s.kb;
     g.ws = ws; g.flags = flags; g.epoch = epoch;
+    g.plan_cnt = plan ? plan->plan_cnt : nullptr; g.plan_pre = plan ? plan->plan_pre : nullptr; g.plan_kb = plan ? plan->plan_kb : nullptr;
     if (grid < 1) return cudaSuccess;
-    k_mo_streamk<<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
+    if (plan) k_mo_streamk<true><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
+    else k_mo_streamk<false><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

@@ -4,9 +4,11 @@
 
 namespace qmc {
 
-cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st);
+// tilemax ([MT][KB], may be NULL): max |entry| of every A stage, for the optional screening of the MO contraction
+cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st);
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
-                      int grid, unsigned epoch, cudaStream_t st);
+                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st);
+cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int rows, cudaStream_t st);
 int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm);
 size_t mo_ws_bytes(int grid);
 size_t phiT_bytes(const SysDev& s, int rows);

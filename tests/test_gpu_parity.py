@@ -355,3 +355,33 @@ def test_config3_mo_rows_full_size():
         for n in (0, 7, 25, 26, 39):
             ref = o.mo_rows(spin, pts[n])
             assert np.abs(M[n] - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------ optional screening of the MO contraction
+
+def test_screened_contraction_matches_oracle_config1():
+    wl = qi.make_workload(1)
+    # the walkers, sweeps and floors of test_config1_trajectories_subset_delay32, with the screening on
+    rep = run_and_compare(wl, range(100, 124), 4, wl.delay_k, floor=True, flags=qb.QMC_LOG_RATIOS | qb.QMC_SCREEN_MO)
+    _assert_report(rep)
+
+
+def test_screened_contraction_equals_dense_config2():
+    # 256-water system, 64 walkers, one sweep with delay_k 64: skipping the A stages whose largest entry is below 1e-24
+    # changes no decision and moves nothing beyond rounding, while a good part of the contraction is not executed
+    wl = qi.make_workload(2, n_walkers=64)
+    g = qb.qmc_init_from(wl.system)
+    out = {}
+    for name, flags in (("dense", 0), ("screened", qb.QMC_SCREEN_MO)):
+        gw = qb.qmc_walkers_create(g, wl.positions(), wl.seed, flags=flags)
+        qb.qmc_sweep(gw, 1, wl.tau, wl.delay_k)
+        out[name] = (qb.qmc_get_accept_log(gw).cpu().numpy(), qb.qmc_get_positions(gw).cpu().numpy(),
+                     qb.qmc_get_eloc(gw)[0].cpu().numpy(), qb.qmc_get_logpsi(gw)[0].cpu().numpy(), qb.qmc_get_mo_work(gw))
+        qb.qmc_walkers_destroy(gw)
+    a, b = out["dense"], out["screened"]
+    assert np.array_equal(a[0] & 1, b[0] & 1)
+    assert np.abs(a[1] - b[1]).max() < TOL_POS
+    assert np.abs(a[3] - b[3]).max() < 1e-10 * np.abs(a[3]).max()
+    assert np.abs(a[2] - b[2]).max() < 1e-6          # E_L ~ 1e4 Ha: rounding-level agreement (reading A26)
+    executed, dense = b[4]
+    assert a[4] == (0, 0) and dense == 2048 * 3 * 8 * 192 and executed < 0.8 * dense
