@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--paper-regime", action="store_true",
                     help="row f4: the paper's own regime -- water clusters of 8/16/24/152 valence electrons, 4320 walkers per GPU "
                          "(PAPER.md L279-302) -- on the one-launch small-system path and on the per-electron path; one JSON line each")
+    ap.add_argument("--no-screened", action="store_true", help="skip the extra leg with QMC_SCREEN_MO")
     ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -257,6 +258,7 @@ def run_ours(args):
     assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
     assert st1["nonfinite"] == 0
     red = reduce_report(ms, n_moves, float(eloc.sum()), float((eloc * eloc).sum()), W, backend_device="cuda")
+    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not args.no_screened else None
     # row f1 (outside the timed region): one DMC generation + one comb reconfiguration on the same crowd
     f1 = None
     if not args.no_dmc:
@@ -273,6 +275,31 @@ def run_ours(args):
                   walkers_copied=int((src.cpu().numpy() != np.arange(W)).sum()), e_trial=e_t, e_mixed=e_mixed, limiter_a=1.0,
                   what="qmc_dmc_step(1) = sweep with limited drift + weight update; qmc_branch = comb + copies of A^-1 and row caches")
     qb.qmc_walkers_destroy(gw)
+
+    # ---- the same K sweeps with the optional screening of the MO contraction (QMC_SCREEN_MO); NOT the headline value
+    screened = None
+    if not args.no_screened:
+        gw3 = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=qb.QMC_SCREEN_MO)
+        for _ in range(args.warmup):
+            qb.qmc_sweep(gw3, 1, wl.tau, k)
+        w0 = qb.qmc_get_mo_work(gw3)
+        ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev2.record()
+        qb.qmc_sweep(gw3, args.steps, wl.tau, k)
+        ev3.record()
+        torch.cuda.synchronize()
+        ms3 = ev2.elapsed_time(ev3)
+        w1 = qb.qmc_get_mo_work(gw3)
+        sb = qb.qmc_get_accept_log(gw3).cpu().numpy()
+        el3 = qb.qmc_get_eloc(gw3)[0]
+        screened = dict(value=W * sysm.n_elec * args.steps / (ms3 * 1e-3), unit=UNIT, ms_per_step=ms3 / args.steps,
+                        theta=1e-24, stages_executed_frac=(w1[0] - w0[0]) / max(w1[1] - w0[1], 1),
+                        decisions_differing_from_dense=int(((sb & 1) != (dense_bits & 1)).sum()), decisions_compared=int(sb.size),
+                        max_abs_eloc_diff_from_dense=float((el3 - eloc).abs().max()),
+                        what="same crowd, same sweeps, A stages of Phi whose largest |entry| is below theta not contracted "
+                             "(per GPU; rank 0's crowd); the headline `value` above is the dense contraction")
+        qb.qmc_walkers_destroy(gw3)
 
     # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps
     e2e = None
@@ -352,6 +379,7 @@ def run_ours(args):
         stage_share={s: share[s] / tot_share for s in share},
         eloc_mean=red["e_sum"] / red["n_walkers"],
         f1_dmc=f1,
+        screened_mo=screened,
     )
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = oracle_sample(wl, 3, 1, args.cpu_moves)[0]
