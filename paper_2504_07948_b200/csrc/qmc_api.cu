@@ -147,6 +147,42 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
         f += 2 * sh_l[i] + 1;
     }
     if (f != mo->n_basis) return fail(QMC_ERR_ARG, "qmc_init: n_basis != sum over shells of 2l+1");
+    // Internal order of the basis functions (the K index of the contraction; any order gives the same sums up to rounding):
+    // shells grouped by how far they reach -- sqrt(ln(1/theta) / smallest exponent) -- and, inside a group, along a Morton
+    // curve through their centres, so that the 32 functions of a k-block die off together in space.  It is what makes the
+    // optional screening (QMC_SCREEN_MO) effective; the caller's order is kept at the ABI (C rows in, qmc_eval_basis out).
+    std::vector<int> order(basis->n_shells), fmap(mo->n_basis);
+    {
+        double lo3[3] = {1e300, 1e300, 1e300}, hi3[3] = {-1e300, -1e300, -1e300};
+        for (const ShellRec& r : recs) {
+            const double c[3] = {r.x, r.y, r.z};
+            for (int q = 0; q < 3; q++) { lo3[q] = std::min(lo3[q], c[q]); hi3[q] = std::max(hi3[q], c[q]); }
+        }
+        std::vector<uint64_t> key(basis->n_shells);
+        for (int i = 0; i < basis->n_shells; i++) {
+            double amin = 1e300;
+            for (int q = 0; q < recs[i].nprim; q++) amin = std::min(amin, fabs(alpha[recs[i].poff + q]));
+            const double reach = amin > 0.0 ? sqrt(55.0 / amin) : 1e300;
+            int cls = 0;
+            for (double edge : {3.0, 5.0, 8.0, 12.0, 17.0}) cls += reach > edge;
+            const double c[3] = {recs[i].x, recs[i].y, recs[i].z};
+            uint64_t mort = 0;
+            for (int q = 0; q < 3; q++) {
+                const double span = hi3[q] - lo3[q];
+                uint64_t v = span > 0.0 ? (uint64_t)((c[q] - lo3[q]) / span * 1023.0) : 0;
+                for (int b = 0; b < 10; b++) mort |= ((v >> b) & 1ull) << (3 * b + q);
+            }
+            key[i] = ((uint64_t)cls << 32) | mort;
+            order[i] = i;
+        }
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key[a] < key[b]; });
+        int fn = 0;
+        for (int i : order) {
+            for (int m = 0; m < 2 * recs[i].l + 1; m++) fmap[recs[i].f0 + m] = fn + m;
+            recs[i].f0 = fn;
+            fn += 2 * recs[i].l + 1;
+        }
+    }
 
     qmc_system* S = new qmc_system();
     S->stream = st;
@@ -182,17 +218,17 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     {   // shells that own a function of each 32-function k-block (a shell may straddle two blocks), grouped by l
         std::vector<int4> cnts(d.kb);
         std::vector<KbShell> list;
-        int lo = 0;
+        int lo = 0;  // positions in `order` (the shells sorted by their first internal function)
         for (int kb = 0; kb < d.kb; kb++) {
             const int f_lo = kb * 32, f_hi = f_lo + 32;
-            while (lo < basis->n_shells && recs[lo].f0 + 2 * recs[lo].l + 1 <= f_lo) lo++;
+            while (lo < basis->n_shells && recs[order[lo]].f0 + 2 * recs[order[lo]].l + 1 <= f_lo) lo++;
             int hi = lo;
-            while (hi < basis->n_shells && recs[hi].f0 < f_hi) hi++;
+            while (hi < basis->n_shells && recs[order[hi]].f0 < f_hi) hi++;
             int c[3] = {0, 0, 0};
             const int off = (int)list.size();
             for (int l = 0; l < 3; l++)
-                for (int i = lo; i < hi; i++)
-                    if (recs[i].l == l) {
+                for (int oi = lo; oi < hi; oi++)
+                    if (const int i = order[oi]; recs[i].l == l) {
                         KbShell k;
                         memset(&k, 0, sizeof(k));
                         k.x = recs[i].x; k.y = recs[i].y; k.z = recs[i].z;
@@ -213,6 +249,11 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
         CUS(cudaStreamSynchronize(st));
         d.kb_counts = dcn;
         d.kb_list = dli;
+        int* dfm;
+        CUS(S->pool.alloc((void**)&dfm, fmap.size() * sizeof(int), st));
+        CUS(cudaMemcpyAsync(dfm, fmap.data(), fmap.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+        CUS(cudaStreamSynchronize(st));
+        d.fmap = dfm;
     }
     for (int sp = 0; sp < 2; sp++) {
         double* dC;
@@ -224,7 +265,7 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
             size_t bytes = (size_t)d.n_basis * d.ns[sp] * 8;
             CUS(cudaMalloc((void**)&tmp, bytes));
             cudaError_t e = cudaMemcpyAsync(tmp, src, bytes, cudaMemcpyDefault, st);
-            if (e == cudaSuccess) e = launch_tile_C(tmp, d.n_basis, d.ns[sp], dC, d.kb, st);
+            if (e == cudaSuccess) e = launch_tile_C(tmp, d.n_basis, d.ns[sp], dC, d.kb, d.fmap, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             cudaFree(tmp);
             CUS(e);
@@ -716,7 +757,7 @@ static int eval_common(const qmc_system* sys, int spin, int n_points, const doub
             e = launch_mo(s, spin, Phi, 5 * n_points, V, s.nsp[spin], ws, flags, grid, 1u, nullptr, st);
             if (e == cudaSuccess) e = launch_export_rows(V, (long)n_points * 5, width, s.nsp[spin], dst, st);
         } else {
-            e = launch_export_phi(Phi, (long)n_points * 5, width, s.kb, dst, st);
+            e = launch_export_phi(Phi, (long)n_points * 5, width, s.kb, s.fmap, dst, st);
         }
     }
     if (e == cudaSuccess && !dev_out) e = cudaMemcpyAsync(out, stage, out_bytes, cudaMemcpyDeviceToHost, st);

@@ -42,6 +42,7 @@ struct SysDev {
     const ShellRec* shells;
     const int4* kb_counts;  // [kb]: number of s, p, d shells owning a function of k-block kb (32 functions), list offset
     const KbShell* kb_list; // shells of every k-block, grouped s | p | d (a shell may be in two blocks)
+    const int* fmap;        // [n_basis] caller's function index -> internal one (shells grouped by reach, Morton-ordered)
     const double* alpha;
     const double* coef;
     const double* CT[2];  // tiled, see mo_streamk.cuh

@@ -743,28 +743,29 @@ cudaError_t launch_export_rows(const double* src, long n_rows, int width, long l
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
-__global__ void k_tile_C(const double* __restrict__ in, int nb, int ns, double* __restrict__ CT, int kb) {
+__global__ void k_tile_C(const double* __restrict__ in, int nb, int ns, double* __restrict__ CT, int kb, const int* __restrict__ fmap) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long)nb * ns) return;
     const int l = (int)(idx / ns), j = (int)(idx % ns);
-    CT[cT_index(l, j, kb)] = in[idx];
+    CT[cT_index(fmap[l], j, kb)] = in[idx];
 }
-cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, cudaStream_t st) {
+cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, const int* fmap, cudaStream_t st) {
     long n = (long)nb * ns;
     if (n == 0) return cudaSuccess;
-    k_tile_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, CT, kb);
+    k_tile_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, CT, kb, fmap);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
-__global__ void k_export_phi(const double* __restrict__ PhiT, long n_rows, int width, int kb, double* __restrict__ out) {
+__global__ void k_export_phi(const double* __restrict__ PhiT, long n_rows, int width, int kb, const int* __restrict__ fmap,
+                             double* __restrict__ out) {
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= n_rows * width) return;
-    out[idx] = PhiT[phiT_index(idx / width, (int)(idx % width), kb)];
+    out[idx] = PhiT[phiT_index(idx / width, fmap[(int)(idx % width)], kb)];
 }
-cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, double* out, cudaStream_t st) {
+cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, const int* fmap, double* out, cudaStream_t st) {
     long n = n_rows * width;
     if (n == 0) return cudaSuccess;
-    k_export_phi<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(PhiT, n_rows, width, kb, out);
+    k_export_phi<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(PhiT, n_rows, width, kb, fmap, out);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

@@ -12,8 +12,8 @@ cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int row
 int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm);
 size_t mo_ws_bytes(int grid);
 size_t phiT_bytes(const SysDev& s, int rows);
-cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, cudaStream_t st);
-cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, double* out, cudaStream_t st);
+cudaError_t launch_tile_C(const double* in, int nb, int ns, double* CT, int kb, const int* fmap, cudaStream_t st);
+cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb, const int* fmap, double* out, cudaStream_t st);
 // p_acc >= 0: ratio + accept/reject + commit of electron p_acc (spin-local index); p_prop >= 0: proposal of p_prop
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st);
