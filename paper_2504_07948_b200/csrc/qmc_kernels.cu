@@ -212,14 +212,17 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 // a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st) {
-    static size_t configured = 48 * 1024;
+    static size_t configured[2] = {48 * 1024, 48 * 1024};
     const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp);
-    if (smem > configured) {
-        cudaError_t er = cudaFuncSetAttribute(k_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const bool wide = step_threads(s.nsp[spin]) == 512;
+    if (smem > configured[wide]) {
+        cudaError_t er = wide ? cudaFuncSetAttribute(k_step<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                              : cudaFuncSetAttribute(k_step<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (er != cudaSuccess) return er;
-        configured = smem;
+        configured[wide] = smem;
     }
-    k_step<<<wd.W, PT, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+    if (wide) k_step<512><<<wd.W, 512, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+    else k_step<128><<<wd.W, 128, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

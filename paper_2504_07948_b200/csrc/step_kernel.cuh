@@ -18,20 +18,21 @@
 
 namespace qmc {
 
-constexpr int PT = 512;
-constexpr int PW = PT / 32;
+// threads per walker: 512 for the large systems the kernel was tuned on (8 KB rows at config 2), 128 where a row of the
+// inverse is at most 256 doubles -- there 512 threads would mostly wait at barriers, and four times as many CTAs fit an SM
+__host__ __device__ inline int step_threads(int nsp) { return nsp <= 256 ? 128 : 512; }
 
 // shared-memory carve-up (in doubles)
 struct StepLayout {
     int xs, vs, as, c4, bs, cs, rs, ts, red, bc, total;
-    __host__ __device__ StepLayout(int nsp, int kp) {
+    __host__ __device__ StepLayout(int nsp, int kp, int PW /* warps per CTA */) {
         xs = 0; vs = xs + nsp; as = vs + nsp; c4 = as + nsp;
         bs = c4 + 512;
         cs = bs + kp + 1; rs = cs + kp + 1; ts = rs + kp + 1;
         red = ts + kp + 1; bc = red + 8 * PW; total = bc + 16;
     }
 };
-inline size_t step_smem_bytes(int nsp, int kp) { return (size_t)StepLayout(nsp, kp).total * sizeof(double); }
+inline size_t step_smem_bytes(int nsp, int kp) { return (size_t)StepLayout(nsp, kp, step_threads(nsp) / 32).total * sizeof(double); }
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 
@@ -93,13 +94,15 @@ __device__ __forceinline__ void limit_drift(double& gx, double& gy, double& gz, 
 
 // p_acc >= 0: finish the move of electron p_acc of this spin (needs its MO rows in V);  p_prop >= 0: propose the
 // move of electron p_prop.  commit == 0 evaluates the decision but changes no state (stage timing only).
-__global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
+template <int PT>
+__global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
                                                 double tau, double sqrt_tau, int commit) {
     extern __shared__ __align__(16) double sm[];
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], n2 = nsp >> 1, kp = wd.kp, nep = wd.nep;
     const int e0 = spin == 0 ? 0 : s.ns[0];
-    const StepLayout L(nsp, kp);
+    constexpr int PW = PT / 32;
+    const StepLayout L(nsp, kp, PW);
     double *xs = sm + L.xs, *vs = sm + L.vs, *as = sm + L.as, *c4 = sm + L.c4;
     double *bs = sm + L.bs, *cs = sm + L.cs, *rs = sm + L.rs, *ts = sm + L.ts, *red = sm + L.red, *bc = sm + L.bc;
     double* Rw = wd.R + (long)w * 3 * nep;
@@ -264,16 +267,17 @@ __global__ void __launch_bounds__(PT, 2) k_step(SysDev s, WalkDev wd, int spin, 
     const int m = m_old + (accepted ? 1 : 0);
     if (m > 0) {
         // c = S^-1 b: c_n = sum_l SinvT[l][n] b_l, 4 threads per n over interleaved l, fixed-order combine (kp <= 128)
+        constexpr int CP = PT / 128;  // threads per n
         {
             const int n = tid & 127, q = tid >> 7;
             double acc = 0.0;
             if (n < m)
-                for (int l = q; l < m; l += 4) acc += Si[l * kp + n] * bs[l];
+                for (int l = q; l < m; l += CP) acc += Si[l * kp + n] * bs[l];
             c4[q * 128 + n] = acc;
         }
         __syncthreads();
         for (int n = tid; n < m; n += PT) {
-            const double c = (c4[n] + c4[128 + n]) + (c4[256 + n] + c4[384 + n]);
+            const double c = CP == 4 ? (c4[n] + c4[128 + n]) + (c4[256 + n] + c4[384 + n]) : c4[n];
             cs[n] = c;
             wd.cvec[(long)w * kp + n] = c;
         }
