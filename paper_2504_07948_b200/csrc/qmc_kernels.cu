@@ -50,8 +50,9 @@ constexpr int BASIS_MAXPT = (MO_BM + 4) / 5 + 1;  // points that can touch one 1
 // shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
 // stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
 // issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
+template <bool TMAX>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
 __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
-                                                             double* __restrict__ tilemax /* [MT][KB] or NULL: max |entry| of every stage */) {
+                                                             double* __restrict__ tilemax) {
     __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
     __shared__ double spt[3 * BASIS_MAXPT + 3];
     __shared__ unsigned long long smax;  // bit pattern of a non-negative double: integer order = numeric order
@@ -108,7 +109,10 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
             for (int k = 0; k < 5; k++)
-                if (r0 + k >= 0 && r0 + k < MO_BM) { tile[(r0 + k) * MO_ALD + col] = v[k]; vmax = fmax(vmax, fabs(v[k])); }
+                if (r0 + k >= 0 && r0 + k < MO_BM) {
+                    tile[(r0 + k) * MO_ALD + col] = v[k];
+                    if (TMAX) vmax = fmax(vmax, v[k] == v[k] ? fabs(v[k]) : INFINITY);  // a NaN stage is never screened out
+                }
         };
         const double s3 = 1.7320508075688772;
         if (L == 0) {
@@ -125,7 +129,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
         }
     }
-    if (tilemax) {  // NaN entries count as +inf: such a stage is never screened out
+    if (TMAX) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) vmax = fmax(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
         if ((tid & 31) == 0) atomicMax(&smax, (unsigned long long)__double_as_longlong(vmax));
@@ -133,7 +137,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // generic-proxy smem writes -> visible to the TMA engine
     __syncthreads();
     if (tid == 0) {
-        if (tilemax) tilemax[tm * s.kb + kb] = __longlong_as_double((long long)smax);
+        if (TMAX) tilemax[tm * s.kb + kb] = __longlong_as_double((long long)smax);
         bulk_s2g(out + ((long)tm * s.kb + kb) * MO_A_STAGE, tile, MO_A_STAGE * sizeof(double));
         asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory");  // smem must outlive the read
@@ -143,7 +147,8 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
     dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
-    k_basis<<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
+    if (tilemax) k_basis<true><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
+    else k_basis<false><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
