@@ -102,8 +102,9 @@ int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basis* basis, c
 void qmc_finalize(qmc_system* sys);
 
 /* Create a crowd of n_walkers walkers at `positions` ([n_walkers][n_elec][3], ups first, host or device).
- * Evaluates all orbital rows, inverts the Slater matrices (Gauss-Jordan with partial pivoting on the
- * device), and sets log|Psi|, sign and E_L.  RNG streams are keyed (seed; first_walker_id + w, step,
+ * Evaluates all orbital rows, inverts the Slater matrices on the device (Gauss-Jordan with partial pivoting; from 256
+ * electrons per spin a blocked form with implicit row pivoting whose rank-16 updates are FP64 DMMA GEMMs; one
+ * Newton-Schulz refinement step either way), and sets log|Psi|, sign, E_L and unit weights.  RNG streams are keyed (seed; first_walker_id + w, step,
  * electron) with the step counter starting at first_step, so any crowd is a slice of one infinite
  * crowd (reading A20) and sweeps can be resumed bit for bit.  Returns QMC_ERR_SINGULAR if any Slater
  * matrix has a zero pivot.  All later work is enqueued on `cuda_stream`. */
