@@ -112,8 +112,13 @@ __device__ __forceinline__ MoLoc mo_locate(const MoArgs& g, long it) {
     return L;
 }
 
-template <bool SCREEN>
+// HALF: 64-row output tiles (the upper or lower half of an A stage; warp tiles 32 x 32) for contractions with so few
+// iterations per CTA that 128-row tiles would be split over many CTAs (config 1: 20 tiles x 24 k-blocks on 148 CTAs);
+// g.MT then counts 64-row tiles.  Not combined with SCREEN (the plan is per 128-row tile).
+template <bool SCREEN, bool HALF>
 __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
+    static_assert(!(SCREEN && HALF), "screening plans are per 128-row tile");
+    constexpr int BM = HALF ? 64 : 128, TM = BM / 16;
     extern __shared__ __align__(128) unsigned char mo_smem_raw[];
     double* stages = reinterpret_cast<double*>(mo_smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(stages + (size_t)MO_STAGES * (MO_A_STAGE + MO_B_STAGE));
@@ -128,7 +133,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
 
     const long total = SCREEN ? (long)g.plan_pre[g.MT] : (long)g.MT * g.NT * g.KB;
     const long it0 = total * blockIdx.x / gridDim.x, it1 = total * (blockIdx.x + 1) / gridDim.x;
-    constexpr uint32_t STAGE_BYTES = (MO_A_STAGE + MO_B_STAGE) * 8;
+    constexpr uint32_t A_BYTES = BM * MO_ALD * 8, STAGE_BYTES = A_BYTES + MO_B_STAGE * 8;
 
     if (warp == MO_CONSUMER_WARPS) {
         // ===== producer: one thread streams the stages of this CTA's iteration range =====
@@ -142,7 +147,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
                 const int tm = L.tm, tn = L.tn, kb = SCREEN ? g.plan_kb[(long)tm * g.KB + L.i] : L.i;
                 double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
                 mbar_expect_tx(&full[s], STAGE_BYTES);
-                bulk_g2s(As, g.PhiT + ((long)tm * g.KB + kb) * MO_A_STAGE, MO_A_STAGE * 8, &full[s]);
+                bulk_g2s(As, g.PhiT + ((long)(HALF ? tm >> 1 : tm) * g.KB + kb) * MO_A_STAGE + (HALF ? (tm & 1) * BM * MO_ALD : 0), A_BYTES, &full[s]);
                 bulk_g2s(As + MO_A_STAGE, g.CT + ((long)tn * g.KB + kb) * MO_B_STAGE, MO_B_STAGE * 8, &full[s]);
             }
         }
@@ -150,7 +155,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
     }
 
     // ===== consumers =====
-    const int wm0 = (warp >> 2) * 64, wn0 = (warp & 3) * 32;
+    const int wm0 = (warp >> 2) * (BM / 2), wn0 = (warp & 3) * 32;
     const int lr = lane >> 2, lc = lane & 3;
     uint32_t n = 0;
     long it = it0;
@@ -160,9 +165,9 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
         const long rem = it1 - it;
         const int kb_end = (rem < (long)(KBt - ka)) ? (int)(ka + rem) : KBt;
         const int tm = L.tm, tn = L.tn;
-        double acc[MO_TM][MO_TN][2];
+        double acc[TM][MO_TN][2];
 #pragma unroll
-        for (int i = 0; i < MO_TM; i++)
+        for (int i = 0; i < TM; i++)
 #pragma unroll
             for (int j = 0; j < MO_TN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
         for (int kb = ka; kb < kb_end; kb++, n++) {
@@ -172,13 +177,13 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
             const double* Bs = As + MO_A_STAGE;
 #pragma unroll
             for (int kk = 0; kk < MO_BK / 4; kk++) {
-                double af[MO_TM], bf[MO_TN];
+                double af[TM], bf[MO_TN];
 #pragma unroll
-                for (int i = 0; i < MO_TM; i++) af[i] = As[(wm0 + i * 8 + lr) * MO_ALD + kk * 4 + lc];
+                for (int i = 0; i < TM; i++) af[i] = As[(wm0 + i * 8 + lr) * MO_ALD + kk * 4 + lc];
 #pragma unroll
                 for (int j = 0; j < MO_TN; j++) bf[j] = Bs[(kk * 4 + lc) * MO_BLD + wn0 + j * 8 + lr];
 #pragma unroll
-                for (int i = 0; i < MO_TM; i++)
+                for (int i = 0; i < TM; i++)
 #pragma unroll
                     for (int j = 0; j < MO_TN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
             }
@@ -193,7 +198,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
             // park the partial tile for the owner (CTA with the tile's first k-block), then publish
             double* ws = g.ws + (size_t)blockIdx.x * MO_WS_DOUBLES;
 #pragma unroll
-            for (int i = 0; i < MO_TM; i++)
+            for (int i = 0; i < TM; i++)
 #pragma unroll
                 for (int j = 0; j < MO_TN; j++) {
                     ws[((i * MO_TN + j) * 2 + 0) * 256 + tid] = acc[i][j][0];
@@ -223,7 +228,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
                         consumer_bar();
                         const double* ws = g.ws + (size_t)peer * MO_WS_DOUBLES;
 #pragma unroll
-                        for (int i = 0; i < MO_TM; i++)
+                        for (int i = 0; i < TM; i++)
 #pragma unroll
                             for (int j = 0; j < MO_TN; j++) {
                                 acc[i][j][0] += __ldcg(ws + ((i * MO_TN + j) * 2 + 0) * 256 + tid);
@@ -234,9 +239,9 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
                     peer++;
                 }
             }
-            const int m0 = tm * MO_BM, n0 = tn * MO_BN;
+            const int m0 = tm * BM, n0 = tn * MO_BN;
 #pragma unroll
-            for (int i = 0; i < MO_TM; i++) {
+            for (int i = 0; i < TM; i++) {
                 const int row = m0 + wm0 + i * 8 + lr;
 #pragma unroll
                 for (int j = 0; j < MO_TN; j++) {

@@ -195,8 +195,9 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
                       int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st) {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -207,8 +208,12 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
     g.ws = ws; g.flags = flags; g.epoch = epoch;
     g.plan_cnt = plan ? plan->plan_cnt : nullptr; g.plan_pre = plan ? plan->plan_pre : nullptr; g.plan_kb = plan ? plan->plan_kb : nullptr;
     if (grid < 1) return cudaSuccess;
-    if (plan) k_mo_streamk<true><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
-    else k_mo_streamk<false><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
+    // few iterations per CTA: 64-row tiles, so that a tile is split over fewer CTAs and the partial sums are smaller
+    const bool half = !plan && (long)g.MT * g.NT * g.KB < 16L * grid;
+    if (half) g.MT = (rows + 63) / 64;
+    if (plan) k_mo_streamk<true, false><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
+    else if (half) k_mo_streamk<false, true><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
+    else k_mo_streamk<false, false><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
