@@ -330,10 +330,10 @@ def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None):
 
 
 def test_config2_full_crowd_sampled_walkers():
-    # 256-water config exactly as bench.py runs it (256 walkers, tau 0.005, delay_k 64), one sweep; 6 sampled
-    # walkers against the oracle.  |E_L| ~ 1e4 Ha here: 1e-9 Ha absolute is 1e-13 relative, at the FP64 floor
+    # 256-water config exactly as bench.py runs it (256 walkers, tau 0.005, delay_k 64), two sweeps (64 flushes, E_L
+    # after a sweep that started from flushed inverses); 6 sampled walkers against the oracle.  |E_L| ~ 1e4 Ha here: 1e-9 Ha absolute is 1e-13 relative, at the FP64 floor
     # of a 2048-term sum, so E_L is held to 1e-9 relative to the kinetic/potential scale (reading A26).
-    worst = _full_size_sampled(2, [0, 1, 100, 127, 200, 255], 1)
+    worst = _full_size_sampled(2, [0, 1, 100, 127, 200, 255], 2)
     assert worst["ratio"] < 10 * TOL_RATIO, worst      # cond(A) up to ~1e6 at N_s = 1024 (A26)
     assert worst["pos"] < TOL_POS, worst
     assert worst["eloc"] < 1e-6, worst
