@@ -209,7 +209,8 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
     g.plan_cnt = plan ? plan->plan_cnt : nullptr; g.plan_pre = plan ? plan->plan_pre : nullptr; g.plan_kb = plan ? plan->plan_kb : nullptr;
     if (grid < 1) return cudaSuccess;
     // few iterations per CTA: 64-row tiles, so that a tile is split over fewer CTAs and the partial sums are smaller
-    const bool half = !plan && (long)g.MT * g.NT * g.KB < 16L * grid;
+    // ... or when the last 128-row tile would be at least half padding (config 3: 320 rows = five 64-row tiles, not three of 128)
+    const bool half = !plan && ((long)g.MT * g.NT * g.KB < 16L * grid || g.MT * MO_BM - rows >= 64);
     if (half) g.MT = (rows + 63) / 64;
     if (plan) k_mo_streamk<true, false><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
     else if (half) k_mo_streamk<false, true><<<grid, MO_THREADS, MO_SMEM_BYTES, st>>>(g);
