@@ -93,6 +93,7 @@ def _lib(long_double: bool = False):
                                                  C.c_double, C.c_double, _dp, _dp, _dp, _u8p]
     lib.oracle_walker_sweep_limited.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                                 C.c_double, _u8p, _dp, _dp, _dp]
+    lib.oracle_walker_dlogpsi_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
     lib.oracle_drift_limiter_scale.restype = C.c_double
     lib.oracle_drift_limiter_scale.argtypes = [C.c_double, C.c_double, C.c_double]
     lib.oracle_delayed_update.restype = C.c_int
@@ -177,6 +178,7 @@ class OracleSystem:
         s = system
         self.n_basis, self.n_up, self.n_dn = s.n_basis, s.n_up, s.n_dn
         self.n_elec = s.n_up + s.n_dn
+        self.n_atoms = s.n_atoms
         self._keep = [_f64(s.atoms_xyz), _f64(s.Z), _i32(s.shell_atom), _i32(s.shell_l), _i32(s.shell_nprim),
                       _i32(s.shell_prim_offset), _f64(s.alpha), _f64(s.coef), _f64(s.C_up), _f64(s.C_dn)]
         k = self._keep
@@ -276,6 +278,12 @@ class OracleWalker:
         self.lib.oracle_walker_dmc_generation(self.sys.h, self.h, seed, walker_id, step, tau, lim_a, e_trial,
                                               C.byref(e), C.byref(w), C.byref(te), bits.ctypes.data_as(_u8p))
         return bits, e.value, w.value, te.value
+
+    def dlogpsi_dR(self):
+        """d ln|Psi| / d R_a for every atom, [n_atoms][3] (row f2, first half; the paper's eq. 3 with lambda = R_a)."""
+        out = np.zeros((self.sys.n_atoms, 3))
+        self.lib.oracle_walker_dlogpsi_dR(self.sys.h, self.h, _d(out))
+        return out
 
     def eloc(self):
         e = C.c_double()

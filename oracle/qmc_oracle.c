@@ -778,6 +778,46 @@ double oracle_sherman_morrison(int n, double *Ainv_d, int p, const double *v_d) 
     return (double)rho;
 }
 
+/* ------------------------------------------------------------------ row f2 (first half): d ln|Psi| / d R_a
+ * The paper's eq. (3) with lambda = a nuclear coordinate:  d ln D / d R_a = tr(A^-1 dA/dR_a).
+ * A basis function centred on atom a depends on r - R_a only, so dPhi_l/dR_a = -grad Phi_l for l on a and 0 otherwise:
+ *   (dA/dR_a,d)[p][j] = - sum_{l on a} C[l][j] d_d Phi_l(r_p),
+ *   d ln D / d R_a,d   = - sum_p sum_j Ainv[j][p] sum_{l on a} C[l][j] d_d Phi_l(r_p)        (both spins added),
+ * plus the Jastrow, where only the electron-nucleus term knows R_a:  dJ/dR_a = - sum_i u_en'(r_ia) (r_i - R_a)/r_ia.
+ * This is the wave-function ("Pulay") term of a QMC force estimator; the derivative of E_L itself (eq. 4) is not built.
+ * out[n_atoms][3].  Plain loops in the order written; a test pins it to finite differences of log|Psi| under a
+ * displacement of the nucleus together with its basis functions. */
+void oracle_walker_dlogpsi_dR(const oracle_system *s, const oracle_walker *w, double *out) {
+    int nb = s->n_basis;
+    real *phi = (real *)malloc((size_t)5 * nb * sizeof(real));
+    real *acc = (real *)calloc((size_t)3 * s->n_atoms, sizeof(real));
+    for (int sp = 0; sp < 2; sp++) {
+        int ns = sp == 0 ? s->n_up : s->n_dn, e0 = sp == 0 ? 0 : s->n_up;
+        const real *Ainv = w->Ainv[sp];
+        for (int p = 0; p < ns; p++) {
+            basis_eval(s, w->R + 3 * (e0 + p), phi, phi + nb, phi + 4 * nb); /* phi | grad [3][nb] | lap */
+            int f = 0;
+            for (int sh = 0; sh < s->n_shells; sh++) {
+                int a = s->sh_atom[sh], nf = 2 * s->sh_l[sh] + 1;
+                for (int m = 0; m < nf; m++, f++) {
+                    real cm = 0; /* (C A^-1)[l][p] = sum_j C[l][j] Ainv[j][p] */
+                    for (int j = 0; j < ns; j++) cm += s->C[sp][(size_t)f * ns + j] * Ainv[(size_t)j * ns + p];
+                    for (int d = 0; d < 3; d++) acc[3 * a + d] -= phi[(size_t)(1 + d) * nb + f] * cm;
+                }
+            }
+        }
+    }
+    for (int i = 0; i < w->ne; i++)
+        for (int a = 0; a < s->n_atoms; a++) {
+            real dx = w->R[3 * i] - s->xyz[3 * a], dy = w->R[3 * i + 1] - s->xyz[3 * a + 1], dz = w->R[3 * i + 2] - s->xyz[3 * a + 2];
+            real r = R_SQRT(dx * dx + dy * dy + dz * dz);
+            real du = pade_du(-s->Z[a], s->b_en, r);
+            acc[3 * a] -= du * dx / r; acc[3 * a + 1] -= du * dy / r; acc[3 * a + 2] -= du * dz / r;
+        }
+    for (int k = 0; k < 3 * s->n_atoms; k++) out[k] = (double)acc[k];
+    free(phi); free(acc);
+}
+
 /* from-scratch log|Psi| and sign at the walker's current positions (pin for the running value) */
 int oracle_walker_logpsi_scratch(const oracle_system *s, const oracle_walker *w, double *logabs, int *sign) {
     real lad_tot = 0; int sg_tot = 1;
