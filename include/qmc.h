@@ -161,6 +161,13 @@ int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff);
  * synchronises the stream. */
 int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed);
 
+/* ---- Row f2, first half: out[W][n_atoms][3] = d ln|Psi| / d R_a at the current configuration -- the paper's eq. (3)
+ * (d ln D / d lambda = tr(A^-1 dA/d lambda)) with the nuclear coordinates as parameters, basis functions
+ * moving with their nucleus, plus the electron-nucleus Jastrow term.  This is the wave-function ("Pulay") term of a QMC
+ * force estimator; the derivative of E_L (eq. 4) is not built.  out: host or device.  Call between sweeps; allocates and
+ * frees a [W][N_s][N_b] scratch (12.9 GB at config 2) and synchronises the stream.  QMC_ERR_NOMEM if that does not fit. */
+int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out);
+
 /* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
  * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
 int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);

@@ -25,7 +25,7 @@ EXPORTED = [
     "qmc_get_Ainv", "qmc_get_logpsi", "qmc_get_eloc", "qmc_get_accept_log", "qmc_get_ratio_log", "qmc_get_stats",
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
-    "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work",
+    "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library(path: str | None = None):
     lib.qmc_dmc_step.argtypes = [vp, i, d, i, d, d]
     lib.qmc_get_weights.argtypes = [vp, vp, vp]
     lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
+    lib.qmc_get_dlogpsi_dR.argtypes = [vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
@@ -182,7 +183,9 @@ def qmc_init(atoms_xyz, Z, shell_atom, shell_l, shell_nprim, shell_prim_offset, 
     h = C.c_void_p()
     sp = _stream_ptr(stream)
     _check(lib.qmc_init(C.byref(h), C.byref(at), C.byref(ba), C.byref(mo), C.byref(ja), sp))
-    return System(h, n_basis, n_up, n_dn, stream)
+    sysh = System(h, n_basis, n_up, n_dn, stream)
+    sysh.n_atoms = len(keep[1])
+    return sysh
 
 
 def qmc_init_from(system, stream=None) -> System:
@@ -234,6 +237,14 @@ def qmc_get_weights(walkers: Walkers, out=None, out_tau_eff=None):
     out_tau_eff = _out((walkers.n_walkers,), torch.float64, out_tau_eff)
     _check(load_library().qmc_get_weights(walkers.handle, _ptr(out), _ptr(out_tau_eff)))
     return out, out_tau_eff
+
+
+def qmc_get_dlogpsi_dR(walkers: Walkers, out=None):
+    """d ln|Psi| / d R_a, [W][n_atoms][3] (row f2, first half)."""
+    import torch
+    out = _out((walkers.n_walkers, walkers.system.n_atoms, 3), torch.float64, out)
+    _check(load_library().qmc_get_dlogpsi_dR(walkers.handle, _ptr(out)))
+    return out
 
 
 def qmc_get_mo_work(walkers: Walkers):

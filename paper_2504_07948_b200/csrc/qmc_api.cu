@@ -254,6 +254,22 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
         CUS(cudaMemcpyAsync(dfm, fmap.data(), fmap.size() * sizeof(int), cudaMemcpyHostToDevice, st));
         CUS(cudaStreamSynchronize(st));
         d.fmap = dfm;
+        // shells grouped by atom (row f2: d ln|Psi| / d R_a)
+        std::vector<int> aoff(atoms->n_atoms + 1, 0), alist(basis->n_shells);
+        for (int i = 0; i < basis->n_shells; i++) aoff[sh_atom[i] + 1]++;
+        for (int a = 0; a < atoms->n_atoms; a++) aoff[a + 1] += aoff[a];
+        {
+            std::vector<int> fill(aoff.begin(), aoff.end() - 1);
+            for (int i = 0; i < basis->n_shells; i++) alist[fill[sh_atom[i]]++] = i;
+        }
+        int *daoff, *dalist;
+        CUS(S->pool.alloc((void**)&daoff, aoff.size() * sizeof(int), st));
+        CUS(S->pool.alloc((void**)&dalist, alist.size() * sizeof(int) + 4, st));
+        CUS(cudaMemcpyAsync(daoff, aoff.data(), aoff.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+        CUS(cudaMemcpyAsync(dalist, alist.data(), alist.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+        CUS(cudaStreamSynchronize(st));
+        d.atom_shell_off = daoff;
+        d.atom_shell_list = dalist;
     }
     for (int sp = 0; sp < 2; sp++) {
         double* dC;
@@ -265,7 +281,11 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
             size_t bytes = (size_t)d.n_basis * d.ns[sp] * 8;
             CUS(cudaMalloc((void**)&tmp, bytes));
             cudaError_t e = cudaMemcpyAsync(tmp, src, bytes, cudaMemcpyDefault, st);
+            double* dCp = nullptr;  // plain copy in the internal function order, zero-padded to [nbp][nsp]
+            if (e == cudaSuccess) e = S->pool.alloc((void**)&dCp, (size_t)d.nbp * d.nsp[sp] * 8, st);
+            d.Cplain[sp] = dCp;
             if (e == cudaSuccess) e = launch_tile_C(tmp, d.n_basis, d.ns[sp], dC, d.kb, d.fmap, st);
+            if (e == cudaSuccess) e = launch_plain_C(tmp, d.n_basis, d.ns[sp], dCp, d.nsp[sp], d.fmap, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             cudaFree(tmp);
             CUS(e);
@@ -610,6 +630,25 @@ extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
     }
     if (e_mixed) CU(cudaMemcpyAsync(e_mixed, w->d_emixed, 8, cudaMemcpyDefault, st));
     CU(cudaStreamSynchronize(st));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out) {
+    if (!w || !out) return fail(QMC_ERR_ARG, "qmc_get_dlogpsi_dR: null argument");
+    const SysDev& s = w->sys->d;
+    const WalkDev& d = w->d;
+    cudaStream_t st = w->stream;
+    const size_t n_out = (size_t)d.W * s.n_atoms * 3;
+    double *Mt = nullptr, *acc = nullptr;
+    CU(cudaMalloc((void**)&Mt, (size_t)d.W * d.ldv * s.nbp * 8 + 16));
+    cudaError_t e = cudaMalloc((void**)&acc, n_out * 8 + 16);
+    if (e == cudaSuccess) e = cudaMemsetAsync(acc, 0, n_out * 8, st);
+    for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) e = launch_dlogpsi_dR(s, d, sp, Mt, acc, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, acc, n_out * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(Mt);
+    cudaFree(acc);
+    CU(e);
     return QMC_OK;
 }
 

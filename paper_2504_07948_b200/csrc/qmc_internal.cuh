@@ -43,6 +43,9 @@ struct SysDev {
     const int4* kb_counts;  // [kb]: number of s, p, d shells owning a function of k-block kb (32 functions), list offset
     const KbShell* kb_list; // shells of every k-block, grouped s | p | d (a shell may be in two blocks)
     const int* fmap;        // [n_basis] caller's function index -> internal one (shells grouped by reach, Morton-ordered)
+    const double* Cplain[2];   // [nbp][nsp] MO coefficients, internal function order, plain row-major (row f2: C A^-1)
+    const int* atom_shell_off; // [n_atoms + 1] shells of every atom in atom_shell_list
+    const int* atom_shell_list;
     const double* alpha;
     const double* coef;
     const double* CT[2];  // tiled, see mo_streamk.cuh

@@ -11,6 +11,7 @@
 #include "block_inverse.cuh"
 #include "dmc_kernels.cuh"
 #include "small_sweep.cuh"
+#include "force_kernels.cuh"
 
 #ifndef QMC_UPD_BM
 // flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
@@ -897,6 +898,34 @@ cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, u
     }
     k_sweep_small<<<(wd.W + wpb - 1) / wpb, wpb * 32, smem, st>>>(s, wd, a);
     COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// row f2, first half (force_kernels.cuh)
+cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st) {
+    long n = (long)nb * ns;
+    if (n == 0) return cudaSuccess;
+    k_plain_C<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in, nb, ns, Cp, nsp, fmap);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st) {
+    if (s.ns[spin] > 0) {
+        // Mt[w][p][f] = sum_j AinvT[w][p][j] C[f][j] = (C A^-1)[f][p]
+        GemmArgs g;
+        g.A = wd.AinvT[spin]; g.lda = s.nsp[spin]; g.strideA = (long)s.nsp[spin] * s.nsp[spin];
+        g.B = s.Cplain[spin]; g.ldb = s.nsp[spin]; g.strideB = 0;   // the same coefficients for every walker
+        g.C = Mt; g.ldc = s.nbp; g.strideC = (long)s.nsp[spin] * s.nbp;
+        g.M = s.nsp[spin]; g.N = s.nbp; g.K = s.nsp[spin];
+        cudaError_t e = gemm_f64_launch<CfgY128>(g, wd.W, EpiStore{}, st);
+        COUNT_LAUNCH();
+        if (e != cudaSuccess) return e;
+    }
+    if (s.ns[spin] > 0 || spin == 0) {
+        k_dlogpsi<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, spin, Mt, acc, spin == 0 ? 1 : 0);
+        COUNT_LAUNCH();
+    }
     return cudaGetLastError();
 }
 

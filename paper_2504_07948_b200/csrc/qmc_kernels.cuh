@@ -42,6 +42,9 @@ cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double*
 bool small_path_ok(const SysDev& s, const WalkDev& wd);
 cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
                                cudaStream_t st);
+cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st);
+// row f2 (first half): acc[W][n_atoms][3] += spin sp's part of d ln|Psi|/dR_a (+ the Jastrow part with spin 0); Mt: scratch [W][nsp][nbp]
+cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st);
 uint64_t launch_count();
 
 }  // namespace qmc
