@@ -274,6 +274,20 @@ def run_ours(args):
         f1 = dict(generation_ms=evs[0].elapsed_time(evs[1]), branch_ms=evs[1].elapsed_time(evs[2]),
                   walkers_copied=int((src.cpu().numpy() != np.arange(W)).sum()), e_trial=e_t, e_mixed=e_mixed, limiter_a=1.0,
                   what="qmc_dmc_step(1) = sweep with limited drift + weight update; qmc_branch = comb + copies of A^-1 and row caches")
+    # row f2, first half (outside the timed region): d ln|Psi| / d R_a of the whole crowd
+    f2 = None
+    if not args.no_dmc:
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        evs[0].record()
+        dl = qb.qmc_get_dlogpsi_dR(gw)
+        evs[1].record()
+        torch.cuda.synchronize()
+        msf = evs[0].elapsed_time(evs[1])
+        gemm_flop = 2.0 * W * sysm.n_basis * (sysm.n_up ** 2 + sysm.n_dn ** 2)
+        f2 = dict(ms=msf, gemm_tflops_lower_bound=gemm_flop / (msf * 1e-3) * 1e-12, max_abs=float(dl.abs().max()),
+                  what="qmc_get_dlogpsi_dR: (C A^-1)^T as one batched DMMA GEMM per spin (2 W N_b N_s^2 flop each) + per-atom contraction; "
+                       "time includes allocating and freeing the [W][N_s][N_b] scratch")
     qb.qmc_walkers_destroy(gw)
 
     # ---- the same K sweeps with the optional screening of the MO contraction (QMC_SCREEN_MO); NOT the headline value
@@ -379,6 +393,7 @@ def run_ours(args):
         stage_share={s: share[s] / tot_share for s in share},
         eloc_mean=red["e_sum"] / red["n_walkers"],
         f1_dmc=f1,
+        f2_dlogpsi_dR=f2,
         screened_mo=screened,
     )
     if world == 1 and not args.no_cpu_baseline:
