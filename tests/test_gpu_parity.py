@@ -388,3 +388,34 @@ def test_screened_contraction_equals_dense_config2():
     assert np.abs(a[2] - b[2]).max() < 1e-6          # E_L ~ 1e4 Ha: rounding-level agreement (reading A26)
     executed, dense = b[4]
     assert a[4] == (0, 0) and dense == 2048 * 3 * 8 * 192 and executed < 0.8 * dense
+
+
+# ------------------------------------------------------------------ the runs exactly as BASELINE.json states them
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_stated_run_keeps_its_state_consistent(cfg):
+    """configs[1] (512 walkers, 50 sweeps, delay 32), configs[2] (256 walkers, 10 sweeps, delay 64) and configs[3]
+    (64 walkers, 5 sweeps, delay 128) in full.  The oracle
+    cannot follow runs of this length (35 core-seconds per walker-sweep at config 2), so what is checked is what has a
+    plain definition at any length: after the last sweep the inverse carried through 1600 / 320 delayed flushes per walker,
+    the running log|Psi| and the local energy equal what a crowd created from scratch at the final positions gives."""
+    wl = qi.make_workload(cfg)
+    sysm = wl.system
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, wl.positions(), wl.seed)
+    qb.qmc_sweep(gw, wl.n_sweeps, wl.tau, wl.delay_k)
+    st = qb.qmc_get_stats(gw)
+    assert st["proposed"] == wl.n_walkers * sysm.n_elec * wl.n_sweeps and st["nonfinite"] == 0
+    assert 0.9 < st["accepted"] / st["proposed"] < 1.0
+    pos = qb.qmc_get_positions(gw)
+    fresh = qb.qmc_walkers_create(g, pos, wl.seed)
+    lp, sg = (x.cpu().numpy() for x in qb.qmc_get_logpsi(gw))
+    lp0, sg0 = (x.cpu().numpy() for x in qb.qmc_get_logpsi(fresh))
+    assert np.array_equal(sg, sg0)                                   # no walker crossed a node unnoticed
+    assert np.abs(lp - lp0).max() < 1e-8 * np.abs(lp0).max()
+    for spin in (0, 1):
+        a, b = qb.qmc_get_Ainv(gw, spin).cpu().numpy(), qb.qmc_get_Ainv(fresh, spin).cpu().numpy()
+        worst = max(rel_frob(a[n], b[n]) for n in range(0, wl.n_walkers, 7))
+        assert worst < 1e-7, worst                                   # rounding carried through the flushes, cond(A) up to ~1e6
+    e, e0 = qb.qmc_get_eloc(gw)[0].cpu().numpy(), qb.qmc_get_eloc(fresh)[0].cpu().numpy()
+    assert np.abs(e - e0).max() < 1e-6 * np.abs(e0).max()
