@@ -78,6 +78,7 @@ struct qmc_walkers {
     uint32_t step;       // global sweep counter (A12)
     uint32_t flags;
     int T_last;          // sweeps in the most recent qmc_sweep call
+    size_t log_capacity; // entries the log buffers can hold
     int* d_status;
     int* d_comb;        // [4 W + 1] reconfiguration scratch: source, pair_dst, pair_src, mult, n_pairs
     double* d_emixed;   // [1]
@@ -353,6 +354,7 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     w->step = first_step;
     w->flags = flags;
     w->T_last = 0;
+    w->log_capacity = 0;
     w->prof_stride = 0;
     memset(w->stage_ms, 0, sizeof(w->stage_ms));
     memset(w->stage_n, 0, sizeof(w->stage_n));
@@ -547,15 +549,20 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
         if (rc) return rc;
         CU(launch_window_reset(d, st));
     }
-    // accept / ratio logs of this call
-    CU(cudaStreamSynchronize(st));
-    w->logpool.free_all();
-    d.bits = nullptr; d.ratio_log = nullptr; d.pacc_log = nullptr;
+    // accept / ratio logs of this call: the buffers are kept from call to call and only grow, so that a loop of
+    // qmc_sweep calls of the same length never synchronises with the host
     const size_t nlog = (size_t)nsteps * s.ne * d.W;
-    CU(w->logpool.alloc((void**)&d.bits, nlog, st));
-    if (w->flags & QMC_LOG_RATIOS) {
-        CU(w->logpool.alloc((void**)&d.ratio_log, nlog * 8, st));
-        CU(w->logpool.alloc((void**)&d.pacc_log, nlog * 8, st));
+    if (nlog > w->log_capacity || !d.bits) {
+        CU(cudaStreamSynchronize(st));
+        w->logpool.free_all();
+        d.bits = nullptr; d.ratio_log = nullptr; d.pacc_log = nullptr;
+        w->log_capacity = 0;
+        CU(w->logpool.alloc((void**)&d.bits, nlog, st, false));
+        if (w->flags & QMC_LOG_RATIOS) {
+            CU(w->logpool.alloc((void**)&d.ratio_log, nlog * 8, st, false));
+            CU(w->logpool.alloc((void**)&d.pacc_log, nlog * 8, st, false));
+        }
+        w->log_capacity = nlog;
     }
     w->T_last = nsteps;
     if (!(w->flags & QMC_LARGE_PATH) && small_path_ok(s, d)) {  // row f4: the whole call in one launch
