@@ -419,3 +419,17 @@ def test_stated_run_keeps_its_state_consistent(cfg):
         assert worst < 1e-7, worst                                   # rounding carried through the flushes, cond(A) up to ~1e6
     e, e0 = qb.qmc_get_eloc(gw)[0].cpu().numpy(), qb.qmc_get_eloc(fresh)[0].cpu().numpy()
     assert np.abs(e - e0).max() < 1e-6 * np.abs(e0).max()
+
+
+# ------------------------------------------------------------------ ragged everything
+
+@pytest.mark.parametrize("n_water,W,k,flags", [(5, 33, 7, 2), (5, 33, 7, 0), (11, 19, 13, 0)])
+def test_odd_sizes_against_oracle(n_water, W, k, flags):
+    """Sizes that are multiples of nothing: 20 / 44 orbitals per spin (padded to 32 / 48), 120 / 264 basis functions (a
+    partial last k-block), 33 / 19 walkers (a partial row tile), delay ranks 7 / 13 (partial windows at the end of a spin
+    block).  5 waters qualify for the one-launch path (flags 0) and are also forced through the per-electron kernels
+    (flags 2 = QMC_LARGE_PATH); 11 waters (44 per spin) only run the latter."""
+    sysm = qi.water_cluster(n_water, qi.MASTER_SEED, cfg=1)
+    wl = qi.Workload(config=1, system=sysm, n_walkers=W, tau=0.01, n_sweeps=3, delay_k=k)
+    rep = run_and_compare(wl, range(W), 3, k, flags=qb.QMC_LOG_RATIOS | flags)
+    _assert_report(rep)
