@@ -93,6 +93,8 @@ def _lib(long_double: bool = False):
                                                  C.c_double, C.c_double, _dp, _dp, _dp, _u8p]
     lib.oracle_walker_sweep_limited.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                                 C.c_double, _u8p, _dp, _dp, _dp]
+    lib.oracle_walker_clone.restype = C.c_void_p
+    lib.oracle_walker_clone.argtypes = [C.c_void_p, C.c_void_p]
     lib.oracle_walker_dlogpsi_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
     lib.oracle_drift_limiter_scale.restype = C.c_double
     lib.oracle_drift_limiter_scale.argtypes = [C.c_double, C.c_double, C.c_double]
@@ -257,6 +259,13 @@ class OracleWalker:
                                            bits.ctypes.data_as(_u8p), _d(ratio), _d(pacc))
         return bits, ratio, pacc
 
+    def clone(self):
+        """Deep copy (what a DMC reconfiguration does to a walker that gets copies)."""
+        c = object.__new__(OracleWalker)
+        c.sys, c.lib = self.sys, self.lib
+        c.h = self.lib.oracle_walker_clone(self.sys.h, self.h)
+        return c
+
     def sweep_limited(self, seed, walker_id, step, tau, lim_a):
         """A sweep with the drift limiter of row f1; returns (bits, ratio, pacc, dr2[accepted, proposed])."""
         ne = self.sys.n_elec
@@ -369,6 +378,46 @@ def comb_reconfigure(weights, xi):
     for d, e in zip(dead, extra):
         source[d] = e
     return source, mult, tot / W
+
+
+def dmc_run(osys, walkers, seed, walker_ids, first_step, n_generations, tau, lim_a, e_trial0, branch_every, feedback,
+            e_start=None, weights=None):
+    """A DMC run with population control (row f1, reading A32), as the loop it is:
+        for every generation g: every walker does dmc_generation with the current E_T;
+        if branch_every > 0 and (g + 1) % branch_every == 0:
+            e_mixed = sum w E_L / sum w; comb reconfiguration with the uniform of step first_step + g + 1 (walkers with
+            copies are cloned into the dead slots, every weight becomes the mean weight);
+            E_T <- e_mixed - feedback * ln(mean weight).
+    Random streams belong to slots (walker_ids[slot]).  Returns a dict: walkers (list, after the run), bits
+    [G][N_e][W], weights [W], eloc [W], e_trial_log [G] (the E_T in effect DURING generation g), e_mixed_log [G] (nan where
+    no reconfiguration happened), sources [G][W] (slot map of each reconfiguration, identity elsewhere)."""
+    W = len(walkers)
+    walkers = list(walkers)
+    e = np.array([w.eloc()[0] for w in walkers]) if e_start is None else np.array(e_start, float)
+    wt = np.ones(W) if weights is None else np.array(weights, float)
+    bits = np.zeros((n_generations, osys.n_elec, W), np.uint8)
+    et_log, em_log = np.zeros(n_generations), np.full(n_generations, np.nan)
+    sources = np.tile(np.arange(W), (n_generations, 1))
+    e_t = float(e_trial0)
+    for g in range(n_generations):
+        et_log[g] = e_t
+        for n in range(W):
+            b, e[n], wt[n], _ = walkers[n].dmc_generation(seed, int(walker_ids[n]), first_step + g, tau, lim_a, e_t, e[n], wt[n])
+            bits[g, :, n] = b
+        if branch_every > 0 and (g + 1) % branch_every == 0:
+            tot = 0.0
+            ew = 0.0
+            for n in range(W):
+                tot = tot + wt[n]
+                ew += wt[n] * e[n]
+            em_log[g] = ew / tot
+            src, mult, mean_w = comb_reconfigure(wt, comb_uniform(seed, first_step + g + 1))
+            new_walkers = [walkers[n] if src[n] == n else walkers[src[n]].clone() for n in range(W)]
+            walkers, e, wt = new_walkers, e[src].copy(), np.full(W, mean_w)
+            sources[g] = src
+            e_t = em_log[g] - feedback * np.log(mean_w)
+    return dict(walkers=walkers, bits=bits, weights=wt, eloc=e, e_trial_log=et_log, e_mixed_log=em_log, sources=sources,
+                e_trial=e_t)
 
 
 # ------------------------------------------------------------------ crowd driver (threads over walkers)

@@ -494,6 +494,28 @@ oracle_walker *oracle_walker_create(const oracle_system *s, const double *R) {
     return w;
 }
 
+/* deep copy of a walker (the copies a DMC reconfiguration makes, row f1) */
+oracle_walker *oracle_walker_clone(const oracle_system *s, const oracle_walker *w) {
+    oracle_walker *c = (oracle_walker *)calloc(1, sizeof(oracle_walker));
+    int nsm = s->n_up > s->n_dn ? s->n_up : s->n_dn;
+    c->ne = w->ne;
+    c->R = (real *)malloc((size_t)3 * w->ne * sizeof(real));
+    memcpy(c->R, w->R, (size_t)3 * w->ne * sizeof(real));
+    for (int sp = 0; sp < 2; sp++) {
+        int ns = sp == 0 ? s->n_up : s->n_dn;
+        c->Ainv[sp] = (real *)malloc(((size_t)ns * ns + 1) * sizeof(real));
+        c->orb[sp] = (real *)malloc(((size_t)ns * 5 * ns + 1) * sizeof(real));
+        memcpy(c->Ainv[sp], w->Ainv[sp], (size_t)ns * ns * sizeof(real));
+        memcpy(c->orb[sp], w->orb[sp], (size_t)ns * 5 * ns * sizeof(real));
+    }
+    c->logabs = w->logabs;
+    c->sign = w->sign;
+    c->scratch = (real *)malloc((size_t)5 * s->n_basis * sizeof(real));
+    c->row = (real *)malloc(((size_t)5 * nsm + 1) * sizeof(real));
+    c->tmp = (real *)malloc(((size_t)nsm + 1) * sizeof(real));
+    return c;
+}
+
 /* re-synchronise from externally supplied positions (comparison protocol) */
 int oracle_walker_set_positions(const oracle_system *s, oracle_walker *w, const double *R) {
     for (int i = 0; i < 3 * w->ne; i++) w->R[i] = (real)R[i];

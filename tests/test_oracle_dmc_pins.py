@@ -211,3 +211,88 @@ def test_comb_uniform_is_a_philox_word_pair():
     x = (int(out[0]) << 32) | int(out[1])
     assert xi == (2 * (x >> 12) + 1) / 2.0 ** 53 and 0.0 < xi < 1.0
     assert oracle.comb_uniform(7948, 12) != xi
+
+
+# ------------------------------------------------------------------ the run with population control (reading A32)
+
+def test_hydrogen_run_with_population_control_is_the_closed_form():
+    """E_L = -1/2 everywhere: the mixed estimator is -1/2 at every reconfiguration, every weight is
+    exp(tau (1/2 + E_T)) per accepted move, so the whole E_T trajectory follows from the accept record alone; the slot
+    maps are the brute-force comb's on those weights."""
+    osys = oracle.OracleSystem(qi.hydrogen_atom())
+    rng = np.random.default_rng(9)
+    W, G, every, fb, tau, seed = 16, 12, 3, 0.5, 0.08, 314
+    walkers = [osys.walker(rng.standard_normal((1, 3))) for _ in range(W)]
+    r = oracle.dmc_run(osys, walkers, seed, range(W), 5, G, tau, 1.0, -0.4, every, fb)
+    wt, e_t = np.ones(W), -0.4
+    n_branch = 0
+    for g in range(G):
+        assert r["e_trial_log"][g] == pytest.approx(e_t, rel=1e-12)
+        wt = wt * np.exp(tau * (r["bits"][g, 0] & 1) * (0.5 + e_t))
+        if (g + 1) % every == 0:
+            n_branch += 1
+            assert r["e_mixed_log"][g] == pytest.approx(-0.5, abs=1e-10)
+            mult = _comb_brute(wt, oracle.comb_uniform(seed, 5 + g + 1))
+            got = np.bincount(r["sources"][g], minlength=W)
+            assert list(got) == mult
+            mean = wt.mean()
+            e_t = -0.5 - fb * math.log(mean)
+            wt = np.full(W, mean)
+        else:
+            assert np.isnan(r["e_mixed_log"][g])
+            assert list(r["sources"][g]) == list(range(W))
+    assert n_branch == 4
+    np.testing.assert_allclose(r["weights"], wt, rtol=1e-9)
+    assert r["e_trial"] == pytest.approx(e_t, rel=1e-10)
+    assert 0.5 < np.mean(r["bits"] & 1) <= 1.0
+
+
+def test_run_clones_are_fresh_walkers_on_the_slot_streams():
+    """After a reconfiguration slot j continues from the positions of walker source[j] on slot j's own random stream:
+    redo the run with walkers rebuilt from positions alone (no clone) and compare decisions, positions and weights."""
+    wl = qi.make_workload(0)
+    osys = oracle.OracleSystem(wl.system)
+    W, G, every, fb, tau, lim = 6, 4, 2, 1.0, 0.02, 1.0
+    ids = [3, 4, 5, 6, 7, 8]
+    start = wl.positions(0, W)
+    r = oracle.dmc_run(osys, [osys.walker(p) for p in start], wl.seed, ids, 2, G, tau, lim, -17.0, every, fb)
+    # by hand
+    ws = [osys.walker(p) for p in start]
+    e = [w.eloc()[0] for w in ws]
+    wt = [1.0] * W
+    e_t = -17.0
+    some_copy = False
+    for g in range(G):
+        for n in range(W):
+            b, e[n], wt[n], _ = ws[n].dmc_generation(wl.seed, ids[n], 2 + g, tau, lim, e_t, e[n], wt[n])
+            assert np.array_equal(b & 1, r["bits"][g, :, n] & 1)
+        if (g + 1) % every == 0:
+            src = r["sources"][g]
+            some_copy |= any(src[n] != n for n in range(W))
+            em = sum(a * b for a, b in zip(wt, e)) / sum(wt)
+            assert r["e_mixed_log"][g] == pytest.approx(em, rel=1e-12)
+            pos = [ws[n].positions().copy() for n in range(W)]
+            ws = [osys.walker(pos[src[n]]) for n in range(W)]
+            e = [e[src[n]] for n in range(W)]
+            mean = sum(wt) / W
+            wt = [mean] * W
+            e_t = em - fb * math.log(mean)
+    assert some_copy
+    for n in range(W):
+        np.testing.assert_allclose(r["walkers"][n].positions(), ws[n].positions(), atol=1e-12)
+        assert r["walkers"][n].eloc()[0] == pytest.approx(ws[n].eloc()[0], abs=1e-8)
+    np.testing.assert_allclose(r["weights"], wt, rtol=1e-10)
+    assert r["e_trial"] == pytest.approx(e_t, rel=1e-12)
+
+
+def test_clone_is_independent_of_its_original():
+    wl = qi.make_workload(0)
+    osys = oracle.OracleSystem(wl.system)
+    a = osys.walker(wl.positions(0, 1)[0])
+    c = a.clone()
+    ref = a.positions().copy()
+    c.sweep(wl.seed, 0, 0, 0.05)
+    assert np.array_equal(a.positions(), ref) and not np.array_equal(c.positions(), ref)
+    b1 = a.sweep(wl.seed, 0, 0, 0.05)
+    assert np.array_equal(a.positions(), c.positions())
+    np.testing.assert_array_equal(a.Ainv(0), c.Ainv(0))
