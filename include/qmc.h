@@ -160,6 +160,19 @@ int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff);
  * NULL): sum w E_L / sum w before the reconfiguration.  Must be called between sweeps (the delay window is empty then);
  * synchronises the stream. */
 int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed);
+/* A DMC run with population control, the whole loop on the device (no host round trip between generations; DESIGN.md
+ * reading A32; "walkers ... branching", L279-302 the production runs):
+ *   E_T = e_trial0
+ *   for g = 0 .. n_generations-1:  one qmc_dmc_step generation with E_T
+ *       if branch_every > 0 and (g + 1) % branch_every == 0:
+ *           qmc_branch;  E_T <- e_mixed - feedback * ln(W_tot / W)      (W_tot / W: the weight every walker leaves with)
+ * e_trial_out (may be NULL): E_T after the run.  branch_log (may be NULL): [n_generations / branch_every][3] =
+ * {e_mixed, E_T after, W_tot / W} of every reconfiguration.  sources (int32, may be NULL): [n_generations /
+ * branch_every][W] slot maps as qmc_branch's.  All three host or device.  The accept / ratio logs cover all
+ * n_generations.  Synchronises the stream once, at the end.  Errors: as qmc_dmc_step; QMC_ERR_ARG if branch_every < 0
+ * or feedback / e_trial0 is not finite. */
+int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int delay_k, double e_trial0, double limiter_a, int branch_every,
+                double feedback, double* e_trial_out, double* branch_log, int32_t* sources);
 
 /* ---- Row f2, first half: out[W][n_atoms][3] = d ln|Psi| / d R_a at the current configuration -- the paper's eq. (3)
  * (d ln D / d lambda = tr(A^-1 dA/d lambda)) with the nuclear coordinates as parameters, basis functions

@@ -26,6 +26,7 @@ EXPORTED = [
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
+    "qmc_dmc_run",
 ]
 
 
@@ -91,6 +92,7 @@ def load_library(path: str | None = None):
     lib.qmc_get_weights.argtypes = [vp, vp, vp]
     lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
     lib.qmc_get_dlogpsi_dR.argtypes = [vp, vp]
+    lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
@@ -261,6 +263,20 @@ def qmc_branch(walkers: Walkers, out_source=None):
     e = C.c_double()
     _check(load_library().qmc_branch(walkers.handle, _ptr(out_source), C.byref(e)))
     return out_source, e.value
+
+
+def qmc_dmc_run(walkers: Walkers, n_generations, tau, delay_k, e_trial0, limiter_a=1.0, branch_every=1, feedback=1.0):
+    """DMC run with population control on the device; returns (e_trial after the run, branch_log [n_branch][3] float64
+    tensor = {e_mixed, E_T after, W_tot / W}, sources [n_branch][W] int32 tensor)."""
+    import torch
+    nb = int(n_generations) // int(branch_every) if branch_every > 0 else 0
+    log = torch.empty((nb, 3), dtype=torch.float64, device="cuda")
+    src = torch.empty((nb, walkers.n_walkers), dtype=torch.int32, device="cuda")
+    e = C.c_double()
+    _check(load_library().qmc_dmc_run(walkers.handle, int(n_generations), float(tau), int(delay_k), float(e_trial0), float(limiter_a),
+                                      int(branch_every), float(feedback), C.byref(e), _ptr(log) if nb else None, _ptr(src) if nb else None))
+    walkers.last_nsteps = int(n_generations)
+    return e.value, log, src
 
 
 def _out(shape, dtype, out, device="cuda"):

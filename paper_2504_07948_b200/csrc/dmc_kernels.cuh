@@ -21,12 +21,14 @@ __global__ void k_dmc_begin(WalkDev wd) {
     wd.dr2[2 * w + 1] = 0.0;
 }
 
-__global__ void k_dmc_weight(WalkDev wd, double tau, double e_trial) {
+// e_trial_dev != nullptr: the trial energy lives on the device (qmc_dmc_run: k_comb moves it between generations)
+__global__ void k_dmc_weight(WalkDev wd, double tau, double e_trial, const double* e_trial_dev) {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= wd.W) return;
     const double acc = wd.dr2[2 * w], all = wd.dr2[2 * w + 1];
     const double te = all > 0.0 ? tau * acc / all : tau;
     const double e_new = wd.eloc[w];
+    if (e_trial_dev) e_trial = *e_trial_dev;
     const double arg = -te * ((wd.eold[w] + e_new) / 2.0 - e_trial);
     wd.weight[w] *= exp(arg);
     wd.eold[w] = e_new;
@@ -42,6 +44,10 @@ struct CombOut {
     int* n_pairs;     // [1]
     double* e_mixed;  // [1] sum w E_L / sum w before the reconfiguration
     int* mult;        // [W] scratch: multiplicities
+    // population control of qmc_dmc_run (reading A32); all null / 0 for a plain qmc_branch
+    double* e_trial_dev;  // [1] E_T <- e_mixed - feedback ln(W_tot / W)
+    double feedback;
+    double* branch_log;   // [3] of this reconfiguration: e_mixed, the new E_T, W_tot / W
 };
 
 // One CTA; the sums and the walk over the teeth are sequential in index order on purpose (one definite result).
@@ -64,6 +70,11 @@ __global__ void __launch_bounds__(256) k_comb(WalkDev wd, CombOut o, uint32_t st
     for (int i = 0; i < W; i++) { tot = tot + wts[i]; ew += wts[i] * wd.eloc[i]; }
     o.e_mixed[0] = ew / tot;
     const double tooth = tot / (double)W;
+    if (o.e_trial_dev) {
+        const double et = ew / tot - o.feedback * log(tooth);
+        o.e_trial_dev[0] = et;
+        if (o.branch_log) { o.branch_log[0] = ew / tot; o.branch_log[1] = et; o.branch_log[2] = tooth; }
+    }
     int i = 0;
     double cum = wts[0];
     for (int j = 0; j < W; j++) {

@@ -533,7 +533,10 @@ extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t*
 // ------------------------------------------------------------------------------------------------ qmc_sweep
 
 // dmc != 0: every sweep is a DMC generation (row f1): limited drift, then the weight update after E_L
-static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a) {
+// e_trial_dev != nullptr: E_T is read from the device.  The accept / ratio logs of this call are steps log_t0 .. log_t0 +
+// nsteps - 1 of a log of log_T steps (log_T < 0: the call is the whole log).
+static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a,
+                      const double* e_trial_dev = nullptr, int log_t0 = 0, int log_T = -1) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
     if (nsteps < 0) return fail(QMC_ERR_ARG, "qmc_sweep: nsteps < 0");
     if (!(tau > 0.0) || !isfinite(tau)) return fail(QMC_ERR_ARG, "qmc_sweep: tau must be > 0");
@@ -551,7 +554,8 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
     }
     // accept / ratio logs of this call: the buffers are kept from call to call and only grow, so that a loop of
     // qmc_sweep calls of the same length never synchronises with the host
-    const size_t nlog = (size_t)nsteps * s.ne * d.W;
+    if (log_T < 0) log_T = nsteps;
+    const size_t nlog = (size_t)log_T * s.ne * d.W;
     if (nlog > w->log_capacity || !d.bits) {
         CU(cudaStreamSynchronize(st));
         w->logpool.free_all();
@@ -564,9 +568,13 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
         }
         w->log_capacity = nlog;
     }
-    w->T_last = nsteps;
+    w->T_last = log_T;
     if (!(w->flags & QMC_LARGE_PATH) && small_path_ok(s, d)) {  // row f4: the whole call in one launch
-        if (nsteps > 0) CU(launch_sweep_small(s, d, nsteps, w->step, tau, dmc, e_trial, st));
+        WalkDev dl = d;
+        const size_t off = (size_t)log_t0 * s.ne * d.W;
+        dl.bits += off;
+        if (dl.ratio_log) { dl.ratio_log += off; dl.pacc_log += off; }
+        if (nsteps > 0) CU(launch_sweep_small(s, dl, nsteps, w->step, tau, dmc, e_trial, e_trial_dev, st));
         w->step += (uint32_t)nsteps;
         return QMC_OK;
     }
@@ -577,7 +585,7 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
             int in_window = 0;
             for (int p = 0; p < ns; p++) {
                 const int e = e0 + p;
-                const long log_off = ((long)t * s.ne + e) * d.W;
+                const long log_off = ((long)(log_t0 + t) * s.ne + e) * d.W;
                 const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
                 const bool pf = w->prof_stride > 0;
                 if (in_window == 0) {  // first proposal of a window: nothing to fuse it with
@@ -615,7 +623,7 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
         prof_begin(w, 5, pf);
         CU(launch_eloc(s, d, st));
         prof_end(w, pf);
-        if (dmc) CU(launch_dmc_weight(d, tau, e_trial, st));
+        if (dmc) CU(launch_dmc_weight(d, tau, e_trial, e_trial_dev, st));
         w->step++;
         if (w->timer.used > 8192) prof_collect(w);
     }
@@ -631,12 +639,58 @@ extern "C" int qmc_dmc_step(qmc_walkers* w, int n_generations, double tau, int d
 extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_branch: null walkers");
     cudaStream_t st = w->stream;
-    CU(launch_branch(w->sys->d, w->d, w->d_comb, w->d_emixed, w->step, st));
+    CU(launch_branch(w->sys->d, w->d, w->d_comb, w->d_emixed, w->step, nullptr, 0.0, nullptr, st));
     if (source) {
         CU(cudaMemcpyAsync(source, w->d_comb, (size_t)w->d.W * 4, cudaMemcpyDefault, st));
     }
     if (e_mixed) CU(cudaMemcpyAsync(e_mixed, w->d_emixed, 8, cudaMemcpyDefault, st));
     CU(cudaStreamSynchronize(st));
+    return QMC_OK;
+}
+
+extern "C" int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int delay_k, double e_trial0, double limiter_a, int branch_every,
+                           double feedback, double* e_trial_out, double* branch_log, int32_t* sources) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_dmc_run: null walkers");
+    if (n_generations < 0 || branch_every < 0) return fail(QMC_ERR_ARG, "qmc_dmc_run: n_generations and branch_every must be >= 0");
+    if (!isfinite(e_trial0) || !isfinite(feedback)) return fail(QMC_ERR_ARG, "qmc_dmc_run: e_trial0 and feedback must be finite");
+    cudaStream_t st = w->stream;
+    const int W = w->d.W;
+    const int n_branch = branch_every > 0 ? n_generations / branch_every : 0;
+    // device side of the run: E_T, the log of the reconfigurations, their slot maps
+    double* dbuf = nullptr;
+    int* dsrc = nullptr;
+    CU(cudaMalloc((void**)&dbuf, (size_t)(1 + 3 * (n_branch > 0 ? n_branch : 1)) * 8));
+    if (sources && n_branch > 0) {
+        cudaError_t e = cudaMalloc((void**)&dsrc, (size_t)n_branch * W * 4);
+        if (e != cudaSuccess) { cudaFree(dbuf); CU(e); }
+    }
+    int rc = QMC_OK;
+    cudaError_t ce = cudaMemcpyAsync(dbuf, &e_trial0, 8, cudaMemcpyHostToDevice, st);
+    const int chunk = branch_every > 0 ? branch_every : (n_generations > 0 ? n_generations : 1);
+    int done = 0, nb = 0;
+    if (n_generations == 0 && ce == cudaSuccess) rc = sweep_impl(w, 0, tau, delay_k, 1, e_trial0, limiter_a, dbuf, 0, 0);
+    while (ce == cudaSuccess && rc == QMC_OK && done < n_generations) {
+        const int n = n_generations - done < chunk ? n_generations - done : chunk;
+        rc = sweep_impl(w, n, tau, delay_k, 1, e_trial0, limiter_a, dbuf, done, n_generations);
+        done += n;
+        if (rc != QMC_OK) break;
+        if (branch_every > 0 && n == chunk) {
+            ce = launch_branch(w->sys->d, w->d, w->d_comb, w->d_emixed, w->step, dbuf, feedback, dbuf + 1 + 3 * nb, st);
+            if (ce == cudaSuccess && dsrc) ce = cudaMemcpyAsync(dsrc + (size_t)nb * W, w->d_comb, (size_t)W * 4, cudaMemcpyDeviceToDevice, st);
+            nb++;
+        }
+    }
+    if (ce == cudaSuccess && rc == QMC_OK) {
+        if (e_trial_out) ce = cudaMemcpyAsync(e_trial_out, dbuf, 8, cudaMemcpyDefault, st);
+        if (ce == cudaSuccess && branch_log && n_branch > 0) ce = cudaMemcpyAsync(branch_log, dbuf + 1, (size_t)n_branch * 24, cudaMemcpyDefault, st);
+        if (ce == cudaSuccess && dsrc) ce = cudaMemcpyAsync(sources, dsrc, (size_t)n_branch * W * 4, cudaMemcpyDefault, st);
+    }
+    cudaError_t cs = cudaStreamSynchronize(st);
+    cudaFree(dbuf);
+    cudaFree(dsrc);
+    if (rc != QMC_OK) return rc;
+    CU(ce);
+    CU(cs);
     return QMC_OK;
 }
 

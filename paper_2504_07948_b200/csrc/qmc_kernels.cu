@@ -840,15 +840,17 @@ cudaError_t launch_dmc_begin(const WalkDev& wd, cudaStream_t st) {
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
-cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, cudaStream_t st) {
-    k_dmc_weight<<<(wd.W + 255) / 256, 256, 0, st>>>(wd, tau, e_trial);
+cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, const double* e_trial_dev, cudaStream_t st) {
+    k_dmc_weight<<<(wd.W + 255) / 256, 256, 0, st>>>(wd, tau, e_trial, e_trial_dev);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
-cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf /* [4 W + 1] */, double* e_mixed, uint32_t step, cudaStream_t st) {
+cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf /* [4 W + 1] */, double* e_mixed, uint32_t step, double* e_trial_dev,
+                          double feedback, double* branch_log, cudaStream_t st) {
     CombOut o;
     o.source = ibuf; o.pair_dst = ibuf + wd.W; o.pair_src = ibuf + 2 * wd.W; o.mult = ibuf + 3 * wd.W; o.n_pairs = ibuf + 4 * wd.W;
     o.e_mixed = e_mixed;
+    o.e_trial_dev = e_trial_dev; o.feedback = feedback; o.branch_log = branch_log;
     const size_t smem = (size_t)wd.W * 8 <= 40 * 1024 ? (size_t)wd.W * 8 : 0;
     k_comb<<<1, 256, smem, st>>>(wd, o, step);
     COUNT_LAUNCH();
@@ -878,9 +880,9 @@ bool small_path_ok(const SysDev& s, const WalkDev& wd) {
     return per_block + per_walker <= 200 * 1024;
 }
 cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
-                               cudaStream_t st) {
+                               const double* e_trial_dev, cudaStream_t st) {
     SmallArgs a;
-    a.nsteps = nsteps; a.step0 = step0; a.tau = tau; a.sqrt_tau = sqrt(tau); a.dmc = dmc; a.e_trial = e_trial;
+    a.nsteps = nsteps; a.step0 = step0; a.tau = tau; a.sqrt_tau = sqrt(tau); a.dmc = dmc; a.e_trial = e_trial; a.e_trial_dev = e_trial_dev;
     a.nsm = s.ns[0] > s.ns[1] ? s.ns[0] : s.ns[1];
     const size_t per_block = small_block_doubles(s, a.nsm) * 8, per_walker = small_walker_doubles(s, wd.nep, a.nsm) * 8;
     // warps per block: as many as fit in ~100 KB (two blocks per SM), at most 8, and no more than needed to give every SM a block

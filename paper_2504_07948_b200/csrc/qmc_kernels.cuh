@@ -37,11 +37,12 @@ cudaError_t launch_enn(const SysDev& s, double* out, cudaStream_t st);
 cudaError_t launch_dmma_peak(double* out, int grid, int threads, int iters, cudaStream_t st);
 cudaError_t launch_fill_double(double* p, int n, double v, cudaStream_t st);
 cudaError_t launch_dmc_begin(const WalkDev& wd, cudaStream_t st);
-cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, cudaStream_t st);
-cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double* e_mixed, uint32_t step, cudaStream_t st);
+cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, const double* e_trial_dev, cudaStream_t st);
+cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double* e_mixed, uint32_t step, double* e_trial_dev, double feedback,
+                          double* branch_log, cudaStream_t st);
 bool small_path_ok(const SysDev& s, const WalkDev& wd);
 cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
-                               cudaStream_t st);
+                               const double* e_trial_dev, cudaStream_t st);
 cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st);
 // row f2 (first half): acc[W][n_atoms][3] += spin sp's part of d ln|Psi|/dR_a (+ the Jastrow part with spin 0); Mt: scratch [W][nsp][nbp]
 cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st);

@@ -18,6 +18,7 @@ struct SmallArgs {
     double tau, sqrt_tau;
     int dmc;          // 1: DMC generation (weights), lim_a in wd.lim_a
     double e_trial;
+    const double* e_trial_dev;  // non-null: E_T is read from the device (qmc_dmc_run)
     int nsm;          // max(ns[0], ns[1])
     int wpb;          // warps (walkers) per block
 };
@@ -58,6 +59,7 @@ __global__ void __launch_bounds__(256) k_sweep_small(SysDev s, WalkDev wd, Small
         }
     }
     double logpsi = wd.logpsi[w], weight = wd.weight[w], e_old = wd.eloc[w];
+    const double e_trial = a.e_trial_dev ? *a.e_trial_dev : a.e_trial;
     unsigned long long n_acc = 0, n_tie = 0, n_nonf = 0;
     const uint32_t wid = wd.first_walker + (uint32_t)w;
     const uint32_t k0 = (uint32_t)(wd.seed & 0xFFFFFFFFull), k1 = (uint32_t)(wd.seed >> 32);
@@ -260,7 +262,7 @@ __global__ void __launch_bounds__(256) k_sweep_small(SysDev s, WalkDev wd, Small
         const double K = -0.5 * ksum, e_new = K + (psum + s.e_nn);
         if (a.dmc) {  // row f1: tau_eff and the branching weight (same expressions as k_dmc_weight)
             const double te = dr2_all > 0.0 ? tau * dr2_acc / dr2_all : tau;
-            const double arg = -te * ((e_old + e_new) / 2.0 - a.e_trial);
+            const double arg = -te * ((e_old + e_new) / 2.0 - e_trial);
             weight *= exp(arg);
             if (lane == 0) wd.tau_eff[w] = te;
         }

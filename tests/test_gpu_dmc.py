@@ -145,3 +145,84 @@ def test_branch_slot_map_copies_and_continuation():
     pos_after = qb.qmc_get_positions(gw).cpu().numpy()
     for d in copies:                                            # a copy and its donor have diverged (different streams)
         assert np.abs(pos_after[d] - pos_after[src[d]]).max() > 1e-6
+
+
+# ------------------------------------------------------------------ qmc_dmc_run: the loop with population control
+
+def test_hydrogen_run_closed_form_on_gpu():
+    sysm = qi.hydrogen_atom()
+    g = qb.qmc_init_from(sysm)
+    rng = np.random.default_rng(4)
+    W, G, every, fb, tau, seed, e_t0 = 64, 20, 4, 0.5, 0.08, 99, -0.4
+    gw = qb.qmc_walkers_create(g, rng.standard_normal((W, 1, 3)), seed)
+    e_t_end, log, src = qb.qmc_dmc_run(gw, G, tau, 1, e_t0, 1.0, every, fb)
+    log, src = log.cpu().numpy(), src.cpu().numpy()
+    bits = qb.qmc_get_accept_log(gw).cpu().numpy()            # [G][1][W]
+    assert bits.shape == (G, 1, W) and log.shape == (G // every, 3)
+    wt, e_t, nb = np.ones(W), e_t0, 0
+    for gen in range(G):
+        wt = wt * np.exp(tau * (bits[gen, 0] & 1) * (0.5 + e_t))
+        if (gen + 1) % every == 0:
+            assert log[nb, 0] == pytest.approx(-0.5, abs=1e-10)
+            s_o, _, mean = oracle.comb_reconfigure(wt, oracle.comb_uniform(seed, gen + 1))
+            assert np.array_equal(src[nb], s_o)
+            e_t = -0.5 - fb * math.log(mean)
+            assert log[nb, 1] == pytest.approx(e_t, rel=1e-10) and log[nb, 2] == pytest.approx(mean, rel=1e-10)
+            wt = np.full(W, mean)
+            nb += 1
+    assert e_t_end == pytest.approx(e_t, rel=1e-10)
+    np.testing.assert_allclose(qb.qmc_get_weights(gw)[0].cpu().numpy(), wt, rtol=1e-9)
+
+
+@pytest.mark.parametrize("flags,k,every", [(0, 1, 2), (2, 1, 2), (2, 4, 3), (0, 1, 0)])
+def test_dmc_run_matches_the_oracle_loop(flags, k, every):
+    wl = qi.make_workload(0)
+    sysm = wl.system
+    W, G, fb, tau, lim, e_t0 = 24, 6, 1.0, 3 * wl.tau, 1.0, -75.0
+    pos = wl.positions(0, W)
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, pos, wl.seed, flags=flags)
+    e_t_end, log, src = qb.qmc_dmc_run(gw, G, tau, k, e_t0, lim, every, fb)
+    log, src = log.cpu().numpy(), src.cpu().numpy()
+    osys = oracle.OracleSystem(sysm)
+    r = oracle.dmc_run(osys, [osys.walker(p) for p in pos], wl.seed, range(W), 0, G, tau, lim, e_t0, every, fb)
+    bits = qb.qmc_get_accept_log(gw).cpu().numpy()
+    diff = (bits & 1) != (r["bits"] & 1)
+    assert not np.any(diff), "accept/reject mismatch (a flagged tie would also end the comparison of a branching run)"
+    gens = [gi for gi in range(G) if every > 0 and (gi + 1) % every == 0]
+    assert len(gens) == log.shape[0] == src.shape[0]
+    for nb, gi in enumerate(gens):
+        assert np.array_equal(src[nb], r["sources"][gi])
+        assert log[nb, 0] == pytest.approx(r["e_mixed_log"][gi], abs=1e-8)
+        assert log[nb, 1] == pytest.approx(r["e_trial_log"][gi + 1] if gi + 1 < G else r["e_trial"], abs=1e-8)
+    if every:
+        assert any(np.any(s != np.arange(W)) for s in src), "test needs at least one copy"
+    assert e_t_end == pytest.approx(r["e_trial"], abs=1e-8)
+    np.testing.assert_allclose(qb.qmc_get_weights(gw)[0].cpu().numpy(), r["weights"], rtol=1e-9)
+    assert np.abs(qb.qmc_get_eloc(gw)[0].cpu().numpy() - r["eloc"]).max() < 1e-8
+    po = np.stack([w.positions() for w in r["walkers"]])
+    assert np.abs(qb.qmc_get_positions(gw).cpu().numpy() - po).max() < 1e-9
+    st = qb.qmc_get_stats(gw)
+    assert st["proposed"] == W * sysm.n_elec * G
+
+
+def test_dmc_run_equals_the_calls_it_replaces():
+    """qmc_dmc_run is qmc_dmc_step + qmc_branch + the E_T rule, minus the host round trips: bit for bit."""
+    wl = qi.make_workload(0)
+    W, G, every, fb, tau = 32, 6, 2, 0.7, 2 * wl.tau
+    pos = wl.positions(0, W)
+    g = qb.qmc_init_from(wl.system)
+    a = qb.qmc_walkers_create(g, pos, wl.seed, flags=2)
+    e_end, log, src = qb.qmc_dmc_run(a, G, tau, 3, -76.0, 1.0, every, fb)
+    b = qb.qmc_walkers_create(g, pos, wl.seed, flags=2)
+    e_t = -76.0
+    for gi in range(G):
+        qb.qmc_dmc_step(b, 1, tau, 3, e_t, 1.0)
+        if (gi + 1) % every == 0:
+            s, em = qb.qmc_branch(b)
+            mean = float(qb.qmc_get_weights(b)[0][0])
+            e_t = em - fb * math.log(mean)
+            assert np.array_equal(s.cpu().numpy(), src[(gi + 1) // every - 1].cpu().numpy())
+    assert e_end == pytest.approx(e_t, rel=1e-14)
+    assert np.array_equal(qb.qmc_get_positions(a).cpu().numpy(), qb.qmc_get_positions(b).cpu().numpy())
+    np.testing.assert_allclose(qb.qmc_get_weights(a)[0].cpu().numpy(), qb.qmc_get_weights(b)[0].cpu().numpy(), rtol=1e-13)
