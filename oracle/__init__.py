@@ -95,6 +95,8 @@ def _lib(long_double: bool = False):
                                                 C.c_double, _u8p, _dp, _dp, _dp]
     lib.oracle_walker_clone.restype = C.c_void_p
     lib.oracle_walker_clone.argtypes = [C.c_void_p, C.c_void_p]
+    lib.oracle_walker_deloc_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
+    lib.oracle_basis_eval_d3.argtypes = [C.c_void_p, _dp, _dp, _dp]
     lib.oracle_walker_dlogpsi_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
     lib.oracle_drift_limiter_scale.restype = C.c_double
     lib.oracle_drift_limiter_scale.argtypes = [C.c_double, C.c_double, C.c_double]
@@ -207,6 +209,14 @@ class OracleSystem:
         self.lib.oracle_basis_eval(self.h, _d(r), _d(phi), _d(grad), _d(lap))
         return phi, grad, lap
 
+    def basis_eval_d3(self, r):
+        """second derivatives [6][n_basis] (xx, yy, zz, xy, xz, yz) and gradient of the Laplacian [3][n_basis]"""
+        r = _f64(r)
+        hess = np.zeros((6, self.n_basis))
+        glap = np.zeros((3, self.n_basis))
+        self.lib.oracle_basis_eval_d3(self.h, _d(r), _d(hess), _d(glap))
+        return hess, glap
+
     def mo_rows(self, spin, r):
         r = _f64(r)
         out = np.zeros((5, self.ns(spin)))
@@ -292,6 +302,12 @@ class OracleWalker:
         """d ln|Psi| / d R_a for every atom, [n_atoms][3] (row f2, first half; the paper's eq. 3 with lambda = R_a)."""
         out = np.zeros((self.sys.n_atoms, 3))
         self.lib.oracle_walker_dlogpsi_dR(self.sys.h, self.h, _d(out))
+        return out
+
+    def deloc_dR(self):
+        """d E_L / d R_a for every atom, [n_atoms][3] (row f2, second half; the paper's eq. 4)."""
+        out = np.zeros((self.sys.n_atoms, 3))
+        self.lib.oracle_walker_deloc_dR(self.sys.h, self.h, _d(out))
         return out
 
     def eloc(self):

@@ -840,6 +840,204 @@ void oracle_walker_dlogpsi_dR(const oracle_system *s, const oracle_walker *w, do
     free(phi); free(acc);
 }
 
+/* ------------------------------------------------------------------ row f2 (second half): d E_L / d R_a, eq. (4)
+ * PAPER.md L177-181:  dE_L/dR_a = tr(A^-1 dB/dR_a - X dA/dR_a),  X = A^-1 B A^-1,  with (Filippi, Assaraf, Moroni 2016,
+ * the "complete mathematical framework" the paper names) B the matrix whose trace with A^-1 is the local energy.  For
+ * Psi = D_up D_dn exp(J) (reading A9):
+ *     E_L = sum_spin tr(A^-1 B) + sum_i c_i + V,
+ *     B[i][j] = -1/2 [ lap phi_j(r_i) + 2 gJ_i . grad phi_j(r_i) ],   c_i = -1/2 [ lap_i J + |gJ_i|^2 ],  gJ_i = grad_i J,
+ * so that, with the electrons held fixed, MO coefficients and Jastrow parameters constant and every basis function and
+ * electron-nucleus Jastrow term moving with its nucleus (reading A33),
+ *     dE_L/dR_a = sum_spin tr(A^-1 dB/dR_a - X dA/dR_a) + sum_i dc_i/dR_a + dV/dR_a .
+ * Pieces, d = x, y, z a component of R_a, x = r_i - R_a, r = |x|, u = u_en of atom a (u1, u2, u3 its derivatives):
+ *     dA[i][j]   = - sum_{l on a} C[l][j] d_d Phi_l(r_i)
+ *     dgJ_i,b    = - [ u2 x_d x_b / r^2 + u1 (delta_db / r - x_d x_b / r^3) ]                (= - d_d d_b u)
+ *     dB[i][j]   = -1/2 [ - sum_{l on a} C[l][j] ( d_d lap Phi_l + 2 sum_b gJ_i,b d_d d_b Phi_l )(r_i)
+ *                         + 2 sum_b dgJ_i,b d_b phi_j(r_i) ]
+ *     dc_i       = -1/2 [ - (u3 + 2 u2 / r - 2 u1 / r^2) x_d / r + 2 sum_b gJ_i,b dgJ_i,b ]
+ *     dV         = - Z_a sum_i x_d / r^3 - sum_{b != a} Z_a Z_b (R_a - R_b)_d / R_ab^3
+ * Every matrix is built explicitly and multiplied by plain triple loops, one (atom, direction) at a time.
+ * out[n_atoms][3].  Pinned by central finite differences of oracle_walker_eloc under a displacement of the nucleus. */
+
+/* second derivatives and the gradient of the Laplacian of every basis function:
+ *   Phi = S g(t):   d_a d_b Phi = g d_a d_b S + 2 g' (d_a S x_b + d_b S x_a + S delta_ab) + 4 g'' S x_a x_b
+ *   lap Phi = S h,  h = (4l+6) g' + 4 t g'':   d_a lap Phi = h d_a S + 2 h' S x_a,   h' = (4l+10) g'' + 4 t g'''
+ * hess [6][nb] in the order xx, yy, zz, xy, xz, yz;  glap [3][nb]. */
+static void basis_eval_d3(const oracle_system *s, const real r[3], real *hess, real *glap) {
+    int nb = s->n_basis;
+    int f = 0;
+    for (int sh = 0; sh < s->n_shells; sh++) {
+        int a = s->sh_atom[sh], l = s->sh_l[sh];
+        real x[3] = {r[0] - s->xyz[3 * a + 0], r[1] - s->xyz[3 * a + 1], r[2] - s->xyz[3 * a + 2]};
+        real t = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+        real g = 0, g1 = 0, g2 = 0, g3 = 0;
+        for (int p = 0; p < s->sh_nprim[sh]; p++) {
+            real al = s->alpha[s->sh_off[sh] + p];
+            real e = s->coef[s->sh_off[sh] + p] * R_EXP(-al * t);
+            g += e;
+            g1 -= al * e;
+            g2 += al * al * e;
+            g3 -= al * al * al * e;
+        }
+        int nf = 2 * l + 1;
+        real S[5], dS[5][3], ddS[5][6];
+        for (int m = 0; m < 5; m++) {
+            S[m] = 0;
+            for (int k = 0; k < 3; k++) dS[m][k] = 0;
+            for (int k = 0; k < 6; k++) ddS[m][k] = 0;
+        }
+        if (l == 0) {
+            S[0] = 1;
+        } else if (l == 1) {
+            for (int m = 0; m < 3; m++) { S[m] = x[m]; dS[m][m] = 1; }
+        } else {
+            S[0] = SQRT3 * x[0] * x[1];  dS[0][0] = SQRT3 * x[1]; dS[0][1] = SQRT3 * x[0];  ddS[0][3] = SQRT3;
+            S[1] = SQRT3 * x[1] * x[2];  dS[1][1] = SQRT3 * x[2]; dS[1][2] = SQRT3 * x[1];  ddS[1][5] = SQRT3;
+            S[2] = x[2] * x[2] - (real)0.5 * (x[0] * x[0] + x[1] * x[1]);
+            dS[2][0] = -x[0]; dS[2][1] = -x[1]; dS[2][2] = 2 * x[2];   ddS[2][0] = -1; ddS[2][1] = -1; ddS[2][2] = 2;
+            S[3] = SQRT3 * x[0] * x[2];  dS[3][0] = SQRT3 * x[2]; dS[3][2] = SQRT3 * x[0];  ddS[3][4] = SQRT3;
+            S[4] = (SQRT3 / 2) * (x[0] * x[0] - x[1] * x[1]);
+            dS[4][0] = SQRT3 * x[0]; dS[4][1] = -SQRT3 * x[1];         ddS[4][0] = SQRT3; ddS[4][1] = -SQRT3;
+        }
+        real h = (real)(4 * l + 6) * g1 + 4 * t * g2;
+        real h1 = (real)(4 * l + 10) * g2 + 4 * t * g3;
+        static const int pa[6] = {0, 1, 2, 0, 0, 1}, pb[6] = {0, 1, 2, 1, 2, 2};
+        for (int m = 0; m < nf; m++, f++) {
+            for (int k = 0; k < 6; k++) {
+                int ia = pa[k], ib = pb[k];
+                real v = g * ddS[m][k] + 2 * g1 * (dS[m][ia] * x[ib] + dS[m][ib] * x[ia]) + 4 * g2 * S[m] * x[ia] * x[ib];
+                if (ia == ib) v += 2 * g1 * S[m];
+                hess[(size_t)k * nb + f] = v;
+            }
+            for (int d = 0; d < 3; d++) glap[(size_t)d * nb + f] = h * dS[m][d] + 2 * h1 * S[m] * x[d];
+        }
+    }
+}
+
+void oracle_basis_eval_d3(const oracle_system *s, const double r[3], double *hess, double *glap) {
+    int nb = s->n_basis;
+    real rr[3] = {r[0], r[1], r[2]};
+    real *b = (real *)malloc((size_t)9 * nb * sizeof(real));
+    basis_eval_d3(s, rr, b, b + 6 * nb);
+    for (int i = 0; i < 6 * nb; i++) hess[i] = (double)b[i];
+    for (int i = 0; i < 3 * nb; i++) glap[i] = (double)b[6 * nb + i];
+    free(b);
+}
+
+static real pade_d3u(real a, real b, real r) { real q = 1 + b * r; return 6 * a * b * b / (q * q * q * q); }
+
+void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, double *out) {
+    int nb = s->n_basis, ne = w->ne, na = s->n_atoms;
+    static const int hidx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};
+    real *acc = (real *)calloc((size_t)3 * na, sizeof(real));
+    real *gJ = (real *)malloc((size_t)3 * ne * sizeof(real));
+    for (int i = 0; i < ne; i++) {
+        real v, lp;
+        jastrow_one(s, w->R, i, w->R + 3 * i, &v, gJ + 3 * i, &lp);
+    }
+    /* function -> atom */
+    int *f_atom = (int *)malloc((size_t)nb * sizeof(int));
+    for (int sh = 0, f = 0; sh < s->n_shells; sh++)
+        for (int m = 0; m < 2 * s->sh_l[sh] + 1; m++, f++) f_atom[f] = s->sh_atom[sh];
+    for (int sp = 0; sp < 2; sp++) {
+        int ns = sp == 0 ? s->n_up : s->n_dn, e0 = sp == 0 ? 0 : s->n_up;
+        if (ns == 0) continue;
+        const real *Ainv = w->Ainv[sp]; /* Ainv[j][i] */
+        const real *C = s->C[sp];
+        size_t nn = (size_t)ns * ns;
+        real *B = (real *)malloc(nn * sizeof(real)), *T = (real *)malloc(nn * sizeof(real)), *X = (real *)malloc(nn * sizeof(real));
+        real *dA = (real *)malloc(nn * sizeof(real)), *dB = (real *)malloc(nn * sizeof(real));
+        /* derivatives of the basis functions at every electron of this spin: [i][14][nb] = grad 0..2 | hess 3..8 | glap 9..11 | value 12 | lap 13 */
+        real *bas = (real *)malloc((size_t)ns * 14 * nb * sizeof(real));
+        for (int i = 0; i < ns; i++) {
+            real *bi = bas + (size_t)i * 14 * nb;
+            basis_eval(s, w->R + 3 * (e0 + i), bi + (size_t)12 * nb, bi, bi + (size_t)13 * nb);
+            basis_eval_d3(s, w->R + 3 * (e0 + i), bi + (size_t)3 * nb, bi + (size_t)9 * nb);
+        }
+        /* B[i][j] from the walker's orbital rows */
+        for (int i = 0; i < ns; i++) {
+            const real *o = w->orb[sp] + (size_t)i * 5 * ns;
+            const real *g = gJ + 3 * (e0 + i);
+            for (int j = 0; j < ns; j++)
+                B[(size_t)i * ns + j] = (real)-0.5 * (o[4 * ns + j] + 2 * (g[0] * o[ns + j] + g[1] * o[2 * ns + j] + g[2] * o[3 * ns + j]));
+        }
+        /* X = A^-1 B A^-1:  T[j][k] = sum_i Ainv[j][i] B[i][k];  X[j][i] = sum_k T[j][k] Ainv[k][i] */
+        for (int j = 0; j < ns; j++)
+            for (int k = 0; k < ns; k++) {
+                real a = 0;
+                for (int i = 0; i < ns; i++) a += Ainv[(size_t)j * ns + i] * B[(size_t)i * ns + k];
+                T[(size_t)j * ns + k] = a;
+            }
+        for (int j = 0; j < ns; j++)
+            for (int i = 0; i < ns; i++) {
+                real a = 0;
+                for (int k = 0; k < ns; k++) a += T[(size_t)j * ns + k] * Ainv[(size_t)k * ns + i];
+                X[(size_t)j * ns + i] = a;
+            }
+        for (int a = 0; a < na; a++)
+            for (int d = 0; d < 3; d++) {
+                for (int i = 0; i < ns; i++) {
+                    const real *bi = bas + (size_t)i * 14 * nb;
+                    const real *o = w->orb[sp] + (size_t)i * 5 * ns;
+                    const real *g = gJ + 3 * (e0 + i);
+                    const real *ri = w->R + 3 * (e0 + i);
+                    real x[3] = {ri[0] - s->xyz[3 * a], ri[1] - s->xyz[3 * a + 1], ri[2] - s->xyz[3 * a + 2]};
+                    real r = R_SQRT(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+                    real u1 = pade_du(-s->Z[a], s->b_en, r), u2 = pade_d2u(-s->Z[a], s->b_en, r);
+                    real dg[3];
+                    for (int b = 0; b < 3; b++) dg[b] = -(u2 * x[d] * x[b] / (r * r) + u1 * ((d == b ? 1 / r : 0) - x[d] * x[b] / (r * r * r)));
+                    for (int j = 0; j < ns; j++) {
+                        real sa = 0, sb = 0;
+                        for (int l = 0; l < nb; l++) {
+                            if (f_atom[l] != a) continue;
+                            real c = C[(size_t)l * ns + j];
+                            sa += c * bi[(size_t)d * nb + l];
+                            real hg = 0;
+                            for (int b = 0; b < 3; b++) hg += g[b] * bi[(size_t)(3 + hidx[d][b]) * nb + l];
+                            sb += c * (bi[(size_t)(9 + d) * nb + l] + 2 * hg);
+                        }
+                        real dgo = dg[0] * o[ns + j] + dg[1] * o[2 * ns + j] + dg[2] * o[3 * ns + j];
+                        dA[(size_t)i * ns + j] = -sa;
+                        dB[(size_t)i * ns + j] = (real)-0.5 * (-sb + 2 * dgo);
+                    }
+                }
+                real tr = 0;
+                for (int i = 0; i < ns; i++)
+                    for (int j = 0; j < ns; j++)
+                        tr += Ainv[(size_t)j * ns + i] * dB[(size_t)i * ns + j] - X[(size_t)j * ns + i] * dA[(size_t)i * ns + j];
+                acc[3 * a + d] += tr;
+            }
+        free(B); free(T); free(X); free(dA); free(dB); free(bas);
+    }
+    /* dc_i and dV */
+    for (int a = 0; a < na; a++)
+        for (int d = 0; d < 3; d++) {
+            real sum = 0;
+            for (int i = 0; i < ne; i++) {
+                const real *g = gJ + 3 * i;
+                real x[3] = {w->R[3 * i] - s->xyz[3 * a], w->R[3 * i + 1] - s->xyz[3 * a + 1], w->R[3 * i + 2] - s->xyz[3 * a + 2]};
+                real r = R_SQRT(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+                real u1 = pade_du(-s->Z[a], s->b_en, r), u2 = pade_d2u(-s->Z[a], s->b_en, r), u3 = pade_d3u(-s->Z[a], s->b_en, r);
+                real gdg = 0;
+                for (int b = 0; b < 3; b++) {
+                    real dgb = -(u2 * x[d] * x[b] / (r * r) + u1 * ((d == b ? 1 / r : 0) - x[d] * x[b] / (r * r * r)));
+                    gdg += g[b] * dgb;
+                }
+                sum += (real)-0.5 * (-(u3 + 2 * u2 / r - 2 * u1 / (r * r)) * x[d] / r + 2 * gdg);
+                sum -= s->Z[a] * x[d] / (r * r * r);
+            }
+            for (int b = 0; b < na; b++) {
+                if (b == a) continue;
+                real y[3] = {s->xyz[3 * a] - s->xyz[3 * b], s->xyz[3 * a + 1] - s->xyz[3 * b + 1], s->xyz[3 * a + 2] - s->xyz[3 * b + 2]};
+                real rr = R_SQRT(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+                sum -= s->Z[a] * s->Z[b] * y[d] / (rr * rr * rr);
+            }
+            acc[3 * a + d] += sum;
+        }
+    for (int k = 0; k < 3 * na; k++) out[k] = (double)acc[k];
+    free(acc); free(gJ); free(f_atom);
+}
+
 /* from-scratch log|Psi| and sign at the walker's current positions (pin for the running value) */
 int oracle_walker_logpsi_scratch(const oracle_system *s, const oracle_walker *w, double *logabs, int *sign) {
     real lad_tot = 0; int sg_tot = 1;
