@@ -288,6 +288,18 @@ def run_ours(args):
         f2 = dict(ms=msf, gemm_tflops_lower_bound=gemm_flop / (msf * 1e-3) * 1e-12, max_abs=float(dl.abs().max()),
                   what="qmc_get_dlogpsi_dR: (C A^-1)^T as one batched DMMA GEMM per spin (2 W N_b N_s^2 flop each) + per-atom contraction; "
                        "time includes allocating and freeing the [W][N_s][N_b] scratch")
+        # second half: d E_L / d R_a by eq. (4), together with the first half from the shared C A^-1
+        torch.cuda.synchronize()
+        evs[0].record()
+        de, dl2 = qb.qmc_get_deloc_dR(gw)
+        evs[1].record()
+        torch.cuda.synchronize()
+        msf2 = evs[0].elapsed_time(evs[1])
+        flop2 = sum(2 * 2.0 * W * sysm.n_basis * n ** 2 + 2 * 2.0 * W * n ** 3 for n in (sysm.n_up, sysm.n_dn))
+        f2["deloc_dR"] = dict(ms=msf2, gemm_tflops_lower_bound=flop2 / (msf2 * 1e-3) * 1e-12, max_abs=float(de.abs().max()),
+                              first_half_unchanged=bool(torch.equal(dl, dl2)),
+                              what="qmc_get_deloc_dR: eq. (4); per spin C A^-1 and C X (2 W N_b N_s^2 flop each), X = A^-1 B A^-1 "
+                                   "(2 x 2 W N_s^3), per-atom contraction with third derivatives of the basis functions; both halves returned")
     qb.qmc_walkers_destroy(gw)
 
     # ---- the same K sweeps with the optional screening of the MO contraction (QMC_SCREEN_MO); NOT the headline value

@@ -180,6 +180,16 @@ int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int delay_k, doub
  * force estimator; the derivative of E_L (eq. 4) is not built.  out: host or device.  Call between sweeps; allocates and
  * frees a [W][N_s][N_b] scratch (12.9 GB at config 2) and synchronises the stream.  QMC_ERR_NOMEM if that does not fit. */
 int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out);
+/* ---- Row f2, second half: deloc[W][n_atoms][3] = d E_L / d R_a at the current configuration by the paper's eq. (4)
+ * (PAPER.md L177-181): tr(A^-1 dB/dR_a - X dA/dR_a), X = A^-1 B A^-1, summed over both spins, plus the derivative of the
+ * Jastrow and potential terms of E_L that are not inside the trace (reading A33).  Electrons fixed; basis
+ * functions and electron-nucleus Jastrow terms move with their nucleus; MO coefficients and Jastrow parameters constant
+ * (no orbital relaxation, no space warp).  dlogpsi (may be NULL): the same call also returns qmc_get_dlogpsi_dR's
+ * result from the shared C A^-1 product -- the two pieces of the force estimator
+ * F_a = -< dE_L/dR_a + 2 (E_L - <E_L>) d ln|Psi|/dR_a >.  deloc, dlogpsi: host or device.  Call between sweeps;
+ * allocates and frees 2 [W][N_s][N_b] + 4 [W][N_s^2] doubles of scratch and synchronises the stream.
+ * QMC_ERR_NOMEM if that does not fit. */
+int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi);
 
 /* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
  * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */

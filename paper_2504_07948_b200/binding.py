@@ -26,7 +26,7 @@ EXPORTED = [
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
-    "qmc_dmc_run",
+    "qmc_dmc_run", "qmc_get_deloc_dR",
 ]
 
 
@@ -92,6 +92,7 @@ def load_library(path: str | None = None):
     lib.qmc_get_weights.argtypes = [vp, vp, vp]
     lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
     lib.qmc_get_dlogpsi_dR.argtypes = [vp, vp]
+    lib.qmc_get_deloc_dR.argtypes = [vp, vp, vp]
     lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
@@ -247,6 +248,17 @@ def qmc_get_dlogpsi_dR(walkers: Walkers, out=None):
     out = _out((walkers.n_walkers, walkers.system.n_atoms, 3), torch.float64, out)
     _check(load_library().qmc_get_dlogpsi_dR(walkers.handle, _ptr(out)))
     return out
+
+
+def qmc_get_deloc_dR(walkers: Walkers, out=None, out_dlogpsi=None, with_dlogpsi=True):
+    """(d E_L / d R_a, d ln|Psi| / d R_a), each [W][n_atoms][3] (row f2; eqs. 3 and 4); the second is None if not asked for."""
+    import torch
+    shape = (walkers.n_walkers, walkers.system.n_atoms, 3)
+    out = _out(shape, torch.float64, out)
+    if with_dlogpsi:
+        out_dlogpsi = _out(shape, torch.float64, out_dlogpsi)
+    _check(load_library().qmc_get_deloc_dR(walkers.handle, _ptr(out), _ptr(out_dlogpsi) if with_dlogpsi else None))
+    return out, (out_dlogpsi if with_dlogpsi else None)
 
 
 def qmc_get_mo_work(walkers: Walkers):

@@ -713,6 +713,33 @@ extern "C" int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out) {
     return QMC_OK;
 }
 
+extern "C" int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi) {
+    if (!w || !deloc) return fail(QMC_ERR_ARG, "qmc_get_deloc_dR: null argument");
+    const SysDev& s = w->sys->d;
+    const WalkDev& d = w->d;
+    cudaStream_t st = w->stream;
+    const size_t W = (size_t)d.W, n_out = W * s.n_atoms * 3;
+    const size_t nsm = (size_t)(s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1]);
+    // one allocation: Mt, Nt [W][nsm][nbp] | Bm [2][W][nsm^2] | U, XT [W][nsm^2] | fg [W][ne][8] | acc_E, acc_psi
+    const size_t n_mt = W * nsm * s.nbp, n_sq = W * nsm * nsm, n_fg = W * s.ne * 8;
+    const size_t total = 2 * n_mt + 4 * n_sq + n_fg + 2 * n_out + 16;
+    double* buf = nullptr;
+    if (cudaMalloc((void**)&buf, total * 8) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(QMC_ERR_NOMEM, "qmc_get_deloc_dR: scratch does not fit");
+    }
+    double *Mt = buf, *Nt = Mt + n_mt, *Bm = Nt + n_mt, *U = Bm + 2 * n_sq, *XT = U + n_sq, *fg = XT + n_sq;
+    double *accE = fg + n_fg, *accP = accE + n_out;
+    cudaError_t e = cudaMemsetAsync(accE, 0, 2 * n_out * 8, st);
+    if (e == cudaSuccess) e = launch_forces(s, d, Mt, Nt, Bm, U, XT, fg, accE, dlogpsi ? accP : nullptr, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(deloc, accE, n_out * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess && dlogpsi) e = cudaMemcpyAsync(dlogpsi, accP, n_out * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(buf);
+    CU(e);
+    return QMC_OK;
+}
+
 extern "C" int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_get_mo_work: null walkers");
     unsigned long long h[2];

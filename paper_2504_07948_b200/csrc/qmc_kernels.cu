@@ -931,6 +931,62 @@ cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, doub
     return cudaGetLastError();
 }
 
+// Row f2, both halves.  Scratch (caller's): Mt, Nt [W][nsp_max][nbp]; Bm, U, XT [W][nsp_max^2]; fg [W][ne][8].
+// acc_E [W][n_atoms][3] += dE_L/dR_a;  acc_psi (may be null) += d ln|Psi|/dR_a.  Both zeroed by the caller.
+cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double* Nt, double* Bm, double* U, double* XT, double* fg,
+                          double* acc_E, double* acc_psi, cudaStream_t st) {
+    const long nsm = s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1];
+    cudaError_t e = cudaMemsetAsync(Bm, 0, (size_t)2 * wd.W * nsm * nsm * 8, st);   // both spins: [2][W][nsm^2]
+    if (e != cudaSuccess) return e;
+    double* Bsp[2] = {Bm, Bm + (long)wd.W * nsm * nsm};
+    k_force_prep<<<dim3((s.ne + 7) / 8, wd.W), 256, 0, st>>>(s, wd, fg, Bsp[0], Bsp[1]);
+    COUNT_LAUNCH();
+    for (int sp = 0; sp < 2; sp++) {
+        const int nsp = s.nsp[sp];
+        const long mat = (long)nsp * nsp;
+        if (s.ns[sp] > 0) {
+            GemmArgs g;
+            // Mt[w][p][f] = sum_j AinvT[w][p][j] C[f][j] = (C A^-1)[f][p]
+            g.A = wd.AinvT[sp]; g.lda = nsp; g.strideA = mat;
+            g.B = s.Cplain[sp]; g.ldb = nsp; g.strideB = 0;
+            g.C = Mt; g.ldc = s.nbp; g.strideC = (long)nsp * s.nbp;
+            g.M = nsp; g.N = s.nbp; g.K = nsp;
+            e = gemm_f64_launch<CfgY128>(g, wd.W, EpiStore{}, st);
+            COUNT_LAUNCH();
+            if (e != cudaSuccess) return e;
+            // U[p][i] = sum_k AinvT[p][k] B[i][k]
+            g.B = Bsp[sp]; g.ldb = nsp; g.strideB = mat;
+            g.C = U; g.ldc = nsp; g.strideC = mat;
+            g.N = nsp;
+            e = gemm_f64_launch<CfgY128>(g, wd.W, EpiStore{}, st);
+            COUNT_LAUNCH();
+            if (e != cudaSuccess) return e;
+            // XT[p][j] = sum_i U[p][i] AinvT[i][j] = X[j][p]
+            g.A = U; g.B = wd.AinvT[sp]; g.C = XT;
+            e = gemm_f64_launch<CfgUpd>(g, wd.W, EpiStore{}, st);
+            COUNT_LAUNCH();
+            if (e != cudaSuccess) return e;
+            // Nt[w][p][f] = sum_j XT[w][p][j] C[f][j] = (C X)[f][p]
+            g.A = XT;
+            g.B = s.Cplain[sp]; g.ldb = nsp; g.strideB = 0;
+            g.C = Nt; g.ldc = s.nbp; g.strideC = (long)nsp * s.nbp;
+            g.N = s.nbp;
+            e = gemm_f64_launch<CfgY128>(g, wd.W, EpiStore{}, st);
+            COUNT_LAUNCH();
+            if (e != cudaSuccess) return e;
+        }
+        if (s.ns[sp] > 0 || sp == 0) {
+            k_deloc<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, sp, Mt, Nt, fg, acc_E, sp == 0 ? 1 : 0);
+            COUNT_LAUNCH();
+            if (acc_psi) {
+                k_dlogpsi<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, sp, Mt, acc_psi, sp == 0 ? 1 : 0);
+                COUNT_LAUNCH();
+            }
+        }
+    }
+    return cudaGetLastError();
+}
+
 uint64_t launch_count() { return g_launches; }
 
 }  // namespace qmc

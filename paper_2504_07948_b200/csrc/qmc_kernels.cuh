@@ -45,6 +45,8 @@ cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, u
                                const double* e_trial_dev, cudaStream_t st);
 cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st);
 // row f2 (first half): acc[W][n_atoms][3] += spin sp's part of d ln|Psi|/dR_a (+ the Jastrow part with spin 0); Mt: scratch [W][nsp][nbp]
+cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double* Nt, double* Bm, double* U, double* XT, double* fg,
+                          double* acc_E, double* acc_psi, cudaStream_t st);
 cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st);
 uint64_t launch_count();
 

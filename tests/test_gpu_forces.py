@@ -56,3 +56,73 @@ def test_dlogpsi_dR_host_output_and_sum_rule():
         lp = qb.qmc_get_logpsi(qb.qmc_walkers_create(g, pos + sh, wl.seed))[0].cpu().numpy()
         lm = qb.qmc_get_logpsi(qb.qmc_walkers_create(g, pos - sh, wl.seed))[0].cpu().numpy()
         np.testing.assert_allclose(got[:, d], -(lp - lm) / (2 * h), rtol=2e-6, atol=2e-7)
+
+
+# ------------------------------------------------------------------ second half: d E_L / d R_a (eq. 4)
+
+@pytest.mark.parametrize("cfg,W,T,k,flags", [(0, 20, 3, 1, 0), (0, 20, 3, 2, 2), (1, 4, 1, 32, 0), ("rand", 9, 2, 2, 2)])
+def test_deloc_dR_matches_oracle(cfg, W, T, k, flags):
+    if cfg == "rand":
+        sysm = qi.random_molecule(3, 4, 6, 6, seed=4)
+        pos = qi.initial_positions(sysm, 0, range(W))
+        seed, tau = 99, 0.01
+    else:
+        wl = qi.make_workload(cfg)
+        sysm, pos, seed, tau = wl.system, wl.positions(0, W), wl.seed, wl.tau
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, pos, seed, flags=flags)
+    qb.qmc_sweep(gw, T, tau, k)
+    de, dp = (x.cpu().numpy() for x in qb.qmc_get_deloc_dR(gw))
+    gpos = qb.qmc_get_positions(gw).cpu().numpy()
+    osys = oracle.OracleSystem(sysm)
+    assert de.shape == dp.shape == (W, sysm.n_atoms, 3)
+    alone = qb.qmc_get_dlogpsi_dR(gw).cpu().numpy()
+    assert np.array_equal(alone, dp)                     # the shared C A^-1 product gives the first half unchanged
+    for n in range(W):
+        ow = osys.walker(gpos[n])
+        ref = ow.deloc_dR()
+        # the trace terms carry cond(A) twice (X = A^-1 B A^-1): 1e-8 of the largest component
+        assert np.abs(de[n] - ref).max() < 1e-8 * max(1.0, np.abs(ref).max()), (n, np.abs(de[n] - ref).max(), np.abs(ref).max())
+        refp = ow.dlogpsi_dR()
+        assert np.abs(dp[n] - refp).max() < 1e-9 * max(1.0, np.abs(refp).max()), n
+
+
+def test_deloc_dR_is_the_finite_difference_of_the_gpu_local_energy():
+    """Independent of the oracle: displace one nucleus (a new system on the GPU) and difference the GPU's own E_L."""
+    import copy
+    wl = qi.make_workload(0)
+    sysm = wl.system
+    W = 6
+    pos = wl.positions(0, W)
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, pos, wl.seed)
+    de = qb.qmc_get_deloc_dR(gw, with_dlogpsi=False)[0].cpu().numpy()
+    h = 1e-5
+    for a in range(sysm.n_atoms):
+        for d in range(3):
+            e = []
+            for sgn in (+1, -1):
+                s2 = copy.copy(sysm)
+                xyz = np.array(sysm.atoms_xyz, dtype=np.float64, copy=True)
+                xyz[a, d] += sgn * h
+                s2.atoms_xyz = xyz
+                g2 = qb.qmc_init_from(s2)
+                e.append(qb.qmc_get_eloc(qb.qmc_walkers_create(g2, pos, wl.seed))[0].cpu().numpy())
+            np.testing.assert_allclose(de[:, a, d], (e[0] - e[1]) / (2 * h), rtol=5e-6, atol=5e-5)
+
+
+def test_deloc_dR_host_output_and_odd_sizes():
+    import torch
+    sysm = qi.random_molecule(5, 7, 11, 11, seed=21)
+    W = 7
+    pos = qi.initial_positions(sysm, 0, range(W))
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, pos, 5, flags=2)
+    qb.qmc_sweep(gw, 1, 0.01, 3)
+    out = torch.empty((W, sysm.n_atoms, 3), dtype=torch.float64)               # host buffer
+    de = qb.qmc_get_deloc_dR(gw, out=out, with_dlogpsi=False)[0].numpy()
+    gpos = qb.qmc_get_positions(gw).cpu().numpy()
+    osys = oracle.OracleSystem(sysm)
+    for n in range(W):
+        ref = osys.walker(gpos[n]).deloc_dR()
+        assert np.abs(de[n] - ref).max() < 1e-8 * max(1.0, np.abs(ref).max()), n
