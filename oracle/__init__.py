@@ -97,6 +97,10 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_clone.argtypes = [C.c_void_p, C.c_void_p]
     lib.oracle_walker_deloc_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
     lib.oracle_basis_eval_d3.argtypes = [C.c_void_p, _dp, _dp, _dp]
+    lib.oracle_walker_vnl.restype = C.c_double
+    lib.oracle_walker_vnl.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int, _ip, _ip, _dp, _dp, _dp,
+                                      C.c_int, _ip, _ip, _dp, _dp, _ip]
+    lib.oracle_quadrature_directions.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _dp]
     lib.oracle_walker_dlogpsi_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
     lib.oracle_drift_limiter_scale.restype = C.c_double
     lib.oracle_drift_limiter_scale.argtypes = [C.c_double, C.c_double, C.c_double]
@@ -310,6 +314,25 @@ class OracleWalker:
         self.lib.oracle_walker_deloc_dR(self.sys.h, self.h, _d(out))
         return out
 
+    def vnl(self, ecp, seed, walker_id, step, details=False):
+        """Non-local pseudopotential energy (row f3) with the quadrature rotations of (seed, walker_id, step).
+        ecp: qmc_inputs.Ecp.  details=True: also (pair_i, pair_I, pts [n][12][3], ratios [n][12])."""
+        ch_atom = np.ascontiguousarray(ecp.ch_atom, np.int32)
+        ch_l = np.ascontiguousarray(ecp.ch_l, np.int32)
+        beta, alpha, rcut = _f64(ecp.ch_beta), _f64(ecp.ch_alpha), _f64(ecp.rcut)
+        assert rcut.shape == (self.sys.n_atoms,)
+        cap = self.sys.n_elec * self.sys.n_atoms if details else 0
+        pi, pI = np.zeros(max(cap, 1), np.int32), np.zeros(max(cap, 1), np.int32)
+        pts, rat = np.zeros((max(cap, 1), 12, 3)), np.zeros((max(cap, 1), 12))
+        n = C.c_int()
+        v = self.lib.oracle_walker_vnl(self.sys.h, self.h, seed, walker_id, step, len(ch_l), ch_atom.ctypes.data_as(_ip),
+                                       ch_l.ctypes.data_as(_ip), _d(beta), _d(alpha), _d(rcut), cap, pi.ctypes.data_as(_ip),
+                                       pI.ctypes.data_as(_ip), _d(pts), _d(rat), C.byref(n))
+        if details:
+            k = n.value
+            return v, pi[:k].copy(), pI[:k].copy(), pts[:k].copy(), rat[:k].copy()
+        return v
+
     def eloc(self):
         e = C.c_double()
         k = C.c_double()
@@ -360,6 +383,13 @@ def comb_uniform(seed, step):
     out = philox4x32_10([0xFFFFFFFF, step & 0xFFFFFFFF, 0xFFFFFFFF, 3], [seed & 0xFFFFFFFF, seed >> 32])
     x = (int(out[0]) << 32) | int(out[1])
     return (2 * (x >> 12) + 1) * 2.0 ** -53
+
+
+def quadrature_directions(seed, walker_id, step, electron):
+    """the 12 rotated icosahedron directions [12][3] of one (walker, step, electron)"""
+    out = np.zeros((12, 3))
+    _lib().oracle_quadrature_directions(seed, walker_id, step, electron, _d(out))
+    return out
 
 
 def comb_reconfigure(weights, xi):

@@ -1038,6 +1038,110 @@ void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, doub
     free(acc); free(gJ); free(f_atom);
 }
 
+/* ------------------------------------------------------------------ row f3: non-local pseudopotential energy
+ * PAPER.md L129 ("ccECP pseudopotentials"), L180 ("the non-local pseudopotential contribution").  The paper prints no
+ * formula; this is the standard semi-local form evaluated by spherical quadrature (Fahy, Wang, Louie 1990; Mitas,
+ * Shirley, Ceperley 1991), reading A34 of DESIGN.md.  Atom I carries channels l with radial functions
+ * v_l(r) = beta_l exp(-alpha_l r^2), cut at rcut_I.  For every electron i with r = |r_i - R_I| < rcut_I,
+ *     (V_nl Psi / Psi)_iI = sum_l (2l+1) v_l(r) sum_q w_q P_l(cos th_q) Psi(.., r_q, ..) / Psi(.., r_i, ..),
+ *     r_q = R_I + r O_q,   cos th_q = O_q . (r_i - R_I) / r,
+ * O_q = Rot * (vertex q of the icosahedron), w_q = 1/12 (exact for spherical polynomials up to degree 5), Rot a
+ * uniformly random rotation drawn per (walker, step, electron) from Philox blocks 4 and 5.  The wave-function ratio
+ * is the determinant ratio (orbital values at r_q against column i of A^-1) times exp(J(r_q) - J(r_i)).
+ * V_nl = sum_i (ascending) sum_I (ascending) of that.  l <= 2. */
+
+/* vertex q = 4 c + 2 a + b  (c = 0,1,2; a, b in {0,1}):  coordinate c is 0, coordinate c+1 is (+/-) n, coordinate c+2 is (+/-) phi n,
+ * the first sign from a, the second from b (0: +, 1: -);  phi = (1 + sqrt 5)/2,  n = 1/sqrt(1 + phi^2) */
+static void icosahedron_vertex(int q, real v[3]) {
+    real phi = ((real)1 + R_SQRT((real)5)) / 2;
+    real n = 1 / R_SQRT(1 + phi * phi);
+    int c = q / 4, a = (q / 2) % 2, b = q % 2;
+    v[c] = 0;
+    v[(c + 1) % 3] = a ? -n : n;
+    v[(c + 2) % 3] = b ? -phi * n : phi * n;
+}
+
+/* uniformly random rotation (Shoemake 1992): three uniforms -> unit quaternion (x, y, z, w) -> matrix, row-major */
+static void quadrature_rotation(uint64_t seed, uint32_t walker, uint32_t step, uint32_t electron, real rot[9]) {
+    uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
+    uint32_t ctr[4] = {walker, step, electron, 4}, o[4];
+    oracle_philox4x32_10(ctr, key, o);
+    real u1 = (real)u01(o[0], o[1]), u2 = (real)u01(o[2], o[3]);
+    ctr[3] = 5; oracle_philox4x32_10(ctr, key, o);
+    real u3 = (real)u01(o[0], o[1]);
+    real a = R_SQRT(1 - u1), b = R_SQRT(u1);
+    real x = a * R_SIN(TWO_PI * u2), y = a * R_COS(TWO_PI * u2), z = b * R_SIN(TWO_PI * u3), w = b * R_COS(TWO_PI * u3);
+    rot[0] = 1 - 2 * (y * y + z * z); rot[1] = 2 * (x * y - z * w);     rot[2] = 2 * (x * z + y * w);
+    rot[3] = 2 * (x * y + z * w);     rot[4] = 1 - 2 * (x * x + z * z); rot[5] = 2 * (y * z - x * w);
+    rot[6] = 2 * (x * z - y * w);     rot[7] = 2 * (y * z + x * w);     rot[8] = 1 - 2 * (x * x + y * y);
+}
+
+void oracle_quadrature_directions(uint64_t seed, uint32_t walker, uint32_t step, uint32_t electron, double dirs[36]) {
+    real rot[9];
+    quadrature_rotation(seed, walker, step, electron, rot);
+    for (int q = 0; q < 12; q++) {
+        real v[3];
+        icosahedron_vertex(q, v);
+        for (int d = 0; d < 3; d++) dirs[3 * q + d] = (double)(rot[3 * d] * v[0] + rot[3 * d + 1] * v[1] + rot[3 * d + 2] * v[2]);
+    }
+}
+
+/* returns V_nl of the walker.  Optional outputs for the pins (may be NULL; at most max_pairs pairs are recorded, all are counted):
+ * pair_i, pair_I [max_pairs], pts [max_pairs][12][3], ratios [max_pairs][12], n_pairs. */
+double oracle_walker_vnl(const oracle_system *s, const oracle_walker *w, uint64_t seed, uint32_t walker_id, uint32_t step,
+                         int n_ch, const int *ch_atom, const int *ch_l, const double *ch_beta, const double *ch_alpha,
+                         const double *rcut, int max_pairs, int *pair_i, int *pair_I, double *pts, double *ratios, int *n_pairs) {
+    int ne = w->ne, np = 0;
+    real vnl = 0;
+    real *row = (real *)malloc((size_t)5 * (s->n_up > s->n_dn ? s->n_up : s->n_dn) * sizeof(real) + 8);
+    for (int i = 0; i < ne; i++) {
+        int sp = spin_of(s, i), ns = sp == 0 ? s->n_up : s->n_dn, p = sp == 0 ? i : i - s->n_up;
+        const real *ri = w->R + 3 * i;
+        real rot[9];
+        quadrature_rotation(seed, walker_id, step, (uint32_t)i, rot);
+        for (int I = 0; I < s->n_atoms; I++) {
+            real x[3] = {ri[0] - s->xyz[3 * I], ri[1] - s->xyz[3 * I + 1], ri[2] - s->xyz[3 * I + 2]};
+            real r = R_SQRT(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+            if (!(r < (real)rcut[I])) continue;
+            real vl[3] = {0, 0, 0};  /* (2l+1) v_l(r) */
+            int any = 0;
+            for (int c = 0; c < n_ch; c++)
+                if (ch_atom[c] == I) {
+                    vl[ch_l[c]] += (real)(2 * ch_l[c] + 1) * (real)ch_beta[c] * R_EXP(-(real)ch_alpha[c] * r * r);
+                    any = 1;
+                }
+            if (!any) continue;
+            real pair_sum = 0;
+            for (int q = 0; q < 12; q++) {
+                real v[3], o[3], rq[3];
+                icosahedron_vertex(q, v);
+                for (int d = 0; d < 3; d++) o[d] = rot[3 * d] * v[0] + rot[3 * d + 1] * v[1] + rot[3 * d + 2] * v[2];
+                for (int d = 0; d < 3; d++) rq[d] = s->xyz[3 * I + d] + r * o[d];
+                real c = (o[0] * x[0] + o[1] * x[1] + o[2] * x[2]) / r;
+                mo_rows(s, sp, rq, row, w->scratch);
+                real det = 0;
+                for (int j = 0; j < ns; j++) det += row[j] * w->Ainv[sp][(size_t)j * ns + p];
+                real rho = det * R_EXP(jastrow_delta(s, w->R, i, ri, rq));
+                real ang = vl[0] + vl[1] * c + vl[2] * ((real)1.5 * c * c - (real)0.5);
+                pair_sum += ang * rho / 12;
+                if (np < max_pairs) {
+                    if (pts) for (int d = 0; d < 3; d++) pts[((size_t)np * 12 + q) * 3 + d] = (double)rq[d];
+                    if (ratios) ratios[(size_t)np * 12 + q] = (double)rho;
+                }
+            }
+            if (np < max_pairs) {
+                if (pair_i) pair_i[np] = i;
+                if (pair_I) pair_I[np] = I;
+            }
+            np++;
+            vnl += pair_sum;
+        }
+    }
+    free(row);
+    if (n_pairs) *n_pairs = np;
+    return (double)vnl;
+}
+
 /* from-scratch log|Psi| and sign at the walker's current positions (pin for the running value) */
 int oracle_walker_logpsi_scratch(const oracle_system *s, const oracle_walker *w, double *logabs, int *sign) {
     real lad_tot = 0; int sg_tot = 1;

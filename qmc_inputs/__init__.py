@@ -348,3 +348,54 @@ def random_molecule(n_heavy: int, n_h: int, n_up: int, n_dn: int, seed: int, spr
     else:
         raise ValueError("random_molecule supports closed-shell or single-spin systems")
     return _assemble(f"rand{n_heavy}h{n_h}", cfg, seed, xyz, Z, is_h, e_atoms, n_up, n_dn)
+
+
+# ------------------------------------------------------------------ row f3: semi-local pseudopotential channels (data only)
+
+@dataclass
+class Ecp:
+    """Non-local channels of a semi-local pseudopotential: channel c sits on atom ch_atom[c], projects on angular
+    momentum ch_l[c] (0..2) and has the radial function ch_beta[c] * exp(-ch_alpha[c] r^2); atom I acts on electrons
+    closer than rcut[I] (0: the atom has no non-local part)."""
+
+    ch_atom: np.ndarray  # [n_ch] int32
+    ch_l: np.ndarray  # [n_ch] int32
+    ch_beta: np.ndarray  # [n_ch] float64 (hartree)
+    ch_alpha: np.ndarray  # [n_ch] float64 (bohr^-2)
+    rcut: np.ndarray  # [N_a] float64 (bohr)
+
+    @property
+    def n_channels(self) -> int:
+        return int(self.ch_l.shape[0])
+
+
+def make_ecp(system: System) -> Ecp:
+    """Synthetic stand-in for the paper's ccECPs (their tables are not reproduced): heavy atoms get an
+    s channel 12 exp(-8 r^2) and a p channel -4 exp(-6 r^2), cut at 1.4 bohr; hydrogens an s channel 2 exp(-10 r^2), cut
+    at 1.0 bohr.  The magnitudes, the one-Gaussian-per-channel shape and the 1-1.5 bohr range are those of first-row
+    ccECP-like potentials; about one to two electrons per heavy atom sit inside the cut-off."""
+    ch_atom, ch_l, beta, alpha = [], [], [], []
+    rcut = np.zeros(system.n_atoms)
+    for a in range(system.n_atoms):
+        if system.Z[a] > 1.5:
+            ch_atom += [a, a]; ch_l += [0, 1]; beta += [12.0, -4.0]; alpha += [8.0, 6.0]
+            rcut[a] = 1.4
+        else:
+            ch_atom += [a]; ch_l += [0]; beta += [2.0]; alpha += [10.0]
+            rcut[a] = 1.0
+    return Ecp(np.array(ch_atom, np.int32), np.array(ch_l, np.int32), np.array(beta), np.array(alpha), rcut)
+
+
+def one_orbital_atom(l: int, m: int, zeta: float = 0.7, b_en: float = 0.5) -> System:
+    """One up electron on one atom at the origin in the single orbital S_lm(r) exp(-zeta r^2) (one shell of angular
+    momentum l, C picks component m) with an electron-nucleus Jastrow: under a rotation about the nucleus the wave
+    function transforms like S_lm alone, which makes the non-local energy a closed form (tests of row f3)."""
+    nf = 2 * l + 1
+    C = np.zeros((nf, 1))
+    C[m, 0] = 1.0
+    return System(name=f"atom_l{l}m{m}", atoms_xyz=np.zeros((1, 3)), Z=np.array([1.0]),
+                  shell_atom=np.array([0], np.int32), shell_l=np.array([l], np.int32),
+                  shell_nprim=np.array([1], np.int32), shell_prim_offset=np.array([0], np.int32),
+                  alpha=np.array([zeta]), coef=np.array([1.0]), n_basis=nf, n_up=1, n_dn=0,
+                  C_up=C, C_dn=np.zeros((nf, 0)), a_anti=0.5, a_para=0.25, b_ee=1.0, b_en=b_en,
+                  electron_atom=np.array([0], np.int32))
