@@ -300,6 +300,24 @@ def run_ours(args):
                               first_half_unchanged=bool(torch.equal(dl, dl2)),
                               what="qmc_get_deloc_dR: eq. (4); per spin C A^-1 and C X (2 W N_b N_s^2 flop each), X = A^-1 B A^-1 "
                                    "(2 x 2 W N_s^3), per-atom contraction with third derivatives of the basis functions; both halves returned")
+    # row f3 (outside the timed region): non-local pseudopotential energy of the whole crowd
+    f3 = None
+    if not args.no_dmc:
+        qb.qmc_set_ecp(gsys, qi.make_ecp(sysm))
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        evs[0].record()
+        vnl, n_pairs = qb.qmc_get_vnl(gw)
+        evs[1].record()
+        torch.cuda.synchronize()
+        ms3 = evs[0].elapsed_time(evs[1])
+        npts = 12 * n_pairs
+        # pairs split between the spins like the electrons; flop of the values-only contraction
+        flop3 = 2.0 * npts * sysm.n_basis * (sysm.n_up + sysm.n_dn) / 2
+        f3 = dict(ms=ms3, pairs=int(n_pairs), pairs_per_walker=n_pairs / W, points=int(npts), contraction_tflops_lower_bound=flop3 / (ms3 * 1e-3) * 1e-12,
+                  points_per_s=npts / (ms3 * 1e-3), vnl_mean=float(vnl.mean()),
+                  what="qmc_get_vnl: 12-point rotated icosahedral quadrature around every (electron, atom) pair inside the cut-offs of "
+                       "qmc_inputs.make_ecp; points batched 5 W at a time through k_basis (values only) -> k_mo_streamk -> k_nl_ratio")
     qb.qmc_walkers_destroy(gw)
 
     # ---- the same K sweeps with the optional screening of the MO contraction (QMC_SCREEN_MO); NOT the headline value
@@ -406,6 +424,7 @@ def run_ours(args):
         eloc_mean=red["e_sum"] / red["n_walkers"],
         f1_dmc=f1,
         f2_dlogpsi_dR=f2,
+        f3_vnl=f3,
         screened_mo=screened,
     )
     if world == 1 and not args.no_cpu_baseline:

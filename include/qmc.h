@@ -191,6 +191,22 @@ int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out);
  * QMC_ERR_NOMEM if that does not fit. */
 int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi);
 
+/* ---- Row f3: non-local pseudopotential energy by spherical quadrature ("ccECP pseudopotentials", L180;
+ * DESIGN.md reading A34).  qmc_set_ecp attaches the non-local channels to a system: channel c sits on atom ch_atom[c],
+ * projects on angular momentum ch_l[c] (0..2), has the radial function ch_beta[c] exp(-ch_alpha[c] r^2); atom I acts on
+ * electrons closer than rcut[I] (n_atoms entries; 0 = none).  Arrays host or device, copied.  May be called again
+ * (replaces the table).  QMC_ERR_ARG on out-of-range entries. */
+int qmc_set_ecp(qmc_system* s, int n_channels, const int32_t* ch_atom, const int32_t* ch_l, const double* ch_beta,
+                const double* ch_alpha, const double* rcut);
+/* vnl[W] (host or device) = sum over electrons i and atoms I with |r_i - R_I| < rcut_I of
+ *     sum_q (1/12) [ sum_l (2l+1) v_l(r) P_l(cos th_q) ] Psi(.., r_q, ..) / Psi(.., r_i, ..),   r_q = R_I + r O_q,
+ * O_q the 12 icosahedron vertices under a uniform random rotation drawn per (walker, sweep counter, electron) from Philox
+ * blocks 4 and 5 (three uniforms -> unit quaternion), cos th_q = O_q . (r_i - R_I)/r; the ratio is the determinant ratio
+ * (orbital values at r_q against the electron's row of A^-T) times exp(J(r_q) - J(r_i)).  Not part of qmc_get_eloc's E_L:
+ * the caller adds it.  n_pairs (may be NULL): (electron, atom) pairs inside the cut-offs, all walkers.  Call between
+ * sweeps; synchronises the stream (the number of pairs is read back once per spin).  QMC_ERR_ARG without qmc_set_ecp. */
+int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs);
+
 /* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
  * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
 int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);

@@ -26,7 +26,7 @@ EXPORTED = [
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
-    "qmc_dmc_run", "qmc_get_deloc_dR",
+    "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl",
 ]
 
 
@@ -93,6 +93,8 @@ def load_library(path: str | None = None):
     lib.qmc_branch.argtypes = [vp, vp, C.POINTER(d)]
     lib.qmc_get_dlogpsi_dR.argtypes = [vp, vp]
     lib.qmc_get_deloc_dR.argtypes = [vp, vp, vp]
+    lib.qmc_set_ecp.argtypes = [vp, i, vp, vp, vp, vp, vp]
+    lib.qmc_get_vnl.argtypes = [vp, vp, C.POINTER(u64)]
     lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
@@ -259,6 +261,27 @@ def qmc_get_deloc_dR(walkers: Walkers, out=None, out_dlogpsi=None, with_dlogpsi=
         out_dlogpsi = _out(shape, torch.float64, out_dlogpsi)
     _check(load_library().qmc_get_deloc_dR(walkers.handle, _ptr(out), _ptr(out_dlogpsi) if with_dlogpsi else None))
     return out, (out_dlogpsi if with_dlogpsi else None)
+
+
+def qmc_set_ecp(system: System, ecp):
+    """Attach the non-local pseudopotential channels (qmc_inputs.Ecp) to a system (row f3)."""
+    import numpy as np
+    ch_atom = np.ascontiguousarray(ecp.ch_atom, np.int32)
+    ch_l = np.ascontiguousarray(ecp.ch_l, np.int32)
+    beta = np.ascontiguousarray(ecp.ch_beta, np.float64)
+    alpha = np.ascontiguousarray(ecp.ch_alpha, np.float64)
+    rcut = np.ascontiguousarray(ecp.rcut, np.float64)
+    _check(load_library().qmc_set_ecp(system.handle, len(ch_l), ch_atom.ctypes.data, ch_l.ctypes.data, beta.ctypes.data,
+                                      alpha.ctypes.data, rcut.ctypes.data))
+
+
+def qmc_get_vnl(walkers: Walkers, out=None):
+    """(V_nl [W] tensor, number of (electron, atom) pairs inside the cut-offs) at the current configuration (row f3)."""
+    import torch
+    out = _out((walkers.n_walkers,), torch.float64, out)
+    n = C.c_uint64()
+    _check(load_library().qmc_get_vnl(walkers.handle, _ptr(out), C.byref(n)))
+    return out, n.value
 
 
 def qmc_get_mo_work(walkers: Walkers):

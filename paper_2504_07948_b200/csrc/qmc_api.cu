@@ -740,6 +740,105 @@ extern "C" int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi) 
     return QMC_OK;
 }
 
+extern "C" int qmc_set_ecp(qmc_system* S, int n_channels, const int32_t* ch_atom, const int32_t* ch_l, const double* ch_beta,
+                           const double* ch_alpha, const double* rcut) {
+    if (!S) return fail(QMC_ERR_ARG, "qmc_set_ecp: null system");
+    if (n_channels < 0 || (n_channels > 0 && (!ch_atom || !ch_l || !ch_beta || !ch_alpha)) || !rcut) return fail(QMC_ERR_ARG, "qmc_set_ecp: null argument");
+    const int na = S->d.n_atoms;
+    std::vector<int> atom, l;
+    std::vector<double> beta, alpha, rc;
+    CU(fetch(atom, ch_atom, (size_t)n_channels));
+    CU(fetch(l, ch_l, (size_t)n_channels));
+    CU(fetch(beta, ch_beta, (size_t)n_channels));
+    CU(fetch(alpha, ch_alpha, (size_t)n_channels));
+    CU(fetch(rc, rcut, (size_t)na));
+    for (int c = 0; c < n_channels; c++) {
+        if (atom[c] < 0 || atom[c] >= na || l[c] < 0 || l[c] > 2) return fail(QMC_ERR_ARG, "qmc_set_ecp: channel atom out of range or l not in 0..2");
+        if (!isfinite(beta[c]) || !(alpha[c] >= 0.0) || !isfinite(alpha[c])) return fail(QMC_ERR_ARG, "qmc_set_ecp: beta must be finite and alpha >= 0");
+    }
+    for (int a = 0; a < na; a++)
+        if (!(rc[a] >= 0.0) || !isfinite(rc[a])) return fail(QMC_ERR_ARG, "qmc_set_ecp: rcut must be finite and >= 0");
+    // channels grouped by atom, the caller's order kept inside an atom
+    std::vector<int> off(na + 1, 0), gl((size_t)n_channels);
+    std::vector<double> gb((size_t)n_channels), ga((size_t)n_channels);
+    for (int c = 0; c < n_channels; c++) off[atom[c] + 1]++;
+    for (int a = 0; a < na; a++) off[a + 1] += off[a];
+    std::vector<int> pos(off.begin(), off.end() - 1);
+    for (int c = 0; c < n_channels; c++) {
+        const int k = pos[atom[c]]++;
+        gl[k] = l[c]; gb[k] = beta[c]; ga[k] = alpha[c];
+    }
+    cudaStream_t st = S->stream;
+    int *d_off = nullptr, *d_l = nullptr;
+    double *d_b = nullptr, *d_a = nullptr, *d_rc = nullptr;
+    CU(S->pool.alloc((void**)&d_off, (size_t)(na + 1) * 4, st));
+    CU(S->pool.alloc((void**)&d_l, (size_t)n_channels * 4, st));
+    CU(S->pool.alloc((void**)&d_b, (size_t)n_channels * 8, st));
+    CU(S->pool.alloc((void**)&d_a, (size_t)n_channels * 8, st));
+    CU(S->pool.alloc((void**)&d_rc, (size_t)na * 8, st));
+    CU(cudaMemcpyAsync(d_off, off.data(), (size_t)(na + 1) * 4, cudaMemcpyHostToDevice, st));
+    if (n_channels > 0) {
+        CU(cudaMemcpyAsync(d_l, gl.data(), (size_t)n_channels * 4, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_b, gb.data(), (size_t)n_channels * 8, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_a, ga.data(), (size_t)n_channels * 8, cudaMemcpyHostToDevice, st));
+    }
+    CU(cudaMemcpyAsync(d_rc, rc.data(), (size_t)na * 8, cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    // an earlier table stays allocated until qmc_finalize (walker sets may still be using it on their streams)
+    S->d.ecp_off = d_off; S->d.ecp_l = d_l; S->d.ecp_beta = d_b; S->d.ecp_alpha = d_a; S->d.ecp_rcut = d_rc;
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs_out) {
+    if (!w || !vnl) return fail(QMC_ERR_ARG, "qmc_get_vnl: null argument");
+    const SysDev& s = w->sys->d;
+    const WalkDev& d = w->d;
+    if (!s.ecp_off) return fail(QMC_ERR_ARG, "qmc_get_vnl: no pseudopotential set (qmc_set_ecp)");
+    cudaStream_t st = w->stream;
+    const size_t W = (size_t)d.W;
+    double* acc = nullptr;
+    CU(cudaMalloc((void**)&acc, W * 8 + 16));
+    cudaError_t e = cudaMemsetAsync(acc, 0, W * 8, st);
+    uint64_t total = 0;
+    for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) {
+        NlArgs a;
+        memset(&a, 0, sizeof(a));
+        a.spin = sp; a.e0 = sp == 0 ? 0 : s.ns[0]; a.ns = s.ns[sp]; a.step = w->step;
+        if (a.ns == 0) continue;
+        const size_t n = W * (size_t)a.ns;
+        e = cudaMalloc((void**)&a.cnt, (n + 1) * 4);
+        if (e != cudaSuccess) break;
+        int n_pairs = 0;
+        e = launch_nl_count(s, d, a, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&n_pairs, a.cnt + n, 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        int* ibuf = nullptr;
+        double* dbuf = nullptr;
+        if (e == cudaSuccess && n_pairs > 0) {
+            const size_t np = (size_t)n_pairs;
+            e = cudaMalloc((void**)&ibuf, 3 * np * 4);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&dbuf, np * 12 * 5 * 8);
+            if (e == cudaSuccess) {
+                a.pair_w = ibuf; a.pair_e = ibuf + np; a.pair_I = ibuf + 2 * np;
+                a.pts = dbuf; a.ang = dbuf + np * 36; a.terms = a.ang + np * 12;
+            }
+        }
+        if (e == cudaSuccess) e = launch_nl_evaluate(s, d, a, n_pairs, d.mo_grid, &w->mo_epoch, acc, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(a.cnt);
+        cudaFree(ibuf);
+        cudaFree(dbuf);
+        total += (uint64_t)n_pairs;
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(vnl, acc, W * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(acc);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return fail(QMC_ERR_NOMEM, "qmc_get_vnl: scratch does not fit"); }
+    CU(e);
+    if (n_pairs_out) *n_pairs_out = total;
+    return QMC_OK;
+}
+
 extern "C" int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_get_mo_work: null walkers");
     unsigned long long h[2];

@@ -52,6 +52,12 @@ struct SysDev {
     int nt[2];            // 128-column tiles per spin
     double a_anti, a_para, b_ee, b_en;
     double e_nn;  // nuclear repulsion
+    // row f3 (qmc_set_ecp; all null until then): channels grouped by atom, ecp_off [n_atoms + 1]
+    const int* ecp_off;
+    const int* ecp_l;
+    const double* ecp_beta;
+    const double* ecp_alpha;
+    const double* ecp_rcut;  // [n_atoms]
 };
 
 struct WalkDev {
@@ -88,6 +94,19 @@ struct WalkDev {
     double* tilemax;
     int *plan_cnt, *plan_pre, *plan_kb;
     unsigned long long* mo_work;
+};
+
+// row f3 (nlpp_kernels.cuh): one spin of one qmc_get_vnl call
+struct NlArgs {
+    int spin, e0, ns;        // electrons e0 .. e0 + ns - 1
+    int* cnt;                // [W * ns + 1] pairs of (w, p); after the scan: offsets, cnt[W * ns] = total
+    int* pair_w;             // [n_pairs]
+    int* pair_e;             // global electron index
+    int* pair_I;
+    double* pts;             // [n_pairs * 12][3]
+    double* ang;             // [n_pairs * 12] sum_l (2l+1) v_l(r) P_l(cos th_q) / 12
+    double* terms;           // [n_pairs * 12] ang * ratio
+    uint32_t step;
 };
 
 }  // namespace qmc

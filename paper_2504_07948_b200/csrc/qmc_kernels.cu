@@ -12,6 +12,7 @@
 #include "dmc_kernels.cuh"
 #include "small_sweep.cuh"
 #include "force_kernels.cuh"
+#include "nlpp_kernels.cuh"
 
 #ifndef QMC_UPD_BM
 // flush update GEMM tile, measured on B200 at config 2 (k = 64): 64x64 CTA tile, 16x32 warp tiles, 3 stages = 2.50 ms per
@@ -45,39 +46,40 @@ __device__ __forceinline__ void bulk_s2g(void* gmem_dst, const void* smem_src, u
 }
 
 constexpr int BASIS_THREADS = 256;
-constexpr int BASIS_MAXPT = (MO_BM + 4) / 5 + 1;  // points that can touch one 128-row tile (27)
+// NC rows per point: 5 (value, gradient, Laplacian: the sweep) or 1 (values only: the quadrature points of row f3)
+template <int NC> constexpr int BASIS_MAXPT = (MO_BM + NC - 1) / NC + 1;  // points that can touch one 128-row tile (27 / 129)
 
 // Work items are (point, shell) pairs, ordered s-shells | p-shells | d-shells of the k-block, so a warp mixes
 // shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
 // stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
 // issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
-template <bool TMAX>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
+template <bool TMAX, int NC>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
 __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
                                                              double* __restrict__ tilemax) {
     __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
-    __shared__ double spt[3 * BASIS_MAXPT + 3];
+    __shared__ double spt[3 * BASIS_MAXPT<NC> + 3];
     __shared__ unsigned long long smax;  // bit pattern of a non-negative double: integer order = numeric order
     if (threadIdx.x == 0) smax = 0ull;
     double vmax = 0.0;
     const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
     const int row_lo = tm * MO_BM;
-    const int pt_lo = row_lo / 5;
-    int pt_hi = (row_lo + MO_BM + 4) / 5;
+    const int pt_lo = row_lo / NC;
+    int pt_hi = (row_lo + MO_BM + NC - 1) / NC;
     if (pt_hi > n_points) pt_hi = n_points;
     const int npt = pt_hi - pt_lo;
     const int f_lo = kb * MO_BK;
-    if (row_lo + MO_BM <= 5 * n_points && f_lo + MO_BK <= s.n_basis) {
+    if (row_lo + MO_BM <= NC * n_points && f_lo + MO_BK <= s.n_basis) {
         // every (row, function) of the tile gets written below: only the 4 padding columns need zeros
         for (int i = tid; i < MO_BM * 2; i += BASIS_THREADS)
             reinterpret_cast<double2*>(tile + (i >> 1) * MO_ALD + MO_BK)[i & 1] = make_double2(0.0, 0.0);
     } else {
         for (int i = tid; i < MO_A_STAGE / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
     }
-    if (tid < 3 * npt) spt[tid] = pts[3 * pt_lo + tid];
+    for (int i = tid; i < 3 * npt; i += BASIS_THREADS) spt[i] = pts[3 * pt_lo + i];
     __syncthreads();
     const int4 cnt = s.kb_counts[kb];  // x, y, z = number of s, p, d shells; w = offset of this block's list
     const KbShell* __restrict__ list = s.kb_list + cnt.w;
-    const int r_base = pt_lo * 5 - row_lo;
+    const int r_base = pt_lo * NC - row_lo;
     const int n0 = npt * cnt.x, n1 = n0 + npt * cnt.y, n2 = n1 + npt * cnt.z;
     for (int q = tid; q < n2; q += BASIS_THREADS) {
         int L, qq, c, base;
@@ -100,7 +102,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             g1 -= al * e;
             g2 += al * al * e;
         }
-        const int r0 = r_base + pi * 5;  // local row of the value component (may be < 0 or > 123)
+        const int r0 = r_base + pi * NC;  // local row of the value component (may be < 0 or > 123)
         const int c0 = rec.f0 - f_lo;
         const double lapfac = (double)(4 * L + 6) * g1 + 4.0 * t * g2;
         const double tg1 = 2.0 * g1;
@@ -109,7 +111,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
             if (col < 0 || col >= MO_BK) return;
             const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
-            for (int k = 0; k < 5; k++)
+            for (int k = 0; k < NC; k++)
                 if (r0 + k >= 0 && r0 + k < MO_BM) {
                     tile[(r0 + k) * MO_ALD + col] = v[k];
                     if (TMAX) vmax = fmax(vmax, v[k] == v[k] ? fabs(v[k]) : INFINITY);  // a NaN stage is never screened out
@@ -148,8 +150,16 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
     dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
-    if (tilemax) k_basis<true><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
-    else k_basis<false><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
+    if (tilemax) k_basis<true, 5><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
+    else k_basis<false, 5><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+// values only: row = point
+cudaError_t launch_basis_values(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
+    if (n_points == 0) return cudaSuccess;
+    dim3 grid(s.kb, (n_points + MO_BM - 1) / MO_BM);
+    k_basis<false, 1><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
@@ -983,6 +993,46 @@ cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double
                 COUNT_LAUNCH();
             }
         }
+    }
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// row f3: non-local pseudopotential energy (nlpp_kernels.cuh).  Two phases because the number of (electron, atom) pairs
+// inside the cut-offs is data: nl_pairs_count leaves the offsets on the device (the host reads the total), nl_evaluate
+// runs the points through basis values -> contraction -> ratios in chunks of 5 W points (the sweep's own Phi / V buffers).
+cudaError_t launch_nl_count(const SysDev& s, const WalkDev& wd, const NlArgs& a, cudaStream_t st) {
+    const long n = (long)wd.W * a.ns;
+    if (n == 0) return cudaMemsetAsync(a.cnt, 0, 4, st);
+    k_nl_count<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s, wd, a);
+    COUNT_LAUNCH();
+    k_nl_scan<<<1, 1024, 0, st>>>(a.cnt, n);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+cudaError_t launch_nl_evaluate(const SysDev& s, const WalkDev& wd, const NlArgs& a, int n_pairs, int n_sm, unsigned* mo_epoch, double* vnl,
+                               cudaStream_t st) {
+    const long n = (long)wd.W * a.ns;
+    if (n_pairs > 0) {
+        k_nl_fill<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(s, wd, a);
+        COUNT_LAUNCH();
+        const long npts = 12L * n_pairs;
+        k_nl_points<<<(unsigned)((npts + 255) / 256), 256, 0, st>>>(s, wd, a, n_pairs);
+        COUNT_LAUNCH();
+        const long chunk = 5L * wd.W;
+        for (long p0 = 0; p0 < npts; p0 += chunk) {
+            const int m = (int)(npts - p0 < chunk ? npts - p0 : chunk);
+            cudaError_t e = launch_basis_values(s, a.pts + 3 * p0, m, wd.Phi, st);
+            if (e != cudaSuccess) return e;
+            e = launch_mo(s, a.spin, wd.Phi, m, wd.V, wd.ldv, wd.mo_ws, wd.mo_flags, mo_grid_for(s, a.spin, m, n_sm), ++*mo_epoch, nullptr, st);
+            if (e != cudaSuccess) return e;
+            k_nl_ratio<<<(m + 7) / 8, 256, 0, st>>>(s, wd, a, p0, m, wd.V);
+            COUNT_LAUNCH();
+        }
+    }
+    if (n > 0) {
+        k_nl_reduce<<<wd.W, 256, 0, st>>>(wd, a, vnl);
+        COUNT_LAUNCH();
     }
     return cudaGetLastError();
 }

@@ -6,6 +6,7 @@ namespace qmc {
 
 // tilemax ([MT][KB], may be NULL): max |entry| of every A stage, for the optional screening of the MO contraction
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st);
+cudaError_t launch_basis_values(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st);
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
                       int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st);
 cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int rows, cudaStream_t st);
@@ -45,6 +46,9 @@ cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, u
                                const double* e_trial_dev, cudaStream_t st);
 cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st);
 // row f2 (first half): acc[W][n_atoms][3] += spin sp's part of d ln|Psi|/dR_a (+ the Jastrow part with spin 0); Mt: scratch [W][nsp][nbp]
+cudaError_t launch_nl_count(const SysDev& s, const WalkDev& wd, const NlArgs& a, cudaStream_t st);
+cudaError_t launch_nl_evaluate(const SysDev& s, const WalkDev& wd, const NlArgs& a, int n_pairs, int n_sm, unsigned* mo_epoch, double* vnl,
+                               cudaStream_t st);
 cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double* Nt, double* Bm, double* U, double* XT, double* fg,
                           double* acc_E, double* acc_psi, cudaStream_t st);
 cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st);
