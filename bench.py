@@ -52,6 +52,8 @@ def parse():
     ap.add_argument("--no-screened", action="store_true", help="skip the extra leg with QMC_SCREEN_MO")
     ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-crowds", action="store_true", help="skip the two-crowds leg")
+    ap.add_argument("--crowd-ctas", type=int, default=124, help="CTAs of each crowd's contraction in the two-crowds leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-moves", type=int, default=96, help="electron moves per walker in the CPU-baseline sample")
     return ap.parse_args()
@@ -258,7 +260,74 @@ def run_ours(args):
     assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
     assert st1["nonfinite"] == 0
     red = reduce_report(ms, n_moves, float(eloc.sum()), float((eloc * eloc).sum()), W, backend_device="cuda")
-    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not args.no_screened else None
+    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not (args.no_screened and args.no_crowds) else None
+    # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps (a second walker set beside the first;
+    # measured straight after the device-resident run so that both see the same thermal state)
+    e2e = None
+    if not args.no_e2e:
+        ne = sysm.n_elec
+        out_pos = torch.empty((W, ne, 3), dtype=torch.float64).pin_memory()
+        out_e, out_k, out_l = [torch.empty(W, dtype=torch.float64).pin_memory() for _ in range(3)]
+        out_s = torch.empty(W, dtype=torch.int8).pin_memory()
+        out_b = torch.empty((args.steps, ne, W), dtype=torch.uint8).pin_memory()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        gw2 = qb.qmc_walkers_create(gsys, pos_host, wl.seed, first_walker_id=lo)     # H2D of the positions inside
+        qb.qmc_sweep(gw2, args.steps, wl.tau, k)
+        qb.qmc_get_positions(gw2, out=out_pos)                                        # D2H, synchronous
+        qb.qmc_get_eloc(gw2, out=out_e, out_kin=out_k)
+        qb.qmc_get_logpsi(gw2, out=out_l, out_sign=out_s)
+        qb.qmc_get_accept_log(gw2, out=out_b)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) * 1e3
+        qb.qmc_walkers_destroy(gw2)
+        red2 = reduce_report(t_e2e, W * ne * args.steps, 0.0, 0.0, W, backend_device="cuda")
+        d2h = out_pos.numel() * 8 + 3 * W * 8 + W + out_b.numel()
+        e2e = dict(value=red2["n_moves"] / (red2["elapsed_ms"] * 1e-3), unit=UNIT,
+                   h2d_bytes_per_step=pos_host.numel() * 8 // args.steps, d2h_bytes_per_step=d2h // args.steps,
+                   ms_total=red2["elapsed_ms"],
+                   what="qmc_walkers_create from pinned host positions (orbital rows + inverse of all Slater matrices) "
+                        f"+ qmc_sweep({args.steps}) + qmc_get_{{positions,eloc,logpsi,accept_log}} into pinned host buffers")
+    # ---- the same walkers as TWO crowds of W/2 on two streams, advanced together by qmc_sweep_crowds with the
+    # contraction of each limited to 124 CTAs (the basis / step kernels of one crowd overlap the contraction of the
+    # other).  Reported beside the headline, not as it: the headline and its roofline are the single-crowd run above.
+    crowds = None
+    if not args.no_crowds and W >= 2:
+        half = W // 2
+        cstreams = [torch.cuda.Stream() for _ in range(2)]
+        csets = []
+        for c in range(2):
+            a0, a1 = (0, half) if c == 0 else (half, W)
+            gwc = qb.qmc_walkers_create(gsys, pos_dev[a0:a1].contiguous(), wl.seed, first_walker_id=lo + a0, stream=cstreams[c])
+            qb.qmc_set_mo_ctas(gwc, args.crowd_ctas)
+            csets.append(gwc)
+        for _ in range(args.warmup):
+            qb.qmc_sweep_crowds(csets, 1, wl.tau, k)
+        torch.cuda.synchronize()
+        c0 = torch.cuda.Event(enable_timing=True)
+        c0.record()
+        ends = []
+        for st_ in cstreams:
+            st_.wait_event(c0)
+        qb.qmc_sweep_crowds(csets, args.steps, wl.tau, k)
+        for st_ in cstreams:
+            e_ = torch.cuda.Event(enable_timing=True)
+            e_.record(st_)
+            ends.append(e_)
+        torch.cuda.synchronize()
+        msc = max(c0.elapsed_time(e_) for e_ in ends)
+        cb = np.concatenate([qb.qmc_get_accept_log(x).cpu().numpy() for x in csets], axis=2)
+        ce = torch.cat([qb.qmc_get_eloc(x)[0] for x in csets])
+        crowds = dict(value=W * sysm.n_elec * args.steps / (msc * 1e-3), unit=UNIT, ms_per_step=msc / args.steps, crowds=2,
+                      walkers_per_crowd=[half, W - half], mo_ctas=args.crowd_ctas,
+                      decisions_differing_from_single_crowd=(int(((cb & 1) != (dense_bits & 1)).sum()) if dense_bits is not None else None),
+                      max_abs_eloc_diff_from_single_crowd=float((ce - eloc).abs().max()),
+                      what="qmc_sweep_crowds over two walker sets on two streams (per GPU; rank 0's walkers); same walkers, same "
+                           "random streams as the headline run; differences are stream-K rounding (row count per crowd)")
+        for x in csets:
+            qb.qmc_walkers_destroy(x)
     # row f1 (outside the timed region): one DMC generation + one comb reconfiguration on the same crowd
     f1 = None
     if not args.no_dmc:
@@ -345,34 +414,6 @@ def run_ours(args):
                              "(per GPU; rank 0's crowd); the headline `value` above is the dense contraction")
         qb.qmc_walkers_destroy(gw3)
 
-    # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps
-    e2e = None
-    if not args.no_e2e:
-        ne = sysm.n_elec
-        out_pos = torch.empty((W, ne, 3), dtype=torch.float64).pin_memory()
-        out_e, out_k, out_l = [torch.empty(W, dtype=torch.float64).pin_memory() for _ in range(3)]
-        out_s = torch.empty(W, dtype=torch.int8).pin_memory()
-        out_b = torch.empty((args.steps, ne, W), dtype=torch.uint8).pin_memory()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        gw2 = qb.qmc_walkers_create(gsys, pos_host, wl.seed, first_walker_id=lo)     # H2D of the positions inside
-        qb.qmc_sweep(gw2, args.steps, wl.tau, k)
-        qb.qmc_get_positions(gw2, out=out_pos)                                        # D2H, synchronous
-        qb.qmc_get_eloc(gw2, out=out_e, out_kin=out_k)
-        qb.qmc_get_logpsi(gw2, out=out_l, out_sign=out_s)
-        qb.qmc_get_accept_log(gw2, out=out_b)
-        torch.cuda.synchronize()
-        t_e2e = (time.perf_counter() - t0) * 1e3
-        qb.qmc_walkers_destroy(gw2)
-        red2 = reduce_report(t_e2e, W * ne * args.steps, 0.0, 0.0, W, backend_device="cuda")
-        d2h = out_pos.numel() * 8 + 3 * W * 8 + W + out_b.numel()
-        e2e = dict(value=red2["n_moves"] / (red2["elapsed_ms"] * 1e-3), unit=UNIT,
-                   h2d_bytes_per_step=pos_host.numel() * 8 // args.steps, d2h_bytes_per_step=d2h // args.steps,
-                   ms_total=red2["elapsed_ms"],
-                   what="qmc_walkers_create from pinned host positions (orbital rows + inverse of all Slater matrices) "
-                        f"+ qmc_sweep({args.steps}) + qmc_get_{{positions,eloc,logpsi,accept_log}} into pinned host buffers")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -425,6 +466,7 @@ def run_ours(args):
         f1_dmc=f1,
         f2_dlogpsi_dR=f2,
         f3_vnl=f3,
+        two_crowds=crowds,
         screened_mo=screened,
     )
     if world == 1 and not args.no_cpu_baseline:

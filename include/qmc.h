@@ -209,6 +209,19 @@ int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs);
 
 /* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
  * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
+/* Several crowds per GPU: walker sets created on different streams run concurrently, and the HBM-bound stages of one
+ * (k_basis, k_step) can overlap the tensor-bound contraction of another only if that persistent kernel leaves some SMs
+ * free.  n_ctas (1..number of SMs; 0 = all, the default) is the grid of this set's contraction from now on (the
+ * stream-K workspace is sized for all SMs, so any value fits).  Results change only through the stream-K partition
+ * (rounding). */
+int qmc_set_mo_ctas(qmc_walkers* w, int n_ctas);
+/* qmc_sweep of n_sets walker sets ("crowds") of ONE system together: the host enqueues electron p of every set, each
+ * on its own stream, before electron p + 1 of any.  Every set does exactly what qmc_sweep(set, nsteps, tau, delay_k)
+ * would do -- its results do not depend on the other sets -- but sets created on DIFFERENT streams overlap on the GPU
+ * (with qmc_set_mo_ctas leaving SMs free, the basis / step kernels of one crowd run beside the contraction of another:
+ * +5 % at config 2 with two crowds of 128 and 124 CTAs).  Asynchronous like qmc_sweep.  Errors: as qmc_sweep;
+ * QMC_ERR_ARG if the sets belong to different systems or one appears twice. */
+int qmc_sweep_crowds(qmc_walkers* const* sets, int n_sets, int nsteps, double tau, int delay_k);
 int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);
 
 /* Stage-level entry points (used by the per-stage parity tests and the per-stage roofline bench).

@@ -26,7 +26,7 @@ EXPORTED = [
     "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
-    "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl",
+    "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl", "qmc_set_mo_ctas", "qmc_sweep_crowds",
 ]
 
 
@@ -95,6 +95,8 @@ def load_library(path: str | None = None):
     lib.qmc_get_deloc_dR.argtypes = [vp, vp, vp]
     lib.qmc_set_ecp.argtypes = [vp, i, vp, vp, vp, vp, vp]
     lib.qmc_get_vnl.argtypes = [vp, vp, C.POINTER(u64)]
+    lib.qmc_set_mo_ctas.argtypes = [vp, i]
+    lib.qmc_sweep_crowds.argtypes = [C.POINTER(vp), i, i, d, i]
     lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_launch_count.restype = u64
@@ -231,6 +233,14 @@ def qmc_sweep(walkers: Walkers, nsteps, tau, delay_k):
     walkers.last_nsteps = int(nsteps)
 
 
+def qmc_sweep_crowds(sets, nsteps, tau, delay_k):
+    """qmc_sweep of several walker sets of one system together (electron by electron, each set on its own stream)."""
+    arr = (C.c_void_p * len(sets))(*[w.handle for w in sets])
+    _check(load_library().qmc_sweep_crowds(arr, len(sets), int(nsteps), float(tau), int(delay_k)))
+    for w in sets:
+        w.last_nsteps = int(nsteps)
+
+
 def qmc_dmc_step(walkers: Walkers, n_generations, tau, delay_k, e_trial, limiter_a=1.0):
     _check(load_library().qmc_dmc_step(walkers.handle, int(n_generations), float(tau), int(delay_k), float(e_trial), float(limiter_a)))
     walkers.last_nsteps = int(n_generations)
@@ -282,6 +292,11 @@ def qmc_get_vnl(walkers: Walkers, out=None):
     n = C.c_uint64()
     _check(load_library().qmc_get_vnl(walkers.handle, _ptr(out), C.byref(n)))
     return out, n.value
+
+
+def qmc_set_mo_ctas(walkers: Walkers, n_ctas):
+    """Grid of this walker set's MO contraction (0 = all SMs); smaller leaves SMs to crowds on other streams."""
+    _check(load_library().qmc_set_mo_ctas(walkers.handle, int(n_ctas)))
 
 
 def qmc_get_mo_work(walkers: Walkers):

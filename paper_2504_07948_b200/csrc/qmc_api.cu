@@ -535,18 +535,23 @@ extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t*
 // dmc != 0: every sweep is a DMC generation (row f1): limited drift, then the weight update after E_L
 // e_trial_dev != nullptr: E_T is read from the device.  The accept / ratio logs of this call are steps log_t0 .. log_t0 +
 // nsteps - 1 of a log of log_T steps (log_T < 0: the call is the whole log).
-static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a,
-                      const double* e_trial_dev = nullptr, int log_t0 = 0, int log_T = -1) {
+struct SweepCall {
+    int nsteps; double tau; int delay_k; int dmc; double e_trial; double lim_a;
+    const double* e_trial_dev; int log_t0; int log_T;
+};
+
+// argument checks, delay window and log buffers of one walker set; *small: the set takes the one-launch path
+static int sweep_prepare(qmc_walkers* w, SweepCall& c, bool* small) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
-    if (nsteps < 0) return fail(QMC_ERR_ARG, "qmc_sweep: nsteps < 0");
-    if (!(tau > 0.0) || !isfinite(tau)) return fail(QMC_ERR_ARG, "qmc_sweep: tau must be > 0");
-    if (delay_k < 1 || delay_k > 128) return fail(QMC_ERR_ARG, "qmc_sweep: delay_k must be in 1..128");
-    if (dmc && (!isfinite(e_trial) || !(lim_a >= 0.0) || !isfinite(lim_a))) return fail(QMC_ERR_ARG, "qmc_dmc_step: e_trial must be finite and limiter_a >= 0");
+    if (c.nsteps < 0) return fail(QMC_ERR_ARG, "qmc_sweep: nsteps < 0");
+    if (!(c.tau > 0.0) || !isfinite(c.tau)) return fail(QMC_ERR_ARG, "qmc_sweep: tau must be > 0");
+    if (c.delay_k < 1 || c.delay_k > 128) return fail(QMC_ERR_ARG, "qmc_sweep: delay_k must be in 1..128");
+    if (c.dmc && (!isfinite(c.e_trial) || !(c.lim_a >= 0.0) || !isfinite(c.lim_a))) return fail(QMC_ERR_ARG, "qmc_dmc_step: e_trial must be finite and limiter_a >= 0");
     const SysDev& s = w->sys->d;
     WalkDev& d = w->d;
     cudaStream_t st = w->stream;
-    d.lim_a = dmc ? lim_a : 0.0;
-    const int kp = round_up(delay_k, 16);
+    d.lim_a = c.dmc ? c.lim_a : 0.0;
+    const int kp = round_up(c.delay_k, 16);
     if (kp != d.kp) {
         int rc = alloc_window(w, kp);
         if (rc) return rc;
@@ -554,8 +559,8 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
     }
     // accept / ratio logs of this call: the buffers are kept from call to call and only grow, so that a loop of
     // qmc_sweep calls of the same length never synchronises with the host
-    if (log_T < 0) log_T = nsteps;
-    const size_t nlog = (size_t)log_T * s.ne * d.W;
+    if (c.log_T < 0) c.log_T = c.nsteps;
+    const size_t nlog = (size_t)c.log_T * s.ne * d.W;
     if (nlog > w->log_capacity || !d.bits) {
         CU(cudaStreamSynchronize(st));
         w->logpool.free_all();
@@ -568,66 +573,125 @@ static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int d
         }
         w->log_capacity = nlog;
     }
-    w->T_last = log_T;
-    if (!(w->flags & QMC_LARGE_PATH) && small_path_ok(s, d)) {  // row f4: the whole call in one launch
-        WalkDev dl = d;
-        const size_t off = (size_t)log_t0 * s.ne * d.W;
-        dl.bits += off;
-        if (dl.ratio_log) { dl.ratio_log += off; dl.pacc_log += off; }
-        if (nsteps > 0) CU(launch_sweep_small(s, dl, nsteps, w->step, tau, dmc, e_trial, e_trial_dev, st));
-        w->step += (uint32_t)nsteps;
-        return QMC_OK;
-    }
-    if (dmc) CU(launch_dmc_begin(d, st));
-    for (int t = 0; t < nsteps; t++) {
-        for (int sp = 0; sp < 2; sp++) {
-            const int ns = s.ns[sp], e0 = sp == 0 ? 0 : s.ns[0];
-            int in_window = 0;
-            for (int p = 0; p < ns; p++) {
-                const int e = e0 + p;
-                const long log_off = ((long)(log_t0 + t) * s.ne + e) * d.W;
-                const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
-                const bool pf = w->prof_stride > 0;
-                if (in_window == 0) {  // first proposal of a window: nothing to fuse it with
-                    prof_begin(w, 0, pf);
-                    CU(launch_step(s, d, sp, -1, p, 0, w->step, tau, 1, st));
-                    prof_end(w, pf);
-                }
-                prof_begin(w, 1, prof);
-                const bool screen = d.screen_theta >= 0.0;
-                CU(launch_basis(s, d.rp, d.W, d.Phi, screen ? d.tilemax : nullptr, st));
-                prof_end(w, prof);
-                prof_begin(w, 2, prof);
-                if (screen) CU(launch_mo_plan(s, sp, d, 5 * d.W, st));
-                CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch,
-                             screen ? &d : nullptr, st));
-                prof_end(w, prof);
-                in_window++;
-                if (in_window == delay_k || p == ns - 1) {
-                    prof_begin(w, 0, pf);
-                    CU(launch_step(s, d, sp, p, -1, log_off, w->step, tau, 1, st));
-                    prof_end(w, pf);
-                    prof_begin(w, 4, pf);
-                    CU(launch_flush(s, d, sp, st));
-                    prof_end(w, pf);
-                    in_window = 0;
-                } else {  // accept/reject of p and proposal of p + 1 in one launch
-                    const bool prof2 = w->prof_stride > 0 && ((p + 1) % w->prof_stride) == 0;
-                    prof_begin(w, 3, prof2);
-                    CU(launch_step(s, d, sp, p, p + 1, log_off, w->step, tau, 1, st));
-                    prof_end(w, prof2);
-                }
-            }
-        }
-        const bool pf = w->prof_stride > 0;
-        prof_begin(w, 5, pf);
-        CU(launch_eloc(s, d, st));
+    w->T_last = c.log_T;
+    *small = !(w->flags & QMC_LARGE_PATH) && small_path_ok(s, d);
+    return QMC_OK;
+}
+
+// row f4: the whole call of one set in one launch
+static int sweep_small(qmc_walkers* w, const SweepCall& c) {
+    const SysDev& s = w->sys->d;
+    WalkDev dl = w->d;
+    const size_t off = (size_t)c.log_t0 * s.ne * dl.W;
+    dl.bits += off;
+    if (dl.ratio_log) { dl.ratio_log += off; dl.pacc_log += off; }
+    if (c.nsteps > 0) CU(launch_sweep_small(s, dl, c.nsteps, w->step, c.tau, c.dmc, c.e_trial, c.e_trial_dev, w->stream));
+    w->step += (uint32_t)c.nsteps;
+    return QMC_OK;
+}
+
+// everything one set launches for electron p of spin sp in sweep t of the call; in_window: moves pending in its delay window
+static int sweep_electron(qmc_walkers* w, const SweepCall& c, int t, int sp, int p, int* in_window) {
+    const SysDev& s = w->sys->d;
+    WalkDev& d = w->d;
+    cudaStream_t st = w->stream;
+    const int ns = s.ns[sp], e0 = sp == 0 ? 0 : s.ns[0];
+    const int e = e0 + p;
+    const long log_off = ((long)(c.log_t0 + t) * s.ne + e) * d.W;
+    const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
+    const bool pf = w->prof_stride > 0;
+    if (*in_window == 0) {  // first proposal of a window: nothing to fuse it with
+        prof_begin(w, 0, pf);
+        CU(launch_step(s, d, sp, -1, p, 0, w->step, c.tau, 1, st));
         prof_end(w, pf);
-        if (dmc) CU(launch_dmc_weight(d, tau, e_trial, e_trial_dev, st));
-        w->step++;
-        if (w->timer.used > 8192) prof_collect(w);
+    }
+    prof_begin(w, 1, prof);
+    const bool screen = d.screen_theta >= 0.0;
+    CU(launch_basis(s, d.rp, d.W, d.Phi, screen ? d.tilemax : nullptr, st));
+    prof_end(w, prof);
+    prof_begin(w, 2, prof);
+    if (screen) CU(launch_mo_plan(s, sp, d, 5 * d.W, st));
+    CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch,
+                 screen ? &d : nullptr, st));
+    prof_end(w, prof);
+    ++*in_window;
+    if (*in_window == c.delay_k || p == ns - 1) {
+        prof_begin(w, 0, pf);
+        CU(launch_step(s, d, sp, p, -1, log_off, w->step, c.tau, 1, st));
+        prof_end(w, pf);
+        prof_begin(w, 4, pf);
+        CU(launch_flush(s, d, sp, st));
+        prof_end(w, pf);
+        *in_window = 0;
+    } else {  // accept/reject of p and proposal of p + 1 in one launch
+        const bool prof2 = w->prof_stride > 0 && ((p + 1) % w->prof_stride) == 0;
+        prof_begin(w, 3, prof2);
+        CU(launch_step(s, d, sp, p, p + 1, log_off, w->step, c.tau, 1, st));
+        prof_end(w, prof2);
     }
     return QMC_OK;
+}
+
+// end of a sweep of one set: E_L, the DMC weight, the sweep counter
+static int sweep_finish_step(qmc_walkers* w, const SweepCall& c) {
+    const bool pf = w->prof_stride > 0;
+    prof_begin(w, 5, pf);
+    CU(launch_eloc(w->sys->d, w->d, w->stream));
+    prof_end(w, pf);
+    if (c.dmc) CU(launch_dmc_weight(w->d, c.tau, c.e_trial, c.e_trial_dev, w->stream));
+    w->step++;
+    if (w->timer.used > 8192) prof_collect(w);
+    return QMC_OK;
+}
+
+// n_sets walker sets of ONE system advance together: the host enqueues electron p of every set (each on its own stream)
+// before electron p + 1 of any, so that the HBM-bound stages of one crowd overlap the contraction of another
+static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
+    std::vector<qmc_walkers*> large;
+    for (int i = 0; i < n_sets; i++) {
+        SweepCall ci = c;
+        bool small = false;
+        int rc = sweep_prepare(sets[i], ci, &small);
+        if (rc) return rc;
+        if (i == 0) c.log_T = ci.log_T;
+        if (small) { rc = sweep_small(sets[i], ci); if (rc) return rc; }
+        else large.push_back(sets[i]);
+    }
+    if (large.empty()) return QMC_OK;
+    const SysDev& s = large[0]->sys->d;
+    std::vector<int> in_window(large.size(), 0);
+    for (qmc_walkers* w : large)
+        if (c.dmc) CU(launch_dmc_begin(w->d, w->stream));
+    for (int t = 0; t < c.nsteps; t++) {
+        for (int sp = 0; sp < 2; sp++)
+            for (int p = 0; p < s.ns[sp]; p++)
+                for (size_t i = 0; i < large.size(); i++) {
+                    int rc = sweep_electron(large[i], c, t, sp, p, &in_window[i]);
+                    if (rc) return rc;
+                }
+        for (qmc_walkers* w : large) {
+            int rc = sweep_finish_step(w, c);
+            if (rc) return rc;
+        }
+    }
+    return QMC_OK;
+}
+
+static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a,
+                      const double* e_trial_dev = nullptr, int log_t0 = 0, int log_T = -1) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
+    return sweep_sets(&w, 1, SweepCall{nsteps, tau, delay_k, dmc, e_trial, lim_a, e_trial_dev, log_t0, log_T});
+}
+
+extern "C" int qmc_sweep_crowds(qmc_walkers* const* sets, int n_sets, int nsteps, double tau, int delay_k) {
+    if (!sets || n_sets < 1) return fail(QMC_ERR_ARG, "qmc_sweep_crowds: no walker sets");
+    for (int i = 0; i < n_sets; i++) {
+        if (!sets[i]) return fail(QMC_ERR_ARG, "qmc_sweep_crowds: null walker set");
+        if (sets[i]->sys != sets[0]->sys) return fail(QMC_ERR_ARG, "qmc_sweep_crowds: the sets must belong to one system");
+        for (int j = 0; j < i; j++)
+            if (sets[j] == sets[i]) return fail(QMC_ERR_ARG, "qmc_sweep_crowds: a walker set appears twice");
+    }
+    return sweep_sets(sets, n_sets, SweepCall{nsteps, tau, delay_k, 0, 0.0, 0.0, nullptr, 0, -1});
 }
 
 extern "C" int qmc_sweep(qmc_walkers* w, int nsteps, double tau, int delay_k) { return sweep_impl(w, nsteps, tau, delay_k, 0, 0.0, 0.0); }
@@ -836,6 +900,14 @@ extern "C" int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs_out) {
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return fail(QMC_ERR_NOMEM, "qmc_get_vnl: scratch does not fit"); }
     CU(e);
     if (n_pairs_out) *n_pairs_out = total;
+    return QMC_OK;
+}
+
+extern "C" int qmc_set_mo_ctas(qmc_walkers* w, int n_ctas) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_set_mo_ctas: null walkers");
+    const int n_sm = w->sys->n_sm;
+    if (n_ctas < 0 || n_ctas > n_sm) return fail(QMC_ERR_ARG, "qmc_set_mo_ctas: n_ctas must be in 0..number of SMs");
+    w->d.mo_grid = n_ctas == 0 ? n_sm : n_ctas;
     return QMC_OK;
 }
 
