@@ -96,6 +96,7 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_clone.restype = C.c_void_p
     lib.oracle_walker_clone.argtypes = [C.c_void_p, C.c_void_p]
     lib.oracle_walker_deloc_dR.argtypes = [C.c_void_p, C.c_void_p, _dp]
+    lib.oracle_walker_deloc_dR_atoms.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _ip, _dp]
     lib.oracle_basis_eval_d3.argtypes = [C.c_void_p, _dp, _dp, _dp]
     lib.oracle_walker_vnl.restype = C.c_double
     lib.oracle_walker_vnl.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int, _ip, _ip, _dp, _dp, _dp,
@@ -308,8 +309,13 @@ class OracleWalker:
         self.lib.oracle_walker_dlogpsi_dR(self.sys.h, self.h, _d(out))
         return out
 
-    def deloc_dR(self):
-        """d E_L / d R_a for every atom, [n_atoms][3] (row f2, second half; the paper's eq. 4)."""
+    def deloc_dR(self, atoms=None):
+        """d E_L / d R_a for every atom (or the listed ones), [n][3] (row f2, second half; the paper's eq. 4)."""
+        if atoms is not None:
+            sel = np.ascontiguousarray(atoms, np.int32)
+            out = np.zeros((len(sel), 3))
+            self.lib.oracle_walker_deloc_dR_atoms(self.sys.h, self.h, len(sel), sel.ctypes.data_as(_ip), _d(out))
+            return out
         out = np.zeros((self.sys.n_atoms, 3))
         self.lib.oracle_walker_deloc_dR(self.sys.h, self.h, _d(out))
         return out

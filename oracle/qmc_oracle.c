@@ -926,10 +926,13 @@ void oracle_basis_eval_d3(const oracle_system *s, const double r[3], double *hes
 
 static real pade_d3u(real a, real b, real r) { real q = 1 + b * r; return 6 * a * b * b / (q * q * q * q); }
 
-void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, double *out) {
+/* the atoms sel[0..n_sel) only (out[n_sel][3]): every atom's derivative is computed independently of the others, so a
+ * test at full size can afford a few of them */
+void oracle_walker_deloc_dR_atoms(const oracle_system *s, const oracle_walker *w, int n_sel, const int *sel, double *out) {
     int nb = s->n_basis, ne = w->ne, na = s->n_atoms;
     static const int hidx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};
-    real *acc = (real *)calloc((size_t)3 * na, sizeof(real));
+    real *acc = (real *)calloc((size_t)3 * n_sel, sizeof(real));
+    int *flist = (int *)malloc((size_t)nb * sizeof(int)); /* functions of the current atom */
     real *gJ = (real *)malloc((size_t)3 * ne * sizeof(real));
     for (int i = 0; i < ne; i++) {
         real v, lp;
@@ -974,7 +977,10 @@ void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, doub
                 for (int k = 0; k < ns; k++) a += T[(size_t)j * ns + k] * Ainv[(size_t)k * ns + i];
                 X[(size_t)j * ns + i] = a;
             }
-        for (int a = 0; a < na; a++)
+        for (int ia = 0; ia < n_sel; ia++) {
+            int a = sel[ia], nfa = 0;
+            for (int l = 0; l < nb; l++)
+                if (f_atom[l] == a) flist[nfa++] = l;
             for (int d = 0; d < 3; d++) {
                 for (int i = 0; i < ns; i++) {
                     const real *bi = bas + (size_t)i * 14 * nb;
@@ -988,8 +994,8 @@ void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, doub
                     for (int b = 0; b < 3; b++) dg[b] = -(u2 * x[d] * x[b] / (r * r) + u1 * ((d == b ? 1 / r : 0) - x[d] * x[b] / (r * r * r)));
                     for (int j = 0; j < ns; j++) {
                         real sa = 0, sb = 0;
-                        for (int l = 0; l < nb; l++) {
-                            if (f_atom[l] != a) continue;
+                        for (int li = 0; li < nfa; li++) {
+                            int l = flist[li];
                             real c = C[(size_t)l * ns + j];
                             sa += c * bi[(size_t)d * nb + l];
                             real hg = 0;
@@ -1005,13 +1011,15 @@ void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, doub
                 for (int i = 0; i < ns; i++)
                     for (int j = 0; j < ns; j++)
                         tr += Ainv[(size_t)j * ns + i] * dB[(size_t)i * ns + j] - X[(size_t)j * ns + i] * dA[(size_t)i * ns + j];
-                acc[3 * a + d] += tr;
+                acc[3 * ia + d] += tr;
             }
+        }
         free(B); free(T); free(X); free(dA); free(dB); free(bas);
     }
     /* dc_i and dV */
-    for (int a = 0; a < na; a++)
+    for (int ia = 0; ia < n_sel; ia++)
         for (int d = 0; d < 3; d++) {
+            int a = sel[ia];
             real sum = 0;
             for (int i = 0; i < ne; i++) {
                 const real *g = gJ + 3 * i;
@@ -1032,10 +1040,17 @@ void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, doub
                 real rr = R_SQRT(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
                 sum -= s->Z[a] * s->Z[b] * y[d] / (rr * rr * rr);
             }
-            acc[3 * a + d] += sum;
+            acc[3 * ia + d] += sum;
         }
-    for (int k = 0; k < 3 * na; k++) out[k] = (double)acc[k];
-    free(acc); free(gJ); free(f_atom);
+    for (int k = 0; k < 3 * n_sel; k++) out[k] = (double)acc[k];
+    free(acc); free(gJ); free(f_atom); free(flist);
+}
+
+void oracle_walker_deloc_dR(const oracle_system *s, const oracle_walker *w, double *out) {
+    int *all = (int *)malloc((size_t)s->n_atoms * sizeof(int));
+    for (int a = 0; a < s->n_atoms; a++) all[a] = a;
+    oracle_walker_deloc_dR_atoms(s, w, s->n_atoms, all, out);
+    free(all);
 }
 
 /* ------------------------------------------------------------------ row f3: non-local pseudopotential energy

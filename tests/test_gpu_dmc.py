@@ -226,3 +226,36 @@ def test_dmc_run_equals_the_calls_it_replaces():
     assert e_end == pytest.approx(e_t, rel=1e-14)
     assert np.array_equal(qb.qmc_get_positions(a).cpu().numpy(), qb.qmc_get_positions(b).cpu().numpy())
     np.testing.assert_allclose(qb.qmc_get_weights(a)[0].cpu().numpy(), qb.qmc_get_weights(b)[0].cpu().numpy(), rtol=1e-13)
+
+
+def test_config2_full_size_generation_sampled():
+    """Row f1 at the size and in the launch configuration bench.py times (256-water config, 256 walkers, delay 64):
+    one DMC generation of the whole crowd, two sampled walkers against the oracle's generation."""
+    from concurrent.futures import ThreadPoolExecutor
+    wl = qi.make_workload(2)
+    sysm = wl.system
+    g = qb.qmc_init_from(sysm)
+    gw = qb.qmc_walkers_create(g, wl.positions(), wl.seed)
+    e0 = qb.qmc_get_eloc(gw)[0].cpu().numpy()
+    e_t = float(e0.mean())
+    qb.qmc_dmc_step(gw, 1, wl.tau, wl.delay_k, e_t, 1.0)
+    bits = qb.qmc_get_accept_log(gw).cpu().numpy()
+    wts, te = (x.cpu().numpy() for x in qb.qmc_get_weights(gw))
+    el = qb.qmc_get_eloc(gw)[0].cpu().numpy()
+    osys = oracle.OracleSystem(sysm)
+
+    def one(n):
+        ow = osys.walker(wl.positions(n, n + 1)[0])
+        e_start = ow.eloc()[0]
+        return (n, e_start) + tuple(ow.dmc_generation(wl.seed, n, 0, wl.tau, 1.0, e_t, e_start, 1.0))
+    with ThreadPoolExecutor(max_workers=2) as ex:
+        res = list(ex.map(one, [3, 254]))
+    for n, e_start, ob, e_new, w_new, te_o in res:
+        assert abs(e0[n] - e_start) < 1e-6
+        d = (bits[0, :, n] & 1) != (ob & 1)
+        assert not np.any(d & (((bits[0, :, n] | ob) & 2) == 0)), "unflagged accept/reject mismatch"
+        if not d.any():
+            assert te[n] == pytest.approx(te_o, rel=1e-12)
+            assert abs(el[n] - e_new) < 1e-6                      # reading A26: 1e-9 relative to the energy scale
+            # the exponent tau_eff (E_old + E_new)/2 carries the absolute error of E_L
+            assert wts[n] == pytest.approx(w_new, rel=1e-8)

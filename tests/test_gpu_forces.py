@@ -126,3 +126,37 @@ def test_deloc_dR_host_output_and_odd_sizes():
     for n in range(W):
         ref = osys.walker(gpos[n]).deloc_dR()
         assert np.abs(de[n] - ref).max() < 1e-8 * max(1.0, np.abs(ref).max()), n
+
+
+def test_config2_full_size_forces_and_nlpp_sampled():
+    """Rows f2 and f3 at the size and in the launch configuration bench.py times (256-water config, 256 walkers): the
+    oracle does two sampled walkers, three sampled atoms for dE_L/dR_a and d ln|Psi|/dR_a, and a pseudopotential that
+    is switched on for six atoms only (the oracle then has a few dozen quadrature pairs per walker to do)."""
+    from concurrent.futures import ThreadPoolExecutor
+    wl = qi.make_workload(2)
+    sysm = wl.system
+    atoms = [0, 1, 767]
+    ecp = qi.make_ecp(sysm)
+    rc = np.zeros(sysm.n_atoms)
+    rc[[0, 1, 2, 300, 301, 767]] = 2.0
+    ecp.rcut = rc
+    g = qb.qmc_init_from(sysm)
+    qb.qmc_set_ecp(g, ecp)
+    gw = qb.qmc_walkers_create(g, wl.positions(), wl.seed)
+    de, dp = (x.cpu().numpy() for x in qb.qmc_get_deloc_dR(gw))
+    vnl, n_pairs = qb.qmc_get_vnl(gw)
+    vnl = vnl.cpu().numpy()
+    assert n_pairs > 0
+    osys = oracle.OracleSystem(sysm)
+    sample = [0, 255]
+
+    def one(n):
+        ow = osys.walker(wl.positions(n, n + 1)[0])
+        return n, ow.deloc_dR(atoms), ow.dlogpsi_dR()[atoms], ow.vnl(ecp, wl.seed, n, 0)
+    with ThreadPoolExecutor(max_workers=2) as ex:
+        res = list(ex.map(one, sample))
+    for n, ref_e, ref_p, ref_v in res:
+        # cond(A) up to ~1e6 at N_s = 1024 (reading A26) enters the trace terms twice
+        assert np.abs(de[n][atoms] - ref_e).max() < 1e-7 * max(1.0, np.abs(ref_e).max()), (n, de[n][atoms], ref_e)
+        assert np.abs(dp[n][atoms] - ref_p).max() < 1e-8 * max(1.0, np.abs(ref_p).max()), n
+        assert vnl[n] == pytest.approx(ref_v, rel=1e-8, abs=1e-9), n

@@ -125,3 +125,10 @@ def test_deloc_dR_translation_sum_rule():
         Rm[:, d] -= h
         tot[d] = (osys.walker(Rp).eloc()[0] - osys.walker(Rm).eloc()[0]) / (2 * h)
     np.testing.assert_allclose(f, -tot, rtol=5e-6, atol=5e-6)
+
+
+def test_deloc_dR_atom_subset_is_the_same_numbers():
+    sysm = qi.random_molecule(2, 3, 4, 4, seed=11)
+    w = oracle.OracleSystem(sysm).walker(qi.initial_positions(sysm, 0, [1])[0])
+    full = w.deloc_dR()
+    assert np.array_equal(w.deloc_dR([4, 0, 2]), full[[4, 0, 2]])
