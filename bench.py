@@ -366,7 +366,7 @@ def run_ours(args):
         msf2 = evs[0].elapsed_time(evs[1])
         flop2 = sum(2 * 2.0 * W * sysm.n_basis * n ** 2 + 2 * 2.0 * W * n ** 3 for n in (sysm.n_up, sysm.n_dn))
         f2["deloc_dR"] = dict(ms=msf2, gemm_tflops_lower_bound=flop2 / (msf2 * 1e-3) * 1e-12, max_abs=float(de.abs().max()),
-                              first_half_unchanged=bool(torch.equal(dl, dl2)),
+                              first_half_max_abs_diff=float((dl - dl2).abs().max()),
                               what="qmc_get_deloc_dR: eq. (4); per spin C A^-1 and C X (2 W N_b N_s^2 flop each), X = A^-1 B A^-1 "
                                    "(2 x 2 W N_s^3), per-atom contraction with third derivatives of the basis functions; both halves returned")
     # row f3 (outside the timed region): non-local pseudopotential energy of the whole crowd

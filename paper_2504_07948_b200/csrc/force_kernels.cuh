@@ -133,14 +133,16 @@ __global__ void __launch_bounds__(256, 4) k_force_prep(SysDev s, WalkDev wd, dou
 
 // grid (n_atoms, W), 128 threads.  spin 0 / 1: the trace terms of that spin (threads stride over its electrons);
 // with_rest: also - sum_i dgJ_i . G_i + sum_i dc_i + dV (all electrons, both spins).
+// acc_psi != nullptr: d ln|Psi| / d R_a (what k_dlogpsi computes) from the same radial sums, in the same order.
 __global__ void __launch_bounds__(128) k_deloc(SysDev s, WalkDev wd, int spin, const double* __restrict__ Mt, const double* __restrict__ Nt,
-                                               const double* __restrict__ fg, double* __restrict__ acc, int with_rest) {
-    __shared__ double red[3 * 4];
+                                               const double* __restrict__ fg, double* __restrict__ acc, double* __restrict__ acc_psi,
+                                               int with_rest) {
+    __shared__ double red[6 * 4];
     const int a = blockIdx.x, w = blockIdx.y, tid = threadIdx.x;
     const int ns = s.ns[spin], nsp = s.nsp[spin], nep = wd.nep, e0 = spin == 0 ? 0 : s.ns[0];
     const double* Rw = wd.R + (long)w * 3 * nep;
     const int sh0 = s.atom_shell_off[a], sh1 = s.atom_shell_off[a + 1];
-    double f3[3] = {0.0, 0.0, 0.0};
+    double f3[3] = {0.0, 0.0, 0.0}, p3[3] = {0.0, 0.0, 0.0};
     for (int p = tid; p < ns; p += 128) {
         const double rx = Rw[e0 + p], ry = Rw[nep + e0 + p], rz = Rw[2 * nep + e0 + p];
         const double* m = Mt + ((long)w * nsp + p) * s.nbp;
@@ -174,6 +176,9 @@ __global__ void __launch_bounds__(128) k_deloc(SysDev s, WalkDev wd, int spin, c
                 f3[0] += (k1 * Sx + k2 * x + k3 * jx + g * Hx) * cm + (g * Sx + tg1 * x) * cn;
                 f3[1] += (k1 * Sy + k2 * y + k3 * jy + g * Hy) * cm + (g * Sy + tg1 * y) * cn;
                 f3[2] += (k1 * Sz + k2 * z + k3 * jz + g * Hz) * cm + (g * Sz + tg1 * z) * cn;
+                p3[0] -= (g * Sx + tg1 * x) * cm;
+                p3[1] -= (g * Sy + tg1 * y) * cm;
+                p3[2] -= (g * Sz + tg1 * z) * cm;
             };
             const double s3 = 1.7320508075688772;
             if (rec.l == 0) {
@@ -206,6 +211,7 @@ __global__ void __launch_bounds__(128) k_deloc(SysDev s, WalkDev wd, int spin, c
             const double c1 = (u2 - u1 * ir) * ir * ir * xv + (0.5 * (u3 + 2.0 * u2 * ir - 2.0 * u1 * ir * ir) - Za * ir * ir) * ir;
             const double c2 = u1 * ir;
             f3[0] += c1 * dx + c2 * vx; f3[1] += c1 * dy + c2 * vy; f3[2] += c1 * dz + c2 * vz;
+            p3[0] -= c2 * dx; p3[1] -= c2 * dy; p3[2] -= c2 * dz;   // - u_en'(r) (r_i - R_a) / r
         }
         for (int bb = tid; bb < s.n_atoms; bb += 128) {
             if (bb == a) continue;
@@ -215,10 +221,15 @@ __global__ void __launch_bounds__(128) k_deloc(SysDev s, WalkDev wd, int spin, c
             f3[0] += c * yx; f3[1] += c * yy; f3[2] += c * yz;
         }
     }
-    block_sum<128, 3>(f3, red);
+    double f6[6] = {f3[0], f3[1], f3[2], p3[0], p3[1], p3[2]};
+    block_sum<128, 6>(f6, red);
     if (tid == 0) {
         double* o = acc + ((long)w * s.n_atoms + a) * 3;
-        o[0] += f3[0]; o[1] += f3[1]; o[2] += f3[2];
+        o[0] += f6[0]; o[1] += f6[1]; o[2] += f6[2];
+        if (acc_psi) {
+            double* q = acc_psi + ((long)w * s.n_atoms + a) * 3;
+            q[0] += f6[3]; q[1] += f6[4]; q[2] += f6[5];
+        }
     }
 }
 

@@ -986,12 +986,8 @@ cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double
             if (e != cudaSuccess) return e;
         }
         if (s.ns[sp] > 0 || sp == 0) {
-            k_deloc<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, sp, Mt, Nt, fg, acc_E, sp == 0 ? 1 : 0);
+            k_deloc<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, sp, Mt, Nt, fg, acc_E, acc_psi, sp == 0 ? 1 : 0);
             COUNT_LAUNCH();
-            if (acc_psi) {
-                k_dlogpsi<<<dim3(s.n_atoms, wd.W), 128, 0, st>>>(s, wd, sp, Mt, acc_psi, sp == 0 ? 1 : 0);
-                COUNT_LAUNCH();
-            }
         }
     }
     return cudaGetLastError();
@@ -1026,7 +1022,7 @@ cudaError_t launch_nl_evaluate(const SysDev& s, const WalkDev& wd, const NlArgs&
             if (e != cudaSuccess) return e;
             e = launch_mo(s, a.spin, wd.Phi, m, wd.V, wd.ldv, wd.mo_ws, wd.mo_flags, mo_grid_for(s, a.spin, m, n_sm), ++*mo_epoch, nullptr, st);
             if (e != cudaSuccess) return e;
-            k_nl_ratio<<<(m + 7) / 8, 256, 0, st>>>(s, wd, a, p0, m, wd.V);
+            k_nl_ratio<<<m, NL_RATIO_THREADS, 0, st>>>(s, wd, a, p0, m, wd.V);
             COUNT_LAUNCH();
         }
     }

@@ -77,7 +77,9 @@ def test_deloc_dR_matches_oracle(cfg, W, T, k, flags):
     osys = oracle.OracleSystem(sysm)
     assert de.shape == dp.shape == (W, sysm.n_atoms, 3)
     alone = qb.qmc_get_dlogpsi_dR(gw).cpu().numpy()
-    assert np.array_equal(alone, dp)                     # the shared C A^-1 product gives the first half unchanged
+    # the first half from the shared C A^-1 product and radial sums: the same numbers as the call of its own (to rounding:
+    # the two kernels contract their multiply-adds differently)
+    assert np.abs(alone - dp).max() <= 1e-12 * max(1.0, np.abs(alone).max())
     for n in range(W):
         ow = osys.walker(gpos[n])
         ref = ow.deloc_dR()
