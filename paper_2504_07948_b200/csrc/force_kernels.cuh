@@ -102,11 +102,7 @@ __global__ void __launch_bounds__(256, 4) k_force_prep(SysDev s, WalkDev wd, dou
     const int ns = s.ns[spin], nsp = s.nsp[spin], nep = wd.nep;
     const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
     const double* orb = wd.Orb[spin] + ((long)w * nsp + p) * 5 * nsp;
-    double gx = 0, gy = 0, gz = 0;
-    for (int j = lane; j < ns; j += 32) {
-        const double a = arow[j];
-        gx += orb[nsp + j] * a; gy += orb[2 * nsp + j] * a; gz += orb[3 * nsp + j] * a;
-    }
+    // the Jastrow gradient first (it does not need the row caches), then ONE pass over the cached rows for G_i and row i of B
     const double* Rw = wd.R + (long)w * 3 * nep;
     const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
     double jx = 0, jy = 0, jz = 0;
@@ -120,15 +116,20 @@ __global__ void __launch_bounds__(256, 4) k_force_prep(SysDev s, WalkDev wd, dou
             jx += wgt * dx; jy += wgt * dy; jz += wgt * dz;
         }
     }
-    gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz);
     jx = warp_sum(jx); jy = warp_sum(jy); jz = warp_sum(jz);
+    double* brow = (spin ? Bm1 : Bm0) + ((long)w * nsp + p) * nsp;
+    double gx = 0, gy = 0, gz = 0;
+    for (int j = lane; j < ns; j += 32) {
+        const double a = arow[j];
+        const double o1 = orb[nsp + j], o2 = orb[2 * nsp + j], o3 = orb[3 * nsp + j];
+        gx += o1 * a; gy += o2 * a; gz += o3 * a;
+        brow[j] = -0.5 * (orb[4 * nsp + j] + 2.0 * (jx * o1 + jy * o2 + jz * o3));
+    }
+    gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz);
     if (lane == 0) {
         double* o = fg + ((long)w * s.ne + e) * 8;
         o[0] = jx; o[1] = jy; o[2] = jz; o[3] = gx; o[4] = gy; o[5] = gz;
     }
-    double* brow = (spin ? Bm1 : Bm0) + ((long)w * nsp + p) * nsp;
-    for (int j = lane; j < ns; j += 32)
-        brow[j] = -0.5 * (orb[4 * nsp + j] + 2.0 * (jx * orb[nsp + j] + jy * orb[2 * nsp + j] + jz * orb[3 * nsp + j]));
 }
 
 // grid (n_atoms, W), 128 threads.  spin 0 / 1: the trace terms of that spin (threads stride over its electrons);
