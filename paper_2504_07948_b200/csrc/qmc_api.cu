@@ -239,6 +239,9 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
                         c[l]++;
                     }
             cnts[kb] = make_int4(c[0], c[1], c[2], off);
+            KbShell zero;
+            memset(&zero, 0, sizeof(zero));
+            list.resize(off + 32, zero);  // fixed 32 slots per block (a block of 32 functions has at most 32 shells)
         }
         if (list.empty()) { KbShell k; memset(&k, 0, sizeof(k)); list.push_back(k); }
         int4* dcn;

@@ -4,6 +4,8 @@
 
 #include <math.h>
 
+#include <type_traits>
+
 #include "gemm_f64.cuh"
 #include "mo_streamk.cuh"
 #include "device_utils.cuh"
@@ -46,22 +48,66 @@ __device__ __forceinline__ void bulk_s2g(void* gmem_dst, const void* smem_src, u
 }
 
 constexpr int BASIS_THREADS = 256;
+constexpr int BASIS_SLD = 14;  // doubles per staged shell record (12 + 2 of padding)
 // NC rows per point: 5 (value, gradient, Laplacian: the sweep) or 1 (values only: the quadrature points of row f3)
 template <int NC> constexpr int BASIS_MAXPT = (MO_BM + NC - 1) / NC + 1;  // points that can touch one 128-row tile (27 / 129)
+
+// exp(x) for the arguments of the primitives, x = -alpha t <= 0 (or NaN, which is returned).  The library exp spent
+// half of the kernel's instructions (ncu source page: about 65 per call, a third of them moves of its constants); this
+// one is 22: n = round(x log2 e) by the 1.5 * 2^52 trick, r = x - n ln 2 in two fused steps (ln 2 split hi + lo),
+// the Taylor polynomial of degree 13 on |r| <= ln 2 / 2 (remainder 4e-18), 2^n added into the exponent field.  Maximum
+// error measured against long-double exp on 2e7 arguments in [-708, 0]: 0.87 ulp (the library's bound is 1 ulp).
+// Below -708 the result (under 3e-308, the subnormal range) is 0.
+struct Exp3 {
+    double a, b, c;
+};
+__device__ __forceinline__ Exp3 exp_neg3(double xa, double xb, double xc) {
+    const double MAGIC = 6755399441055744.0, L2E = 1.4426950408889634, LN2_HI = 0.6931471805599453, LN2_LO = 2.3190468138462996e-17;
+    const double ta = fma(xa, L2E, MAGIC), tb = fma(xb, L2E, MAGIC), tc = fma(xc, L2E, MAGIC);
+    const double na = ta - MAGIC, nb = tb - MAGIC, nc = tc - MAGIC;
+    const double ra = fma(na, -LN2_LO, fma(na, -LN2_HI, xa)), rb = fma(nb, -LN2_LO, fma(nb, -LN2_HI, xb)), rc = fma(nc, -LN2_LO, fma(nc, -LN2_HI, xc));
+    constexpr double K[14] = {1.0, 1.0, 1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0, 1.0 / 362880.0,
+                              1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0};
+    double pa = K[13], pb = K[13], pc = K[13];
+#pragma unroll
+    for (int k = 12; k >= 0; k--) {  // three independent chains
+        pa = fma(pa, ra, K[k]);
+        pb = fma(pb, rb, K[k]);
+        pc = fma(pc, rc, K[k]);
+    }
+    Exp3 e;
+    e.a = __hiloint2double(__double2hiint(pa) + (__double2loint(ta) << 20), __double2loint(pa));
+    e.b = __hiloint2double(__double2hiint(pb) + (__double2loint(tb) << 20), __double2loint(pb));
+    e.c = __hiloint2double(__double2hiint(pc) + (__double2loint(tc) << 20), __double2loint(pc));
+    if (!(xa >= -708.0)) e.a = xa != xa ? xa : 0.0;
+    if (!(xb >= -708.0)) e.b = xb != xb ? xb : 0.0;
+    if (!(xc >= -708.0)) e.c = xc != xc ? xc : 0.0;
+    return e;
+}
 
 // Work items are (point, shell) pairs, ordered s-shells | p-shells | d-shells of the k-block, so a warp mixes
 // shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
 // stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
 // issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
+// The k-block's shell records (fixed 32 slots per block, so their load does not wait for the counts) are staged in
+// shared memory once per CTA.
 template <bool TMAX, int NC>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
 __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
                                                              double* __restrict__ tilemax) {
     __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
     __shared__ double spt[3 * BASIS_MAXPT<NC> + 3];
     __shared__ unsigned long long smax;  // bit pattern of a non-negative double: integer order = numeric order
+    // rows of 14 doubles: the 16-byte reads of eight neighbouring records fall into distinct banks
+    __shared__ __align__(16) double slist[32 * BASIS_SLD];
     if (threadIdx.x == 0) smax = 0ull;
     double vmax = 0.0;
     const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
+    const int4 cnt = s.kb_counts[kb];  // x, y, z = number of s, p, d shells of the block
+    static_assert(BASIS_THREADS >= 32 * 6, "one 16-byte piece of the shell list per thread");
+    if (tid < 32 * 6) {  // all 32 slots, whatever the counts
+        const int sh = tid / 6, j = tid - sh * 6;
+        reinterpret_cast<double2*>(slist + sh * BASIS_SLD)[j] = __ldg(reinterpret_cast<const double2*>(s.kb_list + kb * 32) + tid);
+    }
     const int row_lo = tm * MO_BM;
     const int pt_lo = row_lo / NC;
     int pt_hi = (row_lo + MO_BM + NC - 1) / NC;
@@ -77,8 +123,6 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
     }
     for (int i = tid; i < 3 * npt; i += BASIS_THREADS) spt[i] = pts[3 * pt_lo + i];
     __syncthreads();
-    const int4 cnt = s.kb_counts[kb];  // x, y, z = number of s, p, d shells; w = offset of this block's list
-    const KbShell* __restrict__ list = s.kb_list + cnt.w;
     const int r_base = pt_lo * NC - row_lo;
     const int n0 = npt * cnt.x, n1 = n0 + npt * cnt.y, n2 = n1 + npt * cnt.z;
     for (int q = tid; q < n2; q += BASIS_THREADS) {
@@ -87,11 +131,12 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
         else if (q < n1) { L = 1; qq = q - n0; c = cnt.y; base = cnt.x; }
         else { L = 2; qq = q - n1; c = cnt.z; base = cnt.x + cnt.y; }
         const int pi = qq / c;
-        const KbShell rec = list[base + qq - pi * c];
+        const KbShell rec = *reinterpret_cast<const KbShell*>(slist + (base + qq - pi * c) * BASIS_SLD);
         const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
         const double t = x * x + y * y + z * z;
         // accumulation order p = 0, 1, 2, ... as in the definition of g, g', g''
-        const double e0 = rec.c[0] * exp(-rec.a[0] * t), e1 = rec.c[1] * exp(-rec.a[1] * t), e2 = rec.c[2] * exp(-rec.a[2] * t);
+        const Exp3 ex = exp_neg3(-rec.a[0] * t, -rec.a[1] * t, -rec.a[2] * t);
+        const double e0 = rec.c[0] * ex.a, e1 = rec.c[1] * ex.b, e2 = rec.c[2] * ex.c;
         double g = e0, g1 = -(rec.a[0] * e0), g2 = rec.a[0] * rec.a[0] * e0;
         g += e1; g1 -= rec.a[1] * e1; g2 += rec.a[1] * rec.a[1] * e1;
         g += e2; g1 -= rec.a[2] * e2; g2 += rec.a[2] * rec.a[2] * e2;
@@ -106,31 +151,38 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
         const int c0 = rec.f0 - f_lo;
         const double lapfac = (double)(4 * L + 6) * g1 + 4.0 * t * g2;
         const double tg1 = 2.0 * g1;
-        auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
-            const int col = c0 + m;
-            if (col < 0 || col >= MO_BK) return;
-            const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
+        // CHK = false: shell and point lie wholly inside the stage (the usual case) -- stores at compile-time offsets
+        // from one address, no range tests; CHK = true: the edges of the stage
+        auto body = [&](auto CHK) {
+            constexpr bool chk = decltype(CHK)::value;
+            double* const t0 = tile + r0 * MO_ALD + c0;
+            auto emit = [&](int m, double S, double Sx, double Sy, double Sz) {
+                if (chk && (c0 + m < 0 || c0 + m >= MO_BK)) return;
+                const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
-            for (int k = 0; k < NC; k++)
-                if (r0 + k >= 0 && r0 + k < MO_BM) {
-                    tile[(r0 + k) * MO_ALD + col] = v[k];
-                    if (TMAX) vmax = fmax(vmax, v[k] == v[k] ? fabs(v[k]) : INFINITY);  // a NaN stage is never screened out
-                }
+                for (int k = 0; k < NC; k++)
+                    if (!chk || (r0 + k >= 0 && r0 + k < MO_BM)) {
+                        t0[k * MO_ALD + m] = v[k];
+                        if (TMAX) vmax = fmax(vmax, v[k] == v[k] ? fabs(v[k]) : INFINITY);  // a NaN stage is never screened out
+                    }
+            };
+            const double s3 = 1.7320508075688772;
+            if (L == 0) {
+                emit(0, 1.0, 0.0, 0.0, 0.0);
+            } else if (L == 1) {
+                emit(0, x, 1.0, 0.0, 0.0);
+                emit(1, y, 0.0, 1.0, 0.0);
+                emit(2, z, 0.0, 0.0, 1.0);
+            } else {
+                emit(0, s3 * x * y, s3 * y, s3 * x, 0.0);
+                emit(1, s3 * y * z, 0.0, s3 * z, s3 * y);
+                emit(2, z * z - 0.5 * (x * x + y * y), -x, -y, 2.0 * z);
+                emit(3, s3 * x * z, s3 * z, 0.0, s3 * x);
+                emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
+            }
         };
-        const double s3 = 1.7320508075688772;
-        if (L == 0) {
-            emit(0, 1.0, 0.0, 0.0, 0.0);
-        } else if (L == 1) {
-            emit(0, x, 1.0, 0.0, 0.0);
-            emit(1, y, 0.0, 1.0, 0.0);
-            emit(2, z, 0.0, 0.0, 1.0);
-        } else {
-            emit(0, s3 * x * y, s3 * y, s3 * x, 0.0);
-            emit(1, s3 * y * z, 0.0, s3 * z, s3 * y);
-            emit(2, z * z - 0.5 * (x * x + y * y), -x, -y, 2.0 * z);
-            emit(3, s3 * x * z, s3 * z, 0.0, s3 * x);
-            emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
-        }
+        if (r0 >= 0 && r0 + NC <= MO_BM && c0 >= 0 && c0 + 2 * L + 1 <= MO_BK) body(std::false_type{});
+        else body(std::true_type{});
     }
     if (TMAX) {
 #pragma unroll
