@@ -58,6 +58,8 @@ template <int NC> constexpr int BASIS_MAXPT = (MO_BM + NC - 1) / NC + 1;  // poi
 // the Taylor polynomial of degree 13 on |r| <= ln 2 / 2 (remainder 4e-18), 2^n added into the exponent field.  Maximum
 // error measured against long-double exp on 2e7 arguments in [-708, 0]: 0.87 ulp (the library's bound is 1 ulp).
 // Below -708 the result (under 3e-308, the subnormal range) is 0.
+__constant__ double EXP_TAYLOR[14] = {1.0, 1.0, 1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0, 1.0 / 362880.0,
+                                        1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0};  // 1 / k!
 struct Exp3 {
     double a, b, c;
 };
@@ -66,8 +68,7 @@ __device__ __forceinline__ Exp3 exp_neg3(double xa, double xb, double xc) {
     const double ta = fma(xa, L2E, MAGIC), tb = fma(xb, L2E, MAGIC), tc = fma(xc, L2E, MAGIC);
     const double na = ta - MAGIC, nb = tb - MAGIC, nc = tc - MAGIC;
     const double ra = fma(na, -LN2_LO, fma(na, -LN2_HI, xa)), rb = fma(nb, -LN2_LO, fma(nb, -LN2_HI, xb)), rc = fma(nc, -LN2_LO, fma(nc, -LN2_HI, xc));
-    constexpr double K[14] = {1.0, 1.0, 1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0, 1.0 / 362880.0,
-                              1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0};
+    const double* K = EXP_TAYLOR;  // constant-bank operands of the DFMAs
     double pa = K[13], pb = K[13], pc = K[13];
 #pragma unroll
     for (int k = 12; k >= 0; k--) {  // three independent chains
@@ -125,12 +126,16 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
     __syncthreads();
     const int r_base = pt_lo * NC - row_lo;
     const int n0 = npt * cnt.x, n1 = n0 + npt * cnt.y, n2 = n1 + npt * cnt.z;
+    const float icx = 1.0f / (float)cnt.x, icy = 1.0f / (float)cnt.y, icz = 1.0f / (float)cnt.z;  // a count of 0: never used
     for (int q = tid; q < n2; q += BASIS_THREADS) {
         int L, qq, c, base;
-        if (q < n0) { L = 0; qq = q; c = cnt.x; base = 0; }
-        else if (q < n1) { L = 1; qq = q - n0; c = cnt.y; base = cnt.x; }
-        else { L = 2; qq = q - n1; c = cnt.z; base = cnt.x + cnt.y; }
-        const int pi = qq / c;
+        float ic;
+        if (q < n0) { L = 0; qq = q; c = cnt.x; ic = icx; base = 0; }
+        else if (q < n1) { L = 1; qq = q - n0; c = cnt.y; ic = icy; base = cnt.x; }
+        else { L = 2; qq = q - n1; c = cnt.z; ic = icz; base = cnt.x + cnt.y; }
+        // qq / c without the 45-instruction integer division: c <= 32 and qq < 129 * 32, so (qq + 1/2) / c is at least
+        // 1 / 64 away from an integer and the float product (error below 1e-3) truncates to the quotient
+        const int pi = (int)(((float)qq + 0.5f) * ic);
         const KbShell rec = *reinterpret_cast<const KbShell*>(slist + (base + qq - pi * c) * BASIS_SLD);
         const double x = spt[3 * pi] - rec.x, y = spt[3 * pi + 1] - rec.y, z = spt[3 * pi + 2] - rec.z;
         const double t = x * x + y * y + z * z;

@@ -60,6 +60,36 @@ def test_basis_and_mo_rows(cfg, npts):
             assert np.abs(M[n] - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
+def test_basis_values_elementwise_near_and_far():
+    # The basis kernel has its own exp (arguments <= 0, zero below -708).  The value of a function is S * g with g a sum of
+    # positive terms, so it has no cancellation and must agree with the oracle (libm exp) element by element to a few ulp --
+    # near the atoms, and far out where the tight primitives underflow (alpha t up to 1e5) and the diffuse ones are 1e-100.
+    s = qi.make_system(1)
+    g = qb.qmc_init_from(s)
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(11)
+    near = s.atoms_xyz[rng.integers(0, s.n_atoms, 12)] + rng.standard_normal((12, 3)) * 0.7
+    on_atom = s.atoms_xyz[[0, 5]]                                   # t = 0 for the shells of that atom: exp(-0) = 1 exactly
+    far = s.atoms_xyz.mean(axis=0) + rng.standard_normal((10, 3)) * np.array([[8.0], [20.0], [40.0], [60.0], [90.0]]).repeat(2, axis=0)
+    pts = np.concatenate([near, on_atom, far])
+    B = qb.qmc_eval_basis(g, pts).cpu().numpy()
+    assert np.isfinite(B).all()
+    worst = 0.0
+    # functions of a shell in order (2l + 1 each); the scale of a shell's values is its largest component (one d component
+    # is a difference of squares and may itself be near zero)
+    f0 = np.concatenate([[0], np.cumsum(2 * s.shell_l + 1)])
+    for n in range(len(pts)):
+        phi, gr, lap = o.basis_eval(pts[n])
+        scale = np.concatenate([np.full(2 * l + 1, np.abs(phi[f0[i]:f0[i + 1]]).max()) for i, l in enumerate(s.shell_l)])
+        big = scale > 1e-290
+        if big.any():
+            worst = max(worst, (np.abs(B[n, 0][big] - phi[big]) / scale[big]).max())
+        assert np.abs(B[n, 0][~big] - phi[~big]).max(initial=0.0) < 1e-289
+        ref = np.concatenate([phi[None], gr, lap[None]])
+        assert np.abs(B[n] - ref).max() <= 1e-13 * max(np.abs(ref).max(), 1e-300)
+    assert worst < 2e-14, worst   # about 90 ulp would already fail; measured 1e-15
+
+
 def test_mo_contraction_ragged_tiles():
     # 300 points x 5 rows = 1500 rows: several 128-row tiles and a ragged tail; N_s = 128, K = 768
     s = qi.make_system(1)
