@@ -74,20 +74,25 @@ def test_basis_values_elementwise_near_and_far():
     pts = np.concatenate([near, on_atom, far])
     B = qb.qmc_eval_basis(g, pts).cpu().numpy()
     assert np.isfinite(B).all()
-    worst = 0.0
-    # functions of a shell in order (2l + 1 each); the scale of a shell's values is its largest component (one d component
-    # is a difference of squares and may itself be near zero)
+    # Functions of a shell in order (2l + 1 each).  The scale of a shell's entries is its largest one (a d component is a
+    # difference of squares and may itself be near zero).  exp(x) carries the rounding of its argument, |x| eps with
+    # x = -alpha t, and |x| is about |ln scale|: the bound grows with the depth of the tail.
+    eps = 2.0 ** -52
     f0 = np.concatenate([[0], np.cumsum(2 * s.shell_l + 1)])
+    worst = 0.0
     for n in range(len(pts)):
         phi, gr, lap = o.basis_eval(pts[n])
-        scale = np.concatenate([np.full(2 * l + 1, np.abs(phi[f0[i]:f0[i + 1]]).max()) for i, l in enumerate(s.shell_l)])
-        big = scale > 1e-290
-        if big.any():
-            worst = max(worst, (np.abs(B[n, 0][big] - phi[big]) / scale[big]).max())
-        assert np.abs(B[n, 0][~big] - phi[~big]).max(initial=0.0) < 1e-289
         ref = np.concatenate([phi[None], gr, lap[None]])
-        assert np.abs(B[n] - ref).max() <= 1e-13 * max(np.abs(ref).max(), 1e-300)
-    assert worst < 2e-14, worst   # about 90 ulp would already fail; measured 1e-15
+        for comps, slack in ((slice(0, 1), 4.0), (slice(0, 5), 32.0)):   # values alone; then all five components
+            sc = np.concatenate([np.full(2 * l + 1, np.abs(ref[comps, f0[i]:f0[i + 1]]).max()) for i, l in enumerate(s.shell_l)])
+            big = sc > 1e-290
+            err = np.abs(B[n, comps] - ref[comps])
+            assert err[:, ~big].max(initial=0.0) < 1e-288
+            tol = eps * slack * (4.0 + np.abs(np.log(sc[big]))) * sc[big]
+            ratio = (err[:, big] / tol).max(initial=0.0)
+            worst = max(worst, ratio)
+            assert ratio < 1.0, (n, ratio)
+    print("worst error / bound:", worst)  # 0.47 measured on B200
 
 
 def test_mo_contraction_ragged_tiles():
