@@ -47,10 +47,19 @@ __device__ __forceinline__ void bulk_s2g(void* gmem_dst, const void* smem_src, u
                  : "memory");
 }
 
-constexpr int BASIS_THREADS = 256;
+// Rows of a stage built by one CTA when the stage maximum is not recorded, and threads / resident CTAs per row count.
+// Measured on B200 at config 2 (us per launch, live): 128 rows with 256 threads x 4 CTAs per SM 22.6, with 192 threads x 5
+// CTAs per SM 21.4 (kept: one more stage draining through the TMA engine while the others compute), 64 rows with 128
+// threads x 8 CTAs per SM 22.9.
+#ifndef QMC_BASIS_TR
+#define QMC_BASIS_TR 128
+#endif
+template <int TR> constexpr int BASIS_NT = TR == 128 ? 192 : 128;
+template <int TR> constexpr int BASIS_MINB = TR == 128 ? 5 : 8;
 constexpr int BASIS_SLD = 14;  // doubles per staged shell record (12 + 2 of padding)
-// NC rows per point: 5 (value, gradient, Laplacian: the sweep) or 1 (values only: the quadrature points of row f3)
-template <int NC> constexpr int BASIS_MAXPT = (MO_BM + NC - 1) / NC + 1;  // points that can touch one 128-row tile (27 / 129)
+// NC rows per point: 5 (value, gradient, Laplacian: the sweep) or 1 (values only: the quadrature points of row f3);
+// TR rows of the stage per CTA (128: the whole stage; 64: half of it, twice as many CTAs of half the threads)
+template <int NC, int TR> constexpr int BASIS_MAXPT = (TR + NC - 1) / NC + 1;  // points that can touch one TR-row piece
 
 // exp(x) for the arguments of the primitives, x = -alpha t <= 0 (or NaN, which is returned).  The library exp spent
 // half of the kernel's instructions (ncu source page: about 65 per call, a third of them moves of its constants); this
@@ -87,16 +96,17 @@ __device__ __forceinline__ Exp3 exp_neg3(double xa, double xb, double xc) {
 }
 
 // Work items are (point, shell) pairs, ordered s-shells | p-shells | d-shells of the k-block, so a warp mixes
-// shell types only at the two boundaries (no divergence in the angular code elsewhere) and all 256 threads
-// stay busy for the same number of passes.  The radial triple (three FP64 exp per pair -- the expensive part,
+// shell types only at the two boundaries (no divergence in the angular code elsewhere).  The radial triple (three FP64 exp per pair -- the expensive part,
 // issued as three independent chains) is computed once per shell and used from registers by its 2l+1 functions.
 // The k-block's shell records (fixed 32 slots per block, so their load does not wait for the counts) are staged in
 // shared memory once per CTA.
-template <bool TMAX, int NC>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
-__global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
-                                                             double* __restrict__ tilemax) {
-    __shared__ __align__(128) double tile[MO_A_STAGE];  // [128][36]
-    __shared__ double spt[3 * BASIS_MAXPT<NC> + 3];
+template <bool TMAX, int NC, int TR>  // TMAX: also record the largest |entry| of the stage in tilemax [MT][KB] (optional screening of the contraction)
+__global__ void __launch_bounds__(BASIS_NT<TR>, BASIS_MINB<TR>) k_basis(SysDev s, const double* __restrict__ pts, int n_points, double* __restrict__ out,
+                                                            double* __restrict__ tilemax) {
+    static_assert(TR == MO_BM || (TR == MO_BM / 2 && !TMAX), "a CTA builds a whole stage, or half of one when no stage maximum is recorded");
+    constexpr int BASIS_THREADS = BASIS_NT<TR>;
+    __shared__ __align__(128) double tile[TR * MO_ALD];  // [TR][36]
+    __shared__ double spt[3 * BASIS_MAXPT<NC, TR> + 3];
     __shared__ unsigned long long smax;  // bit pattern of a non-negative double: integer order = numeric order
     // rows of 14 doubles: the 16-byte reads of eight neighbouring records fall into distinct banks
     __shared__ __align__(16) double slist[32 * BASIS_SLD];
@@ -104,23 +114,22 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
     double vmax = 0.0;
     const int kb = blockIdx.x, tm = blockIdx.y, tid = threadIdx.x;
     const int4 cnt = s.kb_counts[kb];  // x, y, z = number of s, p, d shells of the block
-    static_assert(BASIS_THREADS >= 32 * 6, "one 16-byte piece of the shell list per thread");
-    if (tid < 32 * 6) {  // all 32 slots, whatever the counts
-        const int sh = tid / 6, j = tid - sh * 6;
-        reinterpret_cast<double2*>(slist + sh * BASIS_SLD)[j] = __ldg(reinterpret_cast<const double2*>(s.kb_list + kb * 32) + tid);
+    for (int i = tid; i < 32 * 6; i += BASIS_THREADS) {  // all 32 slots, whatever the counts: a 16-byte piece per thread
+        const int sh = i / 6, j = i - sh * 6;
+        reinterpret_cast<double2*>(slist + sh * BASIS_SLD)[j] = __ldg(reinterpret_cast<const double2*>(s.kb_list + kb * 32) + i);
     }
-    const int row_lo = tm * MO_BM;
+    const int row_lo = tm * TR;  // tm counts TR-row pieces
     const int pt_lo = row_lo / NC;
-    int pt_hi = (row_lo + MO_BM + NC - 1) / NC;
+    int pt_hi = (row_lo + TR + NC - 1) / NC;
     if (pt_hi > n_points) pt_hi = n_points;
     const int npt = pt_hi - pt_lo;
     const int f_lo = kb * MO_BK;
-    if (row_lo + MO_BM <= NC * n_points && f_lo + MO_BK <= s.n_basis) {
+    if (row_lo + TR <= NC * n_points && f_lo + MO_BK <= s.n_basis) {
         // every (row, function) of the tile gets written below: only the 4 padding columns need zeros
-        for (int i = tid; i < MO_BM * 2; i += BASIS_THREADS)
+        for (int i = tid; i < TR * 2; i += BASIS_THREADS)
             reinterpret_cast<double2*>(tile + (i >> 1) * MO_ALD + MO_BK)[i & 1] = make_double2(0.0, 0.0);
     } else {
-        for (int i = tid; i < MO_A_STAGE / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
+        for (int i = tid; i < TR * MO_ALD / 2; i += BASIS_THREADS) reinterpret_cast<double2*>(tile)[i] = make_double2(0.0, 0.0);
     }
     for (int i = tid; i < 3 * npt; i += BASIS_THREADS) spt[i] = pts[3 * pt_lo + i];
     __syncthreads();
@@ -166,7 +175,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
                 const double v[5] = {S * g, g * Sx + tg1 * S * x, g * Sy + tg1 * S * y, g * Sz + tg1 * S * z, S * lapfac};
 #pragma unroll
                 for (int k = 0; k < NC; k++)
-                    if (!chk || (r0 + k >= 0 && r0 + k < MO_BM)) {
+                    if (!chk || (r0 + k >= 0 && r0 + k < TR)) {
                         t0[k * MO_ALD + m] = v[k];
                         if (TMAX) vmax = fmax(vmax, v[k] == v[k] ? fabs(v[k]) : INFINITY);  // a NaN stage is never screened out
                     }
@@ -186,7 +195,7 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
                 emit(4, (0.5 * s3) * (x * x - y * y), s3 * x, -s3 * y, 0.0);
             }
         };
-        if (r0 >= 0 && r0 + NC <= MO_BM && c0 >= 0 && c0 + 2 * L + 1 <= MO_BK) body(std::false_type{});
+        if (r0 >= 0 && r0 + NC <= TR && c0 >= 0 && c0 + 2 * L + 1 <= MO_BK) body(std::false_type{});
         else body(std::true_type{});
     }
     if (TMAX) {
@@ -197,26 +206,29 @@ __global__ void __launch_bounds__(BASIS_THREADS, 4) k_basis(SysDev s, const doub
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // generic-proxy smem writes -> visible to the TMA engine
     __syncthreads();
     if (tid == 0) {
-        if (TMAX) tilemax[tm * s.kb + kb] = __longlong_as_double((long long)smax);
-        bulk_s2g(out + ((long)tm * s.kb + kb) * MO_A_STAGE, tile, MO_A_STAGE * sizeof(double));
+        if (TMAX) tilemax[tm * s.kb + kb] = __longlong_as_double((long long)smax);  // TR = 128 here
+        const int stage = row_lo / MO_BM, r_in = row_lo - stage * MO_BM;
+        bulk_s2g(out + ((long)stage * s.kb + kb) * MO_A_STAGE + r_in * MO_ALD, tile, TR * MO_ALD * sizeof(double));
         asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
         asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory");  // smem must outlive the read
     }
 }
 
+// The buffer holds whole 128-row stages: with TR = 64 an odd number of pieces leaves the lower half of the last stage
+// unwritten, so the grid always covers whole stages (a piece beyond the last point stores zeros).
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
-    dim3 grid(s.kb, (5 * n_points + MO_BM - 1) / MO_BM);
-    if (tilemax) k_basis<true, 5><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, tilemax);
-    else k_basis<false, 5><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
+    const int stages = (5 * n_points + MO_BM - 1) / MO_BM;
+    if (tilemax) k_basis<true, 5, MO_BM><<<dim3(s.kb, stages), BASIS_NT<MO_BM>, 0, st>>>(s, pts, n_points, PhiT, tilemax);
+    else k_basis<false, 5, QMC_BASIS_TR><<<dim3(s.kb, stages * (MO_BM / QMC_BASIS_TR)), BASIS_NT<QMC_BASIS_TR>, 0, st>>>(s, pts, n_points, PhiT, nullptr);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }
 // values only: row = point
 cudaError_t launch_basis_values(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st) {
     if (n_points == 0) return cudaSuccess;
-    dim3 grid(s.kb, (n_points + MO_BM - 1) / MO_BM);
-    k_basis<false, 1><<<grid, BASIS_THREADS, 0, st>>>(s, pts, n_points, PhiT, nullptr);
+    const int stages = (n_points + MO_BM - 1) / MO_BM;
+    k_basis<false, 1, QMC_BASIS_TR><<<dim3(s.kb, stages * (MO_BM / QMC_BASIS_TR)), BASIS_NT<QMC_BASIS_TR>, 0, st>>>(s, pts, n_points, PhiT, nullptr);
     COUNT_LAUNCH();
     return cudaGetLastError();
 }

@@ -250,19 +250,22 @@ def test_resume_is_bitwise():
 def test_delay_invariance_and_walker_prefix():
     wl = qi.make_workload(1)
     ref = _run_gpu(wl, 0, 16, 3, 1)
+    # two GPU runs, each held to the BASELINE.json tolerance against the oracle elsewhere, are compared with EACH OTHER
+    # here: by the triangle inequality they may differ by twice that tolerance (the same mathematics summed in another
+    # order -- the rank-k flush groups the updates differently for every k)
     for k in (4, 16, 32, 64, 128):
         got = _run_gpu(wl, 0, 16, 3, k)
         assert np.array_equal(got[0] & 1, ref[0] & 1), f"accept bits differ at delay_k={k}"
-        assert np.abs(got[1] - ref[1]).max() < TOL_POS
-        assert np.abs(got[2] - ref[2]).max() < TOL_ELOC
-        assert max(rel_frob(got[3][n], ref[3][n]) for n in range(16)) < TOL_AINV
+        assert np.abs(got[1] - ref[1]).max() < 2 * TOL_POS
+        assert np.abs(got[2] - ref[2]).max() < 2 * TOL_ELOC
+        assert max(rel_frob(got[3][n], ref[3][n]) for n in range(16)) < 2 * TOL_AINV
     # walkers 5..10 alone == the same walkers inside the larger crowd (A20): same decisions; positions to rounding only,
     # because where the stream-K contraction cuts the K range of a tile depends on how many rows the crowd has
     sub = _run_gpu(wl, 5, 11, 3, 32)
     big = _run_gpu(wl, 0, 16, 3, 32)
     assert np.array_equal(sub[0] & 1, big[0][:, :, 5:11] & 1)
-    assert np.abs(sub[1] - big[1][5:11]).max() < TOL_POS
-    assert np.abs(sub[2] - big[2][5:11]).max() < TOL_ELOC
+    assert np.abs(sub[1] - big[1][5:11]).max() < 2 * TOL_POS
+    assert np.abs(sub[2] - big[2][5:11]).max() < 2 * TOL_ELOC
 
 
 # ------------------------------------------------------------------ ABI behaviour
@@ -355,7 +358,10 @@ def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None):
                 assert (gb[d[0]] | ob[d[0]]) & 2, f"unflagged mismatch cfg {cfg} walker {w} sweep {t} electron {d[0]}"
                 break
             m = np.abs(orat[:hi]) >= RATIO_SMALL
-            worst["ratio"] = max(worst["ratio"], float(np.max(np.abs(ratio[t, :hi, w][m] - orat[:hi][m]) / np.abs(orat[:hi][m]))))
+            rel = np.where(m, np.abs(ratio[t, :hi, w] - orat[:hi]) / np.maximum(np.abs(orat[:hi]), RATIO_SMALL), 0.0)
+            if rel.max() > worst["ratio"]:
+                worst["ratio"] = float(rel.max())
+                worst["ratio_at"] = dict(walker=int(w), sweep=t, electron=int(rel.argmax()), oracle_ratio=float(orat[rel.argmax()]))
         else:
             if n_elec_checked is None:
                 worst["pos"] = max(worst["pos"], float(np.abs(pos[w] - ow.positions()).max()))
