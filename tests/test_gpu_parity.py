@@ -321,7 +321,7 @@ def test_device_and_host_buffers_agree():
 
 # ------------------------------------------------------------------ full-size configs (sampled)
 
-def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None):
+def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None, cond_spin=None):
     """Full crowd of a large config on the GPU in the bench launch configuration; the oracle (double and long
     double) runs the sampled walkers.  n_elec_checked limits the comparison to the first electrons of sweep 0."""
     wl = qi.make_workload(cfg, n_walkers=n_walkers)
@@ -346,7 +346,11 @@ def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None):
         rows = []
         for t in range(T if n_elec_checked is None else 1):
             rows.append(ow.sweep_range(wl.seed, w, t, wl.tau, 0, hi))
+        if cond_spin is not None:  # 2-norm condition number of the walker's Slater matrix, from the oracle's own inverse
+            sv = np.linalg.svd(ow.Ainv(cond_spin), compute_uv=False)
+            cond[w] = float(sv[0] / sv[-1])
         return w, ow, rows
+    cond = {}
     with ThreadPoolExecutor(max_workers=oracle.default_threads()) as ex:
         res = list(ex.map(one, sample))
     worst = dict(ratio=0.0, pos=0.0, eloc=0.0)
@@ -367,6 +371,8 @@ def _full_size_sampled(cfg, sample, T, n_elec_checked=None, n_walkers=None):
                 worst["pos"] = max(worst["pos"], float(np.abs(pos[w] - ow.positions()).max()))
                 worst["eloc"] = max(worst["eloc"], abs(el[w] - ow.eloc()[0]))
     out.update(worst)
+    if cond:
+        out["cond"] = cond
     return out
 
 
@@ -383,8 +389,13 @@ def test_config2_full_crowd_sampled_walkers():
 def test_config3_full_crowd_first_electrons():
     # fragment config exactly as configs[3] states it (64 walkers, 4096 electrons, delay_k 128); three sampled walkers,
     # first 192 electrons of sweep 0 against the oracle (about two minutes of oracle time on the GPU box's host cores)
-    worst = _full_size_sampled(3, [0, 31, 63], 1, n_elec_checked=192)
-    assert worst["ratio"] < 10 * TOL_RATIO, worst
+    # Conditioning (reading A26, DESIGN.md section 6 item 3): two correct FP64 evaluations of a ratio differ by about
+    # cond(A) 2^-53 each from the exact one.  At N_s = 2048 the sampled walkers reach cond(A) = 1.3e7 (walker 63, spin up:
+    # 1.5e-9), above the 1e-9 that holds at N_s = 1024, so the bound is the larger of the two, with cond(A) taken from the
+    # oracle's own inverse of the walker on which the worst error sits (the 192 electrons checked are all spin up).
+    worst = _full_size_sampled(3, [0, 31, 63], 1, n_elec_checked=192, cond_spin=0)
+    cond_at = worst["cond"][worst["ratio_at"]["walker"]] if "ratio_at" in worst else 0.0
+    assert worst["ratio"] < max(10 * TOL_RATIO, 2 * cond_at * 2.0 ** -53), worst
 
 
 def test_config3_mo_rows_full_size():
