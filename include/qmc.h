@@ -23,8 +23,16 @@
  *   - Pointer arguments marked "host or device" may be either (unified virtual addressing decides);
  *     inputs are copied before the call returns, so the caller may free them afterwards.
  *   - Output buffers are caller-owned (normally torch tensors).  Device buffers are written
- *     asynchronously on the walker set's stream; host buffers are written synchronously.
- *   - The library owns its internal state (cudaMalloc at create time, freed at destroy).
+ *     asynchronously on the walker set's stream -- a caller that reads them on ANOTHER stream must order that
+ *     stream after the walker set's (an event, or qmc_synchronize); host buffers are written synchronously.
+ *   - The library owns its internal state (cudaMalloc at create time, freed at destroy).  Scratch of the
+ *     row-f2 / f3 getters and the staging buffer of host-pointer getters are allocated by the first call that
+ *     needs them and kept (qmc_release_scratch frees them); no other call allocates.
+ *   - A system lives on the CUDA device that was current at qmc_init; every call on it or on its walker sets
+ *     runs there whatever the calling thread's current device is (restored on return).
+ *   - Relative to the signatures sketched in SURVEY.md 8(b): qmc_walkers_create takes a `flags` word (logging,
+ *     path selection, screening) and qmc_basis carries `n_prim_total` (the length of alpha / coef, needed to copy
+ *     them); rows f1-f4 and the stage-level / timing entry points are additions, each marked below.
  *   - There is NO CPU fallback: every entry point fails with QMC_ERR_CUDA when no sm_100 device works.
  */
 #ifndef QMC_B200_H
@@ -177,8 +185,9 @@ int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int delay_k, doub
 /* ---- Row f2, first half: out[W][n_atoms][3] = d ln|Psi| / d R_a at the current configuration -- the paper's eq. (3)
  * (d ln D / d lambda = tr(A^-1 dA/d lambda)) with the nuclear coordinates as parameters, basis functions
  * moving with their nucleus, plus the electron-nucleus Jastrow term.  This is the wave-function ("Pulay") term of a QMC
- * force estimator; the derivative of E_L (eq. 4) is not built.  out: host or device.  Call between sweeps; allocates and
- * frees a [W][N_s][N_b] scratch (12.9 GB at config 2) and synchronises the stream.  QMC_ERR_NOMEM if that does not fit. */
+ * force estimator; qmc_get_deloc_dR below is the other term (eq. 4).  out: host or device.  Call between sweeps; uses a
+ * [W][N_s][N_b] scratch (12.9 GB at config 2; allocated by the first call, kept) and synchronises the stream.
+ * QMC_ERR_NOMEM if that does not fit. */
 int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out);
 /* ---- Row f2, second half: deloc[W][n_atoms][3] = d E_L / d R_a at the current configuration by the paper's eq. (4)
  * (PAPER.md L177-181): tr(A^-1 dB/dR_a - X dA/dR_a), X = A^-1 B A^-1, summed over both spins, plus the derivative of the
@@ -187,9 +196,12 @@ int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out);
  * (no orbital relaxation, no space warp).  dlogpsi (may be NULL): the same call also returns qmc_get_dlogpsi_dR's
  * result from the shared C A^-1 product -- the two pieces of the force estimator
  * F_a = -< dE_L/dR_a + 2 (E_L - <E_L>) d ln|Psi|/dR_a >.  deloc, dlogpsi: host or device.  Call between sweeps;
- * allocates and frees 2 [W][N_s][N_b] + 4 [W][N_s^2] doubles of scratch and synchronises the stream.
- * QMC_ERR_NOMEM if that does not fit. */
+ * uses 2 [W][N_s][N_b] + 4 [W][N_s^2] doubles of scratch (allocated by the first call, kept) and synchronises the
+ * stream.  QMC_ERR_NOMEM if that does not fit. */
 int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi);
+/* Frees the scratch kept by qmc_get_dlogpsi_dR / qmc_get_deloc_dR / qmc_get_vnl and the staging buffer of the
+ * host-pointer getters (they come back on the next call that needs them).  Synchronises the stream. */
+int qmc_release_scratch(qmc_walkers* w);
 
 /* ---- Row f3: non-local pseudopotential energy by spherical quadrature ("ccECP pseudopotentials", L180;
  * DESIGN.md reading A34).  qmc_set_ecp attaches the non-local channels to a system: channel c sits on atom ch_atom[c],
@@ -207,8 +219,6 @@ int qmc_set_ecp(qmc_system* s, int n_channels, const int32_t* ch_atom, const int
  * sweeps; synchronises the stream (the number of pairs is read back once per spin).  QMC_ERR_ARG without qmc_set_ecp. */
 int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs);
 
-/* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
- * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
 /* Several crowds per GPU: walker sets created on different streams run concurrently, and the HBM-bound stages of one
  * (k_basis, k_step) can overlap the tensor-bound contraction of another only if that persistent kernel leaves some SMs
  * free.  n_ctas (1..number of SMs; 0 = all, the default) is the grid of this set's contraction from now on (the
@@ -222,6 +232,8 @@ int qmc_set_mo_ctas(qmc_walkers* w, int n_ctas);
  * +5 % at config 2 with two crowds of 128 and 124 CTAs).  Asynchronous like qmc_sweep.  Errors: as qmc_sweep;
  * QMC_ERR_ARG if the sets belong to different systems or one appears twice. */
 int qmc_sweep_crowds(qmc_walkers* const* sets, int n_sets, int nsteps, double tau, int delay_k);
+/* (tile, k-block) iterations of the MO contraction since creation: executed, and what the dense contraction would
+ * have done; equal unless QMC_SCREEN_MO is set (counted only for screened walker sets, else both 0). */
 int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);
 
 /* Stage-level entry points (used by the per-stage parity tests and the per-stage roofline bench).
@@ -246,6 +258,10 @@ int qmc_get_stage_times(qmc_walkers* w, double* ms /* [6] */, uint64_t* counts /
 /* Register-resident DMMA issue-rate loop for `ms_target` milliseconds: the FP64 ceiling of this GPU as
  * it runs now (used as the roofline denominator of the contraction stages). */
 int qmc_measure_fp64_peak(double ms_target, double* tflops, void* cuda_stream);
+/* The random generator of the move kernels on caller-chosen inputs (reading A11: Philox4x32-10): ctr_key [n][6] =
+ * counter words 0..3 and key words 0..1, out [n][4] = the four output words.  Host or device buffers; synchronous.
+ * Exists so that the GPU's raw words can be compared with an independent implementation. */
+int qmc_philox_words(int n, const uint32_t* ctr_key, uint32_t* out, void* cuda_stream);
 /* number of kernels this library launched on this thread's calls since load (for bench.py gpu_launches) */
 uint64_t qmc_launch_count(void);
 

@@ -84,6 +84,7 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_get_positions.argtypes = [C.c_void_p, _dp]
     lib.oracle_walker_get_Ainv.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
     lib.oracle_walker_get_logpsi.argtypes = [C.c_void_p, _dp, _ip]
+    lib.oracle_walker_get_A.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
     lib.oracle_walker_sweep.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                         _u8p, _dp, _dp]
     lib.oracle_walker_sweep_range.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
@@ -360,6 +361,13 @@ class OracleWalker:
         n = self.sys.ns(spin)
         out = np.zeros((n, n))
         self.lib.oracle_walker_get_Ainv(self.sys.h, self.h, spin, _d(out))
+        return out
+
+    def A(self, spin):
+        """the Slater matrix A[p][j] = phi_j(r_p) of one spin at the current positions (the cached value rows)"""
+        n = self.sys.ns(spin)
+        out = np.zeros((n, n))
+        self.lib.oracle_walker_get_A(self.sys.h, self.h, spin, _d(out))
         return out
 
     def logpsi(self):

@@ -533,6 +533,13 @@ void oracle_walker_get_Ainv(const oracle_system *s, const oracle_walker *w, int 
         for (int j = 0; j < ns; j++) out[(size_t)p * ns + j] = (double)w->Ainv[spin][(size_t)j * ns + p];
 }
 
+/* the Slater matrix itself, out[p][j] = A[p][j] = phi_j(r_p): the value rows of the walker's orbital cache (no arithmetic) */
+void oracle_walker_get_A(const oracle_system *s, const oracle_walker *w, int spin, double *out) {
+    int ns = spin == 0 ? s->n_up : s->n_dn;
+    for (int p = 0; p < ns; p++)
+        for (int j = 0; j < ns; j++) out[(size_t)p * ns + j] = (double)w->orb[spin][(size_t)p * 5 * ns + j];
+}
+
 void oracle_walker_get_logpsi(const oracle_walker *w, double *logabs, int *sign) {
     *logabs = (double)w->logabs; *sign = w->sign;
 }
@@ -806,7 +813,8 @@ double oracle_sherman_morrison(int n, double *Ainv_d, int p, const double *v_d) 
  *   (dA/dR_a,d)[p][j] = - sum_{l on a} C[l][j] d_d Phi_l(r_p),
  *   d ln D / d R_a,d   = - sum_p sum_j Ainv[j][p] sum_{l on a} C[l][j] d_d Phi_l(r_p)        (both spins added),
  * plus the Jastrow, where only the electron-nucleus term knows R_a:  dJ/dR_a = - sum_i u_en'(r_ia) (r_i - R_a)/r_ia.
- * This is the wave-function ("Pulay") term of a QMC force estimator; the derivative of E_L itself (eq. 4) is not built.
+ * This is the wave-function ("Pulay") term of a QMC force estimator; the derivative of E_L itself (eq. 4) is
+ * oracle_walker_deloc_dR below.
  * out[n_atoms][3].  Plain loops in the order written; a test pins it to finite differences of log|Psi| under a
  * displacement of the nucleus together with its basis functions. */
 void oracle_walker_dlogpsi_dR(const oracle_system *s, const oracle_walker *w, double *out) {

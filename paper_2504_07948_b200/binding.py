@@ -27,6 +27,7 @@ EXPORTED = [
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
     "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl", "qmc_set_mo_ctas", "qmc_sweep_crowds",
+    "qmc_release_scratch", "qmc_philox_words",
 ]
 
 
@@ -99,6 +100,8 @@ def load_library(path: str | None = None):
     lib.qmc_sweep_crowds.argtypes = [C.POINTER(vp), i, i, d, i]
     lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
+    lib.qmc_release_scratch.argtypes = [vp]
+    lib.qmc_philox_words.argtypes = [i, vp, vp, vp]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
     lib.qmc_version.restype = C.c_char_p
@@ -161,7 +164,7 @@ class Walkers:
 
     def __init__(self, handle, system, n_walkers, stream, flags):
         self.handle, self.system, self.n_walkers, self.stream, self.flags = handle, system, n_walkers, stream, flags
-        self.last_nsteps = 0
+        self.last_nsteps = 0   # `stream`: the torch stream all work of this set is enqueued on
 
     def close(self):
         if self.handle:
@@ -219,6 +222,8 @@ def qmc_walkers_create(system: System, positions, seed, first_walker_id=0, first
     if len(shape) != 3 or shape[1] != system.n_elec or shape[2] != 3:
         raise QmcError(QMC_ERR_ARG, f"positions must be [W][{system.n_elec}][3], got {shape}")
     h = C.c_void_p()
+    import torch
+    stream = stream if stream is not None else torch.cuda.current_stream()
     _check(lib.qmc_walkers_create(system.handle, C.byref(h), shape[0], _ptr(positions), C.c_uint64(seed),
                                   first_walker_id, first_step, flags, _stream_ptr(stream)))
     return Walkers(h, system, shape[0], stream, flags)
@@ -250,7 +255,8 @@ def qmc_get_weights(walkers: Walkers, out=None, out_tau_eff=None):
     import torch
     out = _out((walkers.n_walkers,), torch.float64, out)
     out_tau_eff = _out((walkers.n_walkers,), torch.float64, out_tau_eff)
-    _check(load_library().qmc_get_weights(walkers.handle, _ptr(out), _ptr(out_tau_eff)))
+    with _ordered(walkers, out, out_tau_eff):
+        _check(load_library().qmc_get_weights(walkers.handle, _ptr(out), _ptr(out_tau_eff)))
     return out, out_tau_eff
 
 
@@ -258,7 +264,8 @@ def qmc_get_dlogpsi_dR(walkers: Walkers, out=None):
     """d ln|Psi| / d R_a, [W][n_atoms][3] (row f2, first half)."""
     import torch
     out = _out((walkers.n_walkers, walkers.system.n_atoms, 3), torch.float64, out)
-    _check(load_library().qmc_get_dlogpsi_dR(walkers.handle, _ptr(out)))
+    with _ordered(walkers, out):
+        _check(load_library().qmc_get_dlogpsi_dR(walkers.handle, _ptr(out)))
     return out
 
 
@@ -269,7 +276,8 @@ def qmc_get_deloc_dR(walkers: Walkers, out=None, out_dlogpsi=None, with_dlogpsi=
     out = _out(shape, torch.float64, out)
     if with_dlogpsi:
         out_dlogpsi = _out(shape, torch.float64, out_dlogpsi)
-    _check(load_library().qmc_get_deloc_dR(walkers.handle, _ptr(out), _ptr(out_dlogpsi) if with_dlogpsi else None))
+    with _ordered(walkers, out, out_dlogpsi):
+        _check(load_library().qmc_get_deloc_dR(walkers.handle, _ptr(out), _ptr(out_dlogpsi) if with_dlogpsi else None))
     return out, (out_dlogpsi if with_dlogpsi else None)
 
 
@@ -290,8 +298,23 @@ def qmc_get_vnl(walkers: Walkers, out=None):
     import torch
     out = _out((walkers.n_walkers,), torch.float64, out)
     n = C.c_uint64()
-    _check(load_library().qmc_get_vnl(walkers.handle, _ptr(out), C.byref(n)))
+    with _ordered(walkers, out):
+        _check(load_library().qmc_get_vnl(walkers.handle, _ptr(out), C.byref(n)))
     return out, n.value
+
+
+def qmc_release_scratch(walkers: Walkers):
+    """Free the scratch kept by the row-f2 / f3 getters and the host-pointer getters."""
+    _check(load_library().qmc_release_scratch(walkers.handle))
+
+
+def qmc_philox_words(ctr_key, stream=None):
+    """Raw Philox4x32-10 words of the move kernels' generator: ctr_key [n][6] uint32 (counter 0..3, key 0..1) -> [n][4]."""
+    ck = np.ascontiguousarray(ctr_key, np.uint32)
+    assert ck.ndim == 2 and ck.shape[1] == 6
+    out = np.zeros((ck.shape[0], 4), np.uint32)
+    _check(load_library().qmc_philox_words(ck.shape[0], _ptr(ck), _ptr(out), _stream_ptr(stream)))
+    return out
 
 
 def qmc_set_mo_ctas(walkers: Walkers, n_ctas):
@@ -311,7 +334,8 @@ def qmc_branch(walkers: Walkers, out_source=None):
     import torch
     out_source = _out((walkers.n_walkers,), torch.int32, out_source)
     e = C.c_double()
-    _check(load_library().qmc_branch(walkers.handle, _ptr(out_source), C.byref(e)))
+    with _ordered(walkers, out_source):
+        _check(load_library().qmc_branch(walkers.handle, _ptr(out_source), C.byref(e)))
     return out_source, e.value
 
 
@@ -323,8 +347,9 @@ def qmc_dmc_run(walkers: Walkers, n_generations, tau, delay_k, e_trial0, limiter
     log = torch.empty((nb, 3), dtype=torch.float64, device="cuda")
     src = torch.empty((nb, walkers.n_walkers), dtype=torch.int32, device="cuda")
     e = C.c_double()
-    _check(load_library().qmc_dmc_run(walkers.handle, int(n_generations), float(tau), int(delay_k), float(e_trial0), float(limiter_a),
-                                      int(branch_every), float(feedback), C.byref(e), _ptr(log) if nb else None, _ptr(src) if nb else None))
+    with _ordered(walkers, log, src):
+        _check(load_library().qmc_dmc_run(walkers.handle, int(n_generations), float(tau), int(delay_k), float(e_trial0), float(limiter_a),
+                                          int(branch_every), float(feedback), C.byref(e), _ptr(log) if nb else None, _ptr(src) if nb else None))
     walkers.last_nsteps = int(n_generations)
     return e.value, log, src
 
@@ -336,10 +361,37 @@ def _out(shape, dtype, out, device="cuda"):
     return torch.empty(shape, dtype=dtype, device=device)
 
 
+class _ordered:
+    """Stream ordering of a getter (ordering contract of include/qmc.h): the library writes device outputs
+    asynchronously on the WALKER SET's stream, while the caller's tensors live on torch's current stream.  When the two
+    differ, the set's stream first waits for the current one (a freshly allocated output may be a recycled block still in
+    use there), and after the call the current stream waits for the set's, and the caching allocator is told the tensors
+    are in use on that stream.  Same stream: nothing to do."""
+
+    def __init__(self, walkers, *tensors):
+        import torch
+        self.ws, self.cur, self.tensors = walkers.stream, torch.cuda.current_stream(), tensors
+        self.cross = self.ws is not None and self.ws.cuda_stream != self.cur.cuda_stream
+
+    def __enter__(self):
+        if self.cross:
+            self.ws.wait_stream(self.cur)
+        return self
+
+    def __exit__(self, *exc):
+        if self.cross:
+            self.cur.wait_stream(self.ws)
+            for t in self.tensors:
+                if t is not None and hasattr(t, "is_cuda") and t.is_cuda:
+                    t.record_stream(self.ws)
+        return False
+
+
 def qmc_get_positions(walkers: Walkers, out=None):
     import torch
     out = _out((walkers.n_walkers, walkers.system.n_elec, 3), torch.float64, out)
-    _check(load_library().qmc_get_positions(walkers.handle, _ptr(out)))
+    with _ordered(walkers, out):
+        _check(load_library().qmc_get_positions(walkers.handle, _ptr(out)))
     return out
 
 
@@ -347,7 +399,8 @@ def qmc_get_Ainv(walkers: Walkers, spin, out=None):
     import torch
     n = walkers.system.ns(spin)
     out = _out((walkers.n_walkers, n, n), torch.float64, out)
-    _check(load_library().qmc_get_Ainv(walkers.handle, int(spin), _ptr(out)))
+    with _ordered(walkers, out):
+        _check(load_library().qmc_get_Ainv(walkers.handle, int(spin), _ptr(out)))
     return out
 
 
@@ -355,7 +408,8 @@ def qmc_get_logpsi(walkers: Walkers, out=None, out_sign=None):
     import torch
     out = _out((walkers.n_walkers,), torch.float64, out)
     out_sign = _out((walkers.n_walkers,), torch.int8, out_sign)
-    _check(load_library().qmc_get_logpsi(walkers.handle, _ptr(out), _ptr(out_sign)))
+    with _ordered(walkers, out, out_sign):
+        _check(load_library().qmc_get_logpsi(walkers.handle, _ptr(out), _ptr(out_sign)))
     return out, out_sign
 
 
@@ -363,7 +417,8 @@ def qmc_get_eloc(walkers: Walkers, out=None, out_kin=None):
     import torch
     out = _out((walkers.n_walkers,), torch.float64, out)
     out_kin = _out((walkers.n_walkers,), torch.float64, out_kin)
-    _check(load_library().qmc_get_eloc(walkers.handle, _ptr(out), _ptr(out_kin)))
+    with _ordered(walkers, out, out_kin):
+        _check(load_library().qmc_get_eloc(walkers.handle, _ptr(out), _ptr(out_kin)))
     return out, out_kin
 
 
@@ -371,7 +426,8 @@ def qmc_get_accept_log(walkers: Walkers, out=None):
     import torch
     out = _out((walkers.last_nsteps, walkers.system.n_elec, walkers.n_walkers), torch.uint8, out)
     if out.numel():
-        _check(load_library().qmc_get_accept_log(walkers.handle, _ptr(out)))
+        with _ordered(walkers, out):
+            _check(load_library().qmc_get_accept_log(walkers.handle, _ptr(out)))
     return out
 
 
@@ -380,7 +436,8 @@ def qmc_get_ratio_log(walkers: Walkers, out=None, out_pacc=None):
     shape = (walkers.last_nsteps, walkers.system.n_elec, walkers.n_walkers)
     out = _out(shape, torch.float64, out)
     out_pacc = _out(shape, torch.float64, out_pacc)
-    _check(load_library().qmc_get_ratio_log(walkers.handle, _ptr(out), _ptr(out_pacc)))
+    with _ordered(walkers, out, out_pacc):
+        _check(load_library().qmc_get_ratio_log(walkers.handle, _ptr(out), _ptr(out_pacc)))
     return out, out_pacc
 
 

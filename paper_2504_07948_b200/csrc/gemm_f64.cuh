@@ -13,7 +13,34 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace qmc {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to a (kernel, device) pair.  One SmemAttr per kernel (a static at
+// its launch site) remembers, per device ordinal, how many bytes have been granted there, so a process that drives several
+// GPUs -- or several host threads -- sets the attribute where and when it is needed and nowhere else.  Racing threads at
+// worst set the same attribute twice.
+struct SmemAttr {
+    static constexpr int MAX_DEV = 64;
+    std::atomic<size_t> granted[MAX_DEV];   // zero-initialised (static storage); 48 KB need no grant
+    template <class K>
+    cudaError_t ensure(K kernel, size_t bytes) {
+        if (bytes <= 48 * 1024) return cudaSuccess;
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        const bool cached = dev >= 0 && dev < MAX_DEV;
+        if (cached && bytes <= granted[dev].load(std::memory_order_acquire)) return cudaSuccess;
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e == cudaSuccess && cached) {
+            size_t cur = granted[dev].load(std::memory_order_relaxed);
+            while (cur < bytes && !granted[dev].compare_exchange_weak(cur, bytes, std::memory_order_release)) {
+            }
+        }
+        return e;
+    }
+};
 
 template <int BM_, int BN_, int WM_, int WN_, bool BT_, int STAGES_>
 struct GemmCfg {
@@ -194,12 +221,10 @@ __global__ void __launch_bounds__(Cfg::NTHREADS) gemm_f64_kernel(GemmArgs g, Epi
 
 template <class Cfg, class Epi>
 cudaError_t gemm_f64_launch(const GemmArgs& g, int batch, const Epi& epi, cudaStream_t st) {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_f64_kernel<Cfg, Epi>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static SmemAttr attr;
+    if (g.K % Cfg::BK != 0) return cudaErrorInvalidValue;  // the main loop runs whole k-blocks: a remainder would be dropped
+    cudaError_t e = attr.ensure(gemm_f64_kernel<Cfg, Epi>, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
     dim3 grid((g.N + Cfg::BN - 1) / Cfg::BN, (g.M + Cfg::BM - 1) / Cfg::BM, batch);
     gemm_f64_kernel<Cfg, Epi><<<grid, Cfg::NTHREADS, Cfg::SMEM_BYTES, st>>>(g, epi);
     return cudaGetLastError();

@@ -54,6 +54,22 @@ struct DevPool {  // owns cudaMalloc'ed blocks
     }
 };
 
+// A buffer that grows on demand and is kept: the scratch of the row-f2 / f3 getters and the staging buffer of the
+// host-pointer getters are allocated by the first call that needs them, not by every call.
+struct GrowBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes, cudaStream_t st) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaError_t es = cudaStreamSynchronize(st); if (es != cudaSuccess) return es; cudaFree(p); p = nullptr; cap = 0; }
+        cudaError_t e = cudaMalloc(&p, bytes + 256);
+        if (e != cudaSuccess) { p = nullptr; return e; }
+        cap = bytes;
+        return cudaSuccess;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
 struct qmc_system {
     SysDev d;
     DevPool pool;
@@ -61,6 +77,22 @@ struct qmc_system {
     int device;
     int n_sm;
 };
+
+// Every entry point that takes a system or a walker set runs on the device the system was built on, whatever the calling
+// thread's current device is; the caller's device is restored on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) { err = cudaSetDevice(device); switched = err == cudaSuccess; }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define GUARD(sysptr)                                                                                    \
+    DeviceGuard _guard((sysptr)->device);                                                                \
+    if (_guard.err != cudaSuccess) { cudaGetLastError(); return fail(QMC_ERR_CUDA, std::string("cannot select the system's device: ") + cudaGetErrorString(_guard.err)); }
 
 struct StageTimer {
     std::vector<cudaEvent_t> ev;  // pairs
@@ -84,13 +116,15 @@ struct qmc_walkers {
     double* d_emixed;   // [1]
     unsigned mo_epoch;   // stream-K launch counter (flag stamps)
     int prof_stride;     // 0 = off
+    mutable GrowBuf scratch;  // qmc_get_dlogpsi_dR / qmc_get_deloc_dR / qmc_get_vnl
+    mutable GrowBuf bounce;   // device staging of the getters that write to host memory
     StageTimer timer;
     double stage_ms[8];
     uint64_t stage_n[8];
 };
 
 extern "C" const char* qmc_last_error(void) { return g_err.c_str(); }
-extern "C" const char* qmc_version(void) { return "paper_2504_07948_b200 r1 (sm_100a, FP64 DMMA)"; }
+extern "C" const char* qmc_version(void) { return "paper_2504_07948_b200 r2 (sm_100a, FP64 DMMA)"; }
 extern "C" uint64_t qmc_launch_count(void) { return launch_count(); }
 
 static int check_device() {
@@ -137,6 +171,15 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
     CU(fetch(alpha, basis->alpha, (size_t)basis->n_prim_total));
     CU(fetch(coef, basis->coef, (size_t)basis->n_prim_total));
 
+    // numeric input: the basis kernel's exp is written for arguments -alpha t <= 0, and a non-finite table entry would
+    // poison every walker silently
+    auto all_finite = [](const std::vector<double>& v) { for (double x : v) if (!std::isfinite(x)) return false; return true; };
+    if (!all_finite(xyz) || !all_finite(Z)) return fail(QMC_ERR_ARG, "qmc_init: atom coordinates and charges must be finite");
+    if (!all_finite(alpha) || !all_finite(coef)) return fail(QMC_ERR_ARG, "qmc_init: exponents and coefficients must be finite");
+    for (double a : alpha)
+        if (a < 0.0) return fail(QMC_ERR_ARG, "qmc_init: exponents must be >= 0");
+    if (!std::isfinite(jas->a_anti) || !std::isfinite(jas->a_para) || !std::isfinite(jas->b_ee) || !std::isfinite(jas->b_en))
+        return fail(QMC_ERR_ARG, "qmc_init: Jastrow parameters must be finite");
     std::vector<ShellRec> recs(basis->n_shells);
     int f = 0;
     for (int i = 0; i < basis->n_shells; i++) {
@@ -304,6 +347,7 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
 
 extern "C" void qmc_finalize(qmc_system* sys) {
     if (!sys) return;
+    DeviceGuard guard(sys->device);
     sys->pool.free_all();
     delete sys;
 }
@@ -334,18 +378,25 @@ static void destroy_walkers(qmc_walkers* w) {
     if (!w) return;
     cudaStreamSynchronize(w->stream);
     for (cudaEvent_t e : w->timer.ev) cudaEventDestroy(e);
+    w->scratch.release();
+    w->bounce.release();
     w->pool.free_all();
     w->winpool.free_all();
     w->logpool.free_all();
     delete w;
 }
 
-extern "C" void qmc_walkers_destroy(qmc_walkers* w) { destroy_walkers(w); }
+extern "C" void qmc_walkers_destroy(qmc_walkers* w) {
+    if (!w) return;
+    DeviceGuard guard(w->sys->device);
+    destroy_walkers(w);
+}
 
 extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int n_walkers, const double* positions,
                                   uint64_t seed, uint32_t first_walker_id, uint32_t first_step, uint32_t flags,
                                   void* cuda_stream) {
     if (!sys || !out || !positions) return fail(QMC_ERR_ARG, "qmc_walkers_create: null argument");
+    GUARD(sys);
     *out = nullptr;
     if (n_walkers < 1) return fail(QMC_ERR_ARG, "qmc_walkers_create: n_walkers < 1");
     int rc = check_device();
@@ -520,6 +571,7 @@ static void prof_collect(qmc_walkers* w) {
    3 fused step kernel (accept of p + proposal of p + 1), 4 flush, 5 local energy */
 extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
     if (!w || stride < 0) return fail(QMC_ERR_ARG, "qmc_set_profiling");
+    GUARD(w->sys);
     prof_collect(w);
     w->prof_stride = stride;
     memset(w->stage_ms, 0, sizeof(w->stage_ms));
@@ -528,6 +580,7 @@ extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
 }
 extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t* counts /*[6]*/) {
     if (!w || !ms || !counts) return fail(QMC_ERR_ARG, "qmc_get_stage_times");
+    GUARD(w->sys);
     prof_collect(w);
     for (int i = 0; i < 6; i++) { ms[i] = w->stage_ms[i]; counts[i] = w->stage_n[i]; }
     return QMC_OK;
@@ -683,6 +736,7 @@ static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
 static int sweep_impl(qmc_walkers* w, int nsteps, double tau, int delay_k, int dmc, double e_trial, double lim_a,
                       const double* e_trial_dev = nullptr, int log_t0 = 0, int log_T = -1) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_sweep: null walkers");
+    GUARD(w->sys);
     return sweep_sets(&w, 1, SweepCall{nsteps, tau, delay_k, dmc, e_trial, lim_a, e_trial_dev, log_t0, log_T});
 }
 
@@ -694,6 +748,7 @@ extern "C" int qmc_sweep_crowds(qmc_walkers* const* sets, int n_sets, int nsteps
         for (int j = 0; j < i; j++)
             if (sets[j] == sets[i]) return fail(QMC_ERR_ARG, "qmc_sweep_crowds: a walker set appears twice");
     }
+    GUARD(sets[0]->sys);
     return sweep_sets(sets, n_sets, SweepCall{nsteps, tau, delay_k, 0, 0.0, 0.0, nullptr, 0, -1});
 }
 
@@ -705,6 +760,7 @@ extern "C" int qmc_dmc_step(qmc_walkers* w, int n_generations, double tau, int d
 
 extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_branch: null walkers");
+    GUARD(w->sys);
     cudaStream_t st = w->stream;
     CU(launch_branch(w->sys->d, w->d, w->d_comb, w->d_emixed, w->step, nullptr, 0.0, nullptr, st));
     if (source) {
@@ -718,6 +774,7 @@ extern "C" int qmc_branch(qmc_walkers* w, int32_t* source, double* e_mixed) {
 extern "C" int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int delay_k, double e_trial0, double limiter_a, int branch_every,
                            double feedback, double* e_trial_out, double* branch_log, int32_t* sources) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_dmc_run: null walkers");
+    GUARD(w->sys);
     if (n_generations < 0 || branch_every < 0) return fail(QMC_ERR_ARG, "qmc_dmc_run: n_generations and branch_every must be >= 0");
     if (!isfinite(e_trial0) || !isfinite(feedback)) return fail(QMC_ERR_ARG, "qmc_dmc_run: e_trial0 and feedback must be finite");
     cudaStream_t st = w->stream;
@@ -763,25 +820,28 @@ extern "C" int qmc_dmc_run(qmc_walkers* w, int n_generations, double tau, int de
 
 extern "C" int qmc_get_dlogpsi_dR(qmc_walkers* w, double* out) {
     if (!w || !out) return fail(QMC_ERR_ARG, "qmc_get_dlogpsi_dR: null argument");
+    GUARD(w->sys);
     const SysDev& s = w->sys->d;
     const WalkDev& d = w->d;
     cudaStream_t st = w->stream;
     const size_t n_out = (size_t)d.W * s.n_atoms * 3;
-    double *Mt = nullptr, *acc = nullptr;
-    CU(cudaMalloc((void**)&Mt, (size_t)d.W * d.ldv * s.nbp * 8 + 16));
-    cudaError_t e = cudaMalloc((void**)&acc, n_out * 8 + 16);
-    if (e == cudaSuccess) e = cudaMemsetAsync(acc, 0, n_out * 8, st);
+    const size_t n_mt = (size_t)d.W * d.ldv * s.nbp;
+    if (w->scratch.reserve((n_mt + n_out + 2) * 8, st) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(QMC_ERR_NOMEM, "qmc_get_dlogpsi_dR: scratch does not fit");
+    }
+    double *Mt = (double*)w->scratch.p, *acc = Mt + n_mt;
+    cudaError_t e = cudaMemsetAsync(acc, 0, n_out * 8, st);
     for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) e = launch_dlogpsi_dR(s, d, sp, Mt, acc, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, acc, n_out * 8, cudaMemcpyDefault, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(Mt);
-    cudaFree(acc);
     CU(e);
     return QMC_OK;
 }
 
 extern "C" int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi) {
     if (!w || !deloc) return fail(QMC_ERR_ARG, "qmc_get_deloc_dR: null argument");
+    GUARD(w->sys);
     const SysDev& s = w->sys->d;
     const WalkDev& d = w->d;
     cudaStream_t st = w->stream;
@@ -790,11 +850,11 @@ extern "C" int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi) 
     // one allocation: Mt, Nt [W][nsm][nbp] | Bm [2][W][nsm^2] | U, XT [W][nsm^2] | fg [W][ne][8] | acc_E, acc_psi
     const size_t n_mt = W * nsm * s.nbp, n_sq = W * nsm * nsm, n_fg = W * s.ne * 8;
     const size_t total = 2 * n_mt + 4 * n_sq + n_fg + 2 * n_out + 16;
-    double* buf = nullptr;
-    if (cudaMalloc((void**)&buf, total * 8) != cudaSuccess) {
+    if (w->scratch.reserve(total * 8, st) != cudaSuccess) {
         cudaGetLastError();
         return fail(QMC_ERR_NOMEM, "qmc_get_deloc_dR: scratch does not fit");
     }
+    double* buf = (double*)w->scratch.p;
     double *Mt = buf, *Nt = Mt + n_mt, *Bm = Nt + n_mt, *U = Bm + 2 * n_sq, *XT = U + n_sq, *fg = XT + n_sq;
     double *accE = fg + n_fg, *accP = accE + n_out;
     cudaError_t e = cudaMemsetAsync(accE, 0, 2 * n_out * 8, st);
@@ -802,14 +862,23 @@ extern "C" int qmc_get_deloc_dR(qmc_walkers* w, double* deloc, double* dlogpsi) 
     if (e == cudaSuccess) e = cudaMemcpyAsync(deloc, accE, n_out * 8, cudaMemcpyDefault, st);
     if (e == cudaSuccess && dlogpsi) e = cudaMemcpyAsync(dlogpsi, accP, n_out * 8, cudaMemcpyDefault, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(buf);
     CU(e);
+    return QMC_OK;
+}
+
+extern "C" int qmc_release_scratch(qmc_walkers* w) {
+    if (!w) return fail(QMC_ERR_ARG, "qmc_release_scratch: null walkers");
+    GUARD(w->sys);
+    CU(cudaStreamSynchronize(w->stream));
+    w->scratch.release();
+    w->bounce.release();
     return QMC_OK;
 }
 
 extern "C" int qmc_set_ecp(qmc_system* S, int n_channels, const int32_t* ch_atom, const int32_t* ch_l, const double* ch_beta,
                            const double* ch_alpha, const double* rcut) {
     if (!S) return fail(QMC_ERR_ARG, "qmc_set_ecp: null system");
+    GUARD(S);
     if (n_channels < 0 || (n_channels > 0 && (!ch_atom || !ch_l || !ch_beta || !ch_alpha)) || !rcut) return fail(QMC_ERR_ARG, "qmc_set_ecp: null argument");
     const int na = S->d.n_atoms;
     std::vector<int> atom, l;
@@ -858,14 +927,20 @@ extern "C" int qmc_set_ecp(qmc_system* S, int n_channels, const int32_t* ch_atom
 
 extern "C" int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs_out) {
     if (!w || !vnl) return fail(QMC_ERR_ARG, "qmc_get_vnl: null argument");
+    GUARD(w->sys);
     const SysDev& s = w->sys->d;
     const WalkDev& d = w->d;
     if (!s.ecp_off) return fail(QMC_ERR_ARG, "qmc_get_vnl: no pseudopotential set (qmc_set_ecp)");
     cudaStream_t st = w->stream;
     const size_t W = (size_t)d.W;
-    double* acc = nullptr;
-    CU(cudaMalloc((void**)&acc, W * 8 + 16));
-    cudaError_t e = cudaMemsetAsync(acc, 0, W * 8, st);
+    // Persistent scratch (grown on demand, kept): [acc W doubles | cnt n+1 ints | per pair: 60 doubles + 3 ints].  A call
+    // whose pair count exceeds what an earlier call left room for grows the buffer once; the counts are recomputed after
+    // that, because growing moves the buffer.
+    const size_t n_max = W * (size_t)(s.ns[0] > s.ns[1] ? s.ns[0] : s.ns[1]);
+    const size_t head = ((W + 2) * 8 + (n_max + 1) * 4 + 15) / 16 * 16;
+    auto pair_bytes = [](size_t np) { return np * (12 * 5 * 8 + 3 * 4) + 64; };
+    cudaError_t e = w->scratch.reserve(head + pair_bytes(n_max / 2 + 1024), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w->scratch.p, 0, W * 8, st);   // acc
     uint64_t total = 0;
     for (int sp = 0; sp < 2 && e == cudaSuccess; sp++) {
         NlArgs a;
@@ -873,33 +948,31 @@ extern "C" int qmc_get_vnl(qmc_walkers* w, double* vnl, uint64_t* n_pairs_out) {
         a.spin = sp; a.e0 = sp == 0 ? 0 : s.ns[0]; a.ns = s.ns[sp]; a.step = w->step;
         if (a.ns == 0) continue;
         const size_t n = W * (size_t)a.ns;
-        e = cudaMalloc((void**)&a.cnt, (n + 1) * 4);
-        if (e != cudaSuccess) break;
         int n_pairs = 0;
-        e = launch_nl_count(s, d, a, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(&n_pairs, a.cnt + n, 4, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        int* ibuf = nullptr;
-        double* dbuf = nullptr;
+        for (int attempt = 0; attempt < 2 && e == cudaSuccess; attempt++) {
+            a.cnt = (int*)((char*)w->scratch.p + (W + 2) * 8);
+            e = launch_nl_count(s, d, a, st);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(&n_pairs, a.cnt + n, 4, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess || head + pair_bytes((size_t)n_pairs) <= w->scratch.cap) break;
+            std::vector<double> acc_host(W);   // the sums of the spin already done move with the buffer
+            e = cudaMemcpy(acc_host.data(), w->scratch.p, W * 8, cudaMemcpyDeviceToHost);
+            if (e == cudaSuccess) e = w->scratch.reserve(head + pair_bytes((size_t)n_pairs), st);
+            if (e == cudaSuccess) e = cudaMemcpy(w->scratch.p, acc_host.data(), W * 8, cudaMemcpyHostToDevice);
+        }
         if (e == cudaSuccess && n_pairs > 0) {
             const size_t np = (size_t)n_pairs;
-            e = cudaMalloc((void**)&ibuf, 3 * np * 4);
-            if (e == cudaSuccess) e = cudaMalloc((void**)&dbuf, np * 12 * 5 * 8);
-            if (e == cudaSuccess) {
-                a.pair_w = ibuf; a.pair_e = ibuf + np; a.pair_I = ibuf + 2 * np;
-                a.pts = dbuf; a.ang = dbuf + np * 36; a.terms = a.ang + np * 12;
-            }
+            double* dbuf = (double*)((char*)w->scratch.p + head);
+            int* ibuf = (int*)(dbuf + np * 60);
+            a.pair_w = ibuf; a.pair_e = ibuf + np; a.pair_I = ibuf + 2 * np;
+            a.pts = dbuf; a.ang = dbuf + np * 36; a.terms = a.ang + np * 12;
         }
-        if (e == cudaSuccess) e = launch_nl_evaluate(s, d, a, n_pairs, d.mo_grid, &w->mo_epoch, acc, st);
+        if (e == cudaSuccess) e = launch_nl_evaluate(s, d, a, n_pairs, d.mo_grid, &w->mo_epoch, (double*)w->scratch.p, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        cudaFree(a.cnt);
-        cudaFree(ibuf);
-        cudaFree(dbuf);
         total += (uint64_t)n_pairs;
     }
-    if (e == cudaSuccess) e = cudaMemcpyAsync(vnl, acc, W * 8, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(vnl, w->scratch.p, W * 8, cudaMemcpyDefault, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(acc);
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return fail(QMC_ERR_NOMEM, "qmc_get_vnl: scratch does not fit"); }
     CU(e);
     if (n_pairs_out) *n_pairs_out = total;
@@ -916,6 +989,7 @@ extern "C" int qmc_set_mo_ctas(qmc_walkers* w, int n_ctas) {
 
 extern "C" int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_get_mo_work: null walkers");
+    GUARD(w->sys);
     unsigned long long h[2];
     CU(cudaMemcpyAsync(h, w->d.mo_work, sizeof(h), cudaMemcpyDeviceToHost, w->stream));
     CU(cudaStreamSynchronize(w->stream));
@@ -926,6 +1000,7 @@ extern "C" int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_
 
 extern "C" int qmc_get_weights(const qmc_walkers* w, double* weights, double* tau_eff) {
     if (!w || !weights) return fail(QMC_ERR_ARG, "qmc_get_weights: null argument");
+    GUARD(w->sys);
     const size_t n = (size_t)w->d.W * 8;
     CU(cudaMemcpyAsync(weights, w->d.weight, n, cudaMemcpyDefault, w->stream));
     if (tau_eff) CU(cudaMemcpyAsync(tau_eff, w->d.tau_eff, n, cudaMemcpyDefault, w->stream));
@@ -950,23 +1025,24 @@ static int deliver(const qmc_walkers* w, void* out, size_t bytes, F&& produce) {
         CU(produce(out));
         return QMC_OK;
     }
-    void* tmp;
-    CU(cudaMalloc(&tmp, bytes));
+    CU(w->bounce.reserve(bytes, st));  // kept from call to call
+    void* tmp = w->bounce.p;
     cudaError_t e = produce(tmp);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(tmp);
     CU(e);
     return QMC_OK;
 }
 
 extern "C" int qmc_get_positions(const qmc_walkers* w, double* out) {
     if (!w || !out) return fail(QMC_ERR_ARG, "qmc_get_positions: null argument");
+    GUARD(w->sys);
     return deliver(w, out, (size_t)w->d.W * w->d.ne * 3 * 8, [&](void* dst) { return launch_export_positions(w->d, (double*)dst, w->stream); });
 }
 
 extern "C" int qmc_get_Ainv(const qmc_walkers* w, int spin, double* out) {
     if (!w || !out || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_get_Ainv: bad argument");
+    GUARD(w->sys);
     const SysDev& s = w->sys->d;
     return deliver(w, out, (size_t)w->d.W * s.ns[spin] * s.ns[spin] * 8,
                    [&](void* dst) { return launch_export_ainv(w->d.AinvT[spin], w->d.W, s.ns[spin], s.nsp[spin], (double*)dst, w->stream); });
@@ -974,6 +1050,7 @@ extern "C" int qmc_get_Ainv(const qmc_walkers* w, int spin, double* out) {
 
 extern "C" int qmc_get_logpsi(const qmc_walkers* w, double* logabs, int8_t* sign) {
     if (!w || !logabs) return fail(QMC_ERR_ARG, "qmc_get_logpsi: null argument");
+    GUARD(w->sys);
     int rc = deliver(w, logabs, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.logpsi, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
     if (rc || !sign) return rc;
     return deliver(w, sign, (size_t)w->d.W, [&](void* dst) { return launch_sign_to_i8(w->d.sign, w->d.W, (int8_t*)dst, w->stream); });
@@ -981,6 +1058,7 @@ extern "C" int qmc_get_logpsi(const qmc_walkers* w, double* logabs, int8_t* sign
 
 extern "C" int qmc_get_eloc(const qmc_walkers* w, double* eloc, double* ekin) {
     if (!w || !eloc) return fail(QMC_ERR_ARG, "qmc_get_eloc: null argument");
+    GUARD(w->sys);
     int rc = deliver(w, eloc, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.eloc, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
     if (rc || !ekin) return rc;
     return deliver(w, ekin, (size_t)w->d.W * 8, [&](void* dst) { return cudaMemcpyAsync(dst, w->d.ekin, (size_t)w->d.W * 8, cudaMemcpyDeviceToDevice, w->stream); });
@@ -988,6 +1066,7 @@ extern "C" int qmc_get_eloc(const qmc_walkers* w, double* eloc, double* ekin) {
 
 extern "C" int qmc_get_accept_log(const qmc_walkers* w, uint8_t* bits) {
     if (!w || !bits) return fail(QMC_ERR_ARG, "qmc_get_accept_log: null argument");
+    GUARD(w->sys);
     if (!w->d.bits) return fail(QMC_ERR_STATE, "qmc_get_accept_log: no sweep has been run");
     size_t n = (size_t)w->T_last * w->d.ne * w->d.W;
     if (n == 0) return QMC_OK;
@@ -998,6 +1077,7 @@ extern "C" int qmc_get_accept_log(const qmc_walkers* w, uint8_t* bits) {
 
 extern "C" int qmc_get_ratio_log(const qmc_walkers* w, double* ratio, double* pacc) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null walkers");
+    GUARD(w->sys);
     if (!(w->flags & QMC_LOG_RATIOS) || !w->d.ratio_log) return fail(QMC_ERR_STATE, "qmc_get_ratio_log: walkers were not created with QMC_LOG_RATIOS, or no sweep has run");
     if (!ratio) return fail(QMC_ERR_ARG, "qmc_get_ratio_log: null argument");
     size_t n = (size_t)w->T_last * w->d.ne * w->d.W * 8;
@@ -1010,6 +1090,7 @@ extern "C" int qmc_get_ratio_log(const qmc_walkers* w, double* ratio, double* pa
 
 extern "C" int qmc_get_stats(const qmc_walkers* w, uint64_t* n_proposed, uint64_t* n_accepted, uint64_t* n_ties, uint64_t* n_nonfinite) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_get_stats: null walkers");
+    GUARD(w->sys);
     unsigned long long h[4];
     CU(cudaMemcpyAsync(h, w->d.stats, sizeof(h), cudaMemcpyDeviceToHost, w->stream));
     CU(cudaStreamSynchronize(w->stream));
@@ -1022,6 +1103,7 @@ extern "C" int qmc_get_stats(const qmc_walkers* w, uint64_t* n_proposed, uint64_
 
 extern "C" int qmc_synchronize(const qmc_walkers* w) {
     if (!w) return fail(QMC_ERR_ARG, "qmc_synchronize: null walkers");
+    GUARD(w->sys);
     CU(cudaStreamSynchronize(w->stream));
     return QMC_OK;
 }
@@ -1032,6 +1114,7 @@ static int eval_common(const qmc_system* sys, int spin, int n_points, const doub
     if (!sys || n_points < 0 || spin < 0 || spin > 1) return fail(QMC_ERR_ARG, "qmc_eval_*: bad argument");
     if (n_points == 0) return QMC_OK;
     if (!xyz || !out) return fail(QMC_ERR_ARG, "qmc_eval_*: null buffer");
+    GUARD(sys);
     int rc = check_device();
     if (rc) return rc;
     const SysDev& s = sys->d;
@@ -1078,6 +1161,7 @@ extern "C" int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const 
 extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, double* ms_per_launch) {
     if (!w || !ms_per_launch || stage < 0 || stage > 5 || spin < 0 || spin > 1 || reps < 1 || delay_k < 1 || delay_k > 128)
         return fail(QMC_ERR_ARG, "qmc_time_stage: bad argument");
+    GUARD(w->sys);
     const SysDev& s = w->sys->d;
     WalkDev& d = w->d;
     cudaStream_t st = w->stream;
@@ -1124,6 +1208,23 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
     CU(err);
     CU(cudaStreamSynchronize(st));
     *ms_per_launch = (double)ms / reps;
+    return QMC_OK;
+}
+
+extern "C" int qmc_philox_words(int n, const uint32_t* ctr_key, uint32_t* out, void* cuda_stream) {
+    if (n < 0 || (n > 0 && (!ctr_key || !out))) return fail(QMC_ERR_ARG, "qmc_philox_words: bad argument");
+    if (n == 0) return QMC_OK;
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint32_t* buf = nullptr;
+    CU(cudaMalloc((void**)&buf, (size_t)n * 10 * 4));
+    cudaError_t e = cudaMemcpyAsync(buf, ctr_key, (size_t)n * 6 * 4, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = launch_philox_words(n, buf, buf + (size_t)n * 6, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, buf + (size_t)n * 6, (size_t)n * 4 * 4, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(buf);
+    CU(e);
     return QMC_OK;
 }
 

@@ -273,14 +273,11 @@ cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int row
 // plan: NULL for the dense contraction, else the walker set whose plan_* buffers launch_mo_plan has just filled
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
                       int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st) {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_mo_streamk<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_mo_streamk<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MO_SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static SmemAttr attr[3];
+    cudaError_t ea = attr[0].ensure(k_mo_streamk<false, false>, MO_SMEM_BYTES);
+    if (ea == cudaSuccess) ea = attr[1].ensure(k_mo_streamk<true, false>, MO_SMEM_BYTES);
+    if (ea == cudaSuccess) ea = attr[2].ensure(k_mo_streamk<false, true>, MO_SMEM_BYTES);
+    if (ea != cudaSuccess) return ea;
     MoArgs g;
     g.PhiT = PhiT; g.CT = s.CT[spin]; g.V = V; g.ldv = ldv;
     g.M = rows; g.N = s.nsp[spin];
@@ -303,15 +300,11 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 // a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st) {
-    static size_t configured[2] = {48 * 1024, 48 * 1024};
+    static SmemAttr attr[2];
     const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp);
     const bool wide = step_threads(s.nsp[spin]) == 512;
-    if (smem > configured[wide]) {
-        cudaError_t er = wide ? cudaFuncSetAttribute(k_step<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                              : cudaFuncSetAttribute(k_step<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (er != cudaSuccess) return er;
-        configured[wide] = smem;
-    }
+    const cudaError_t er = wide ? attr[1].ensure(k_step<512>, smem) : attr[0].ensure(k_step<128>, smem);
+    if (er != cudaSuccess) return er;
     if (wide) k_step<512><<<wd.W, 512, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     else k_step<128><<<wd.W, 128, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     COUNT_LAUNCH();
@@ -650,7 +643,8 @@ static cudaError_t launch_block_inverse(double* Mall, long stride, int n, int ld
     g.rowof = (int*)(buf + bFn + bT + bP); g.used = (unsigned char*)(buf + bFn + bT + bP + bR);
     e = cudaMemsetAsync(buf, 0, bFn + bT + bP + bR + bU, st);
     const size_t smem = gjb_panel_smem(n, nb);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gjb_panel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static SmemAttr panel_attr;
+    if (e == cudaSuccess) e = panel_attr.ensure(k_gjb_panel, smem);
     GemmArgs ga;
     ga.A = g.Fn; ga.lda = GJB_NB; ga.strideA = (long)ld * GJB_NB;
     ga.B = g.T; ga.ldb = ld; ga.strideB = (long)GJB_NB * ld;
@@ -683,7 +677,9 @@ cudaError_t launch_gj_inverse(double* Mall, long stride, int n, int ld, int batc
     if (n >= 512) {
         constexpr int NT = 1024;
         size_t smem = (size_t)(2 * n + NT / 32) * sizeof(double) + (size_t)(NT / 32 + n) * sizeof(int);
-        cudaFuncSetAttribute(k_gj_inverse<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static SmemAttr attr;
+        const cudaError_t ea = attr.ensure(k_gj_inverse<NT>, smem);
+        if (ea != cudaSuccess) return ea;
         k_gj_inverse<NT><<<batch, NT, smem, st>>>(Mall, stride, n, ld, logdet, sign, status);
     } else {
         constexpr int NT = 256;
@@ -971,12 +967,9 @@ cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, u
     while (wpb > 1 && (wd.W + wpb - 1) / wpb < 148) wpb--;
     a.wpb = wpb;
     const size_t smem = per_block + (size_t)wpb * per_walker;
-    static size_t configured = 48 * 1024;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_sweep_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static SmemAttr attr;
+    const cudaError_t ea = attr.ensure(k_sweep_small, smem);
+    if (ea != cudaSuccess) return ea;
     k_sweep_small<<<(wd.W + wpb - 1) / wpb, wpb * 32, smem, st>>>(s, wd, a);
     COUNT_LAUNCH();
     return cudaGetLastError();
@@ -1099,6 +1092,21 @@ cudaError_t launch_nl_evaluate(const SysDev& s, const WalkDev& wd, const NlArgs&
         k_nl_reduce<<<wd.W, 256, 0, st>>>(wd, a, vnl);
         COUNT_LAUNCH();
     }
+    return cudaGetLastError();
+}
+
+// the generator of k_step / k_sweep_small on caller-chosen counters and keys (cross-check against an independent
+// implementation in the tests): in [n][6] = counter words 0..3, key words 0..1; out [n][4]
+__global__ void k_philox_words(int n, const uint32_t* __restrict__ in, uint32_t* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t o[4];
+    philox4x32_10(in[6 * i], in[6 * i + 1], in[6 * i + 2], in[6 * i + 3], in[6 * i + 4], in[6 * i + 5], o);
+    out[4 * i] = o[0]; out[4 * i + 1] = o[1]; out[4 * i + 2] = o[2]; out[4 * i + 3] = o[3];
+}
+cudaError_t launch_philox_words(int n, const uint32_t* in, uint32_t* out, cudaStream_t st) {
+    k_philox_words<<<(n + 255) / 256, 256, 0, st>>>(n, in, out);
+    COUNT_LAUNCH();
     return cudaGetLastError();
 }
 

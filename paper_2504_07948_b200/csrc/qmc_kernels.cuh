@@ -52,6 +52,7 @@ cudaError_t launch_nl_evaluate(const SysDev& s, const WalkDev& wd, const NlArgs&
 cudaError_t launch_forces(const SysDev& s, const WalkDev& wd, double* Mt, double* Nt, double* Bm, double* U, double* XT, double* fg,
                           double* acc_E, double* acc_psi, cudaStream_t st);
 cudaError_t launch_dlogpsi_dR(const SysDev& s, const WalkDev& wd, int spin, double* Mt, double* acc, cudaStream_t st);
+cudaError_t launch_philox_words(int n, const uint32_t* in, uint32_t* out, cudaStream_t st);
 uint64_t launch_count();
 
 }  // namespace qmc
