@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--paper-regime", action="store_true",
                     help="row f4: the paper's own regime -- water clusters of 8/16/24/152 valence electrons, 4320 walkers per GPU "
                          "(PAPER.md L279-302) -- on the one-launch small-system path and on the per-electron path; one JSON line each")
+    ap.add_argument("--one-lane", action="store_true", help="QMC_ONE_LANE: the crowd as one lane (the round-1 schedule), for comparison")
     ap.add_argument("--no-screened", action="store_true", help="skip the extra leg with QMC_SCREEN_MO")
     ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -65,6 +66,14 @@ def workload_name(wl, walkers, k):
             f"tau {wl.tau}, delay_k {k}")
 
 
+def config_dict(wl, walkers, k, world):
+    """The `config` object of the JSON line -- the same keys for both arms, so that the driver's same_config check compares
+    like with like (the reference arm times a bounded SAMPLE of this workload: see its cpu_baseline.sample)."""
+    return dict(workload=workload_name(wl, walkers, k), step="one sweep = one proposed move per electron per walker",
+                moves_per_step=walkers * wl.system.n_elec * world,
+                l2="per-step working set (A^-1 + row caches, ~25 GB/GPU) >> 126 MB L2; no flush needed")
+
+
 def flop_model(sysm, n_moves, n_accepted):
     """MO contraction 2*c*N_b*N_s per proposed move (c = 5) + 4*N_s^2 per accepted move."""
     ns = sysm.n_up
@@ -72,15 +81,23 @@ def flop_model(sysm, n_moves, n_accepted):
 
 
 def stage_rooflines(sysm, W, k, acc, ms, hbm_gbs, fp64_tflops):
-    """Per-stage roofline fractions: algorithmic bytes or flops of ONE launch of each stage over
-    its mean duration measured in the timed region.  acc = accepted fraction; the mean number of rows pending in the
-    delay window when a fused step kernel runs is acc*(k-1)/2."""
+    """Per-stage roofline fractions: ALGORITHMIC bytes or flops of ONE launch of each stage
+    (what the method must move, not what the kernel happens to move) over its mean duration measured
+    with CUDA events.  acc = accepted fraction; the mean number of rows pending in the delay window when a fused step
+    kernel runs is mbar = acc*(k-1)/2.  The step kernel = rows a1 + a5 + a6 + a7:
+        8 N_s (1 + 3 + c_r)   drift row of A^-T, three gradient rows of the row cache, c_r = 4 rows of V at r'
+      + 16 mbar N_s           the window (Vbuf and Wbuf rows pending), once each
+      + 24 N_e                the walker's positions (Jastrow)
+      + 7 * 8 N_s acc         commit of an accepted move: five row-cache rows + two window rows written
+    `impl_bytes_per_launch` is what this implementation moves by its own count (Wbuf twice, the x column written and read
+    back, two Jastrow passes, S^-1) -- reported beside the algorithmic figure, never used for `frac`."""
     ns, nb, ne, na = sysm.n_up, sysm.n_basis, sysm.n_elec, sysm.n_atoms
     mbar = acc * (k - 1) / 2.0
-    per_walker_step = (8.0 * ns * (5 + 1 + 1 + acc * (5 + 2) + 1 + 3 + 1)          # V rows, x column r/w, a_p rows, row caches, new window rows
-                       + 8.0 * ns * mbar * (acc * 1 + 2)                            # Wbuf (commit), Vbuf + Wbuf (proposal)
-                       + 8.0 * mbar * mbar * (acc * 2 + 1)                          # S^-1 update and use
-                       + 2 * 24.0 * (ne + na))                                      # partner coordinates, two Jastrow passes
+    per_walker_step = 8.0 * ns * (1 + 3 + 4) + 16.0 * mbar * ns + 24.0 * ne + 7 * 8.0 * ns * acc
+    impl_step = (8.0 * ns * (5 + 1 + 1 + acc * (5 + 2) + 1 + 3 + 1)          # V rows, x column r/w, a_p rows, row caches, new window rows
+                 + 8.0 * ns * mbar * (acc * 1 + 2)                            # Wbuf (commit), Vbuf + Wbuf (proposal)
+                 + 8.0 * mbar * mbar * (acc * 2 + 1)                          # S^-1 update and use
+                 + 2 * 24.0 * (ne + na))                                      # partner coordinates, two Jastrow passes
     m = acc * k
     alg = {
         "basis": ("hbm", 8.0 * 5 * W * nb),
@@ -97,6 +114,8 @@ def stage_rooflines(sysm, W, k, acc, ms, hbm_gbs, fp64_tflops):
         if bound == "hbm":
             a = amount / (t * 1e-3) * 1e-9
             out[st] = dict(bound="hbm", achieved=a, peak=hbm_gbs, unit="GB/s", frac=a / hbm_gbs, bytes_per_launch=amount)
+            if st == "step":
+                out[st]["impl_bytes_per_launch"] = W * impl_step
         else:
             a = amount / (t * 1e-3) * 1e-12
             out[st] = dict(bound="tensor", achieved=a, peak=fp64_tflops, unit="TFLOP/s", frac=a / fp64_tflops, flop_per_launch=amount)
@@ -194,8 +213,7 @@ def run_reference(args):
     line = dict(metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
                 ms_per_step=s_per_step * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
                 data="synthetic", impl="reference",
-                config=dict(workload=workload_name(wl, args.walkers or wl.n_walkers, k),
-                            note="each step is a bounded sample of the workload, see cpu_baseline.sample"),
+                config=config_dict(wl, args.walkers or wl.n_walkers, k, args.gpus),
                 cpu_baseline=cb,
                 e2e=dict(value=cb["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line), flush=True)
@@ -230,12 +248,12 @@ def run_ours(args):
 
     # ---- device-resident run: inputs already in HBM when the timed region starts
     pos_dev = pos_host.cuda()
-    gw = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo)
+    base_flags = qb.QMC_ONE_LANE if args.one_lane else 0
+    gw = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=base_flags)
     for _ in range(args.warmup):
         qb.qmc_sweep(gw, 1, wl.tau, k)
     qb.qmc_synchronize(gw)
     st0 = qb.qmc_get_stats(gw)
-    qb.qmc_set_profiling(gw, args.prof_stride)
     sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = qb.qmc_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -251,16 +269,25 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     launches = qb.qmc_launch_count() - l0
     clocks = sampler.stop() if sampler else None
+    st1 = qb.qmc_get_stats(gw)
+    eloc = qb.qmc_get_eloc(gw)[0].clone()
+    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not (args.no_screened and args.no_crowds) else None
+    # ---- the per-stage times come from a SECOND pass of K sweeps on the same crowd with the in-situ stage timers on (CUDA
+    # events around every prof_stride-th electron's launches): the headline above is timed without that instrumentation
+    qb.qmc_set_profiling(gw, args.prof_stride)
+    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pe0.record()
+    qb.qmc_sweep(gw, args.steps, wl.tau, k)
+    pe1.record()
+    torch.cuda.synchronize()
+    ms_profiled_pass = pe0.elapsed_time(pe1)
     stage = qb.qmc_get_stage_times(gw)
     qb.qmc_set_profiling(gw, 0)
-    st1 = qb.qmc_get_stats(gw)
-    eloc = qb.qmc_get_eloc(gw)[0]
     n_moves = st1["proposed"] - st0["proposed"]
     n_acc = st1["accepted"] - st0["accepted"]
     assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
     assert st1["nonfinite"] == 0
     red = reduce_report(ms, n_moves, float(eloc.sum()), float((eloc * eloc).sum()), W, backend_device="cuda")
-    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not (args.no_screened and args.no_crowds) else None
     # ---- end to end through the C ABI with HOST buffers: one whole job of K sweeps (a second walker set beside the first;
     # measured straight after the device-resident run so that both see the same thermal state)
     e2e = None
@@ -274,7 +301,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        gw2 = qb.qmc_walkers_create(gsys, pos_host, wl.seed, first_walker_id=lo)     # H2D of the positions inside
+        gw2 = qb.qmc_walkers_create(gsys, pos_host, wl.seed, first_walker_id=lo, flags=base_flags)     # H2D of the positions inside
         qb.qmc_sweep(gw2, args.steps, wl.tau, k)
         qb.qmc_get_positions(gw2, out=out_pos)                                        # D2H, synchronous
         qb.qmc_get_eloc(gw2, out=out_e, out_kin=out_k)
@@ -392,7 +419,7 @@ def run_ours(args):
     # ---- the same K sweeps with the optional screening of the MO contraction (QMC_SCREEN_MO); NOT the headline value
     screened = None
     if not args.no_screened:
-        gw3 = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=qb.QMC_SCREEN_MO)
+        gw3 = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=qb.QMC_SCREEN_MO | base_flags)
         for _ in range(args.warmup):
             qb.qmc_sweep(gw3, 1, wl.tau, k)
         w0 = qb.qmc_get_mo_work(gw3)
@@ -446,9 +473,7 @@ def run_ours(args):
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=red["elapsed_ms"] / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
         dtype="f64", data="synthetic",
-        config=dict(workload=workload_name(wl, W, k), step="one sweep = one proposed move per electron per walker",
-                    moves_per_step=W * sysm.n_elec * world, l2="per-step working set (A^-1 + row caches, ~25 GB/GPU) >> 126 MB L2; no flush needed",
-                    prof_stride=args.prof_stride),
+        config=config_dict(wl, W, k, world), prof_stride=args.prof_stride,
         clocks=clocks, e2e=e2e, gpu_launches=int(launches),
         roofline=dict(kernel="k_mo_streamk (MO contraction V = Phi*C, persistent stream-K, DMMA m8n8k4)", bound="tensor", achieved=achieved,
                       peak=peak, unit="TFLOP/s", frac=(achieved / peak) if achieved else None, traffic=traffic,
@@ -459,6 +484,8 @@ def run_ours(args):
         fp64_tflops_model=flop_model(sysm, red["n_moves"], n_acc * world) / secs * 1e-12,
         accept_frac=n_acc / max(n_moves, 1),
         stage_ms_per_launch=stage_ms,
+        stage_timing="second pass of the same K sweeps with qmc_set_profiling on (%.1f ms per sweep against %.1f unprofiled)" % (
+            ms_profiled_pass / args.steps, red["elapsed_ms"] / args.steps),
         stage_roofline=stage_rooflines(sysm, W, k, n_acc / max(n_moves, 1), stage_ms, hbm_gbs, peak),
         hbm_peak_source="MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "6.65 TB/s of fallback (B200_PROFILING.md)",
         stage_share={s: share[s] / tot_share for s in share},

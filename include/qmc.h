@@ -66,6 +66,12 @@ extern "C" {
                              call in one kernel, one warp per walker, with rank-1 updates (delay_k then only changes
                              rounding, reading A13) */
 
+#define QMC_ONE_LANE 8u   /* never split the crowd into two lanes.  By default a large crowd (rows of the inverse longer than
+                             256, per-electron kernels, a walker count that splits without padding the contraction) moves
+                             through the electron steps as two half crowds on two streams, so that the HBM-bound kernels of
+                             one run in the shadow of the other's contraction; results differ from the one-lane run only by
+                             the rounding of the stream-K partition (it depends on the row count). */
+
 typedef struct qmc_system qmc_system;   /* immutable after qmc_init: atoms, basis, MO coefficients, Jastrow (device) */
 typedef struct qmc_walkers qmc_walkers; /* mutable crowd state */
 

@@ -85,6 +85,7 @@ def _lib(long_double: bool = False):
     lib.oracle_walker_get_Ainv.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
     lib.oracle_walker_get_logpsi.argtypes = [C.c_void_p, _dp, _ip]
     lib.oracle_walker_get_A.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
+    lib.oracle_walker_set_Ainv.argtypes = [C.c_void_p, C.c_void_p, C.c_int, _dp]
     lib.oracle_walker_sweep.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
                                         _u8p, _dp, _dp]
     lib.oracle_walker_sweep_range.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_double,
@@ -369,6 +370,12 @@ class OracleWalker:
         out = np.zeros((n, n))
         self.lib.oracle_walker_get_A(self.sys.h, self.h, spin, _d(out))
         return out
+
+    def set_Ainv(self, spin, ainv):
+        """replace the inverse of one spin (orientation of Ainv(): [p][j] = (A^-1)[j][p]); test use only (floors)"""
+        a = _f64(ainv)
+        assert a.shape == (self.sys.ns(spin),) * 2
+        self.lib.oracle_walker_set_Ainv(self.sys.h, self.h, spin, _d(a))
 
     def logpsi(self):
         la = C.c_double()

@@ -540,6 +540,16 @@ void oracle_walker_get_A(const oracle_system *s, const oracle_walker *w, int spi
         for (int j = 0; j < ns; j++) out[(size_t)p * ns + j] = (double)w->orb[spin][(size_t)p * 5 * ns + j];
 }
 
+/* Replace the inverse of one spin by a caller-supplied one (export orientation A18: in[p][j] = (A^-1)[j][p]).  No
+ * arithmetic.  The tests use it to start a DOUBLE-precision walker from the LONG-DOUBLE LU inverse of its own Slater
+ * matrix: how far such a walker's sweep lands from the plain double walker's is a measured conditioning floor (reading
+ * A26) at sizes where a whole long-double sweep is out of reach (config 3). */
+void oracle_walker_set_Ainv(const oracle_system *s, oracle_walker *w, int spin, const double *in) {
+    int ns = spin == 0 ? s->n_up : s->n_dn;
+    for (int p = 0; p < ns; p++)
+        for (int j = 0; j < ns; j++) w->Ainv[spin][(size_t)j * ns + p] = (real)in[(size_t)p * ns + j];
+}
+
 void oracle_walker_get_logpsi(const oracle_walker *w, double *logabs, int *sign) {
     *logabs = (double)w->logabs; *sign = w->sign;
 }

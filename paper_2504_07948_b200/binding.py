@@ -18,6 +18,7 @@ QMC_OK, QMC_ERR_ARG, QMC_ERR_CUDA, QMC_ERR_SINGULAR, QMC_ERR_NOMEM, QMC_ERR_STAT
 QMC_LOG_RATIOS = 1
 QMC_LARGE_PATH = 2
 QMC_SCREEN_MO = 4
+QMC_ONE_LANE = 8
 STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc")
 
 EXPORTED = [

@@ -27,7 +27,10 @@ constexpr int MO_BM = 128, MO_BN = 128, MO_BK = 32;
 constexpr int MO_ALD = 36, MO_BLD = 132;
 constexpr int MO_A_STAGE = MO_BM * MO_ALD;   // doubles
 constexpr int MO_B_STAGE = MO_BK * MO_BLD;   // doubles
-constexpr int MO_STAGES = 3;
+#ifndef QMC_MO_STAGES
+#define QMC_MO_STAGES 3
+#endif
+constexpr int MO_STAGES = QMC_MO_STAGES;
 constexpr int MO_CONSUMER_WARPS = 8;
 constexpr int MO_THREADS = (MO_CONSUMER_WARPS + 1) * 32;
 constexpr size_t MO_SMEM_BYTES = (size_t)MO_STAGES * (MO_A_STAGE + MO_B_STAGE) * 8 + 2 * MO_STAGES * 8 + 16;

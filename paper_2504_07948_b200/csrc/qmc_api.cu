@@ -100,9 +100,26 @@ struct StageTimer {
     size_t used = 0;
 };
 
+// One lane of a crowd: a contiguous range of its walkers that moves through the electron steps on its own stream.  A
+// large crowd runs as TWO lanes, because inside one lane an electron step is a dependency chain (basis -> contraction ->
+// accept/propose) that leaves the tensor pipe idle a fifth of the time; the other lane's contraction fills those gaps, and
+// this lane's HBM-bound kernels run in the shadow of it (they are sized to fit on an SM beside the resident contraction
+// CTA).  Lanes share the crowd's per-walker arrays (views at an offset); each owns what one contraction needs privately.
+struct Lane {
+    WalkDev d;            // view of walkers [off, off + d.W)
+    int off;
+    cudaStream_t stream;  // lane 0: the crowd's stream
+    unsigned own_epoch;   // stream-K launch counter of a private flags buffer (lane 1); lane 0 stamps the crowd's flags
+    unsigned* mo_epoch;   //   buffer and therefore counts with the crowd's counter
+    cudaEvent_t done;
+};
+
 struct qmc_walkers {
     const qmc_system* sys;
     WalkDev d;
+    int n_lanes;
+    Lane lane[2];
+    cudaEvent_t fork_ev;
     DevPool pool;
     DevPool winpool;
     DevPool logpool;
@@ -378,12 +395,83 @@ static void destroy_walkers(qmc_walkers* w) {
     if (!w) return;
     cudaStreamSynchronize(w->stream);
     for (cudaEvent_t e : w->timer.ev) cudaEventDestroy(e);
+    if (w->n_lanes == 2) {
+        cudaStreamSynchronize(w->lane[1].stream);
+        cudaStreamDestroy(w->lane[1].stream);
+        cudaEventDestroy(w->lane[0].done);
+        cudaEventDestroy(w->lane[1].done);
+        cudaEventDestroy(w->fork_ev);
+    }
     w->scratch.release();
     w->bounce.release();
     w->pool.free_all();
     w->winpool.free_all();
     w->logpool.free_all();
     delete w;
+}
+
+// 64-row units of contraction work for `rows` rows, mirroring launch_mo's choice of tile height
+static int mo_row_units(const SysDev& s, int spin, int rows, int grid) {
+    const int mt = (rows + 127) / 128;
+    const bool half = (long)mt * s.nt[spin] * s.kb < 16L * grid || mt * 128 - rows >= 64;
+    return half ? (rows + 63) / 64 : 2 * mt;
+}
+
+// Two lanes where it pays: the per-electron kernels (not the one-launch path), rows long enough for the 256-thread step
+// kernel, and a crowd that splits without adding more than 5 % of padded rows to the contraction (config 2: 1280 rows = 10
+// tiles -> 5 + 5; config 3: 320 rows = five 64-row tiles -> 3 + 3, so it stays one lane).
+static int choose_lanes(const qmc_system* sys, const WalkDev& d, uint32_t flags) {
+    const SysDev& s = sys->d;
+    if ((flags & QMC_ONE_LANE) || d.W < 2) return 1;
+    if (!(flags & QMC_LARGE_PATH) && small_path_ok(s, d)) return 1;
+    const int nspm = s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1];
+    if (nspm <= 256) return 1;
+    const int w0 = (d.W + 1) / 2, w1 = d.W - w0;
+    for (int sp = 0; sp < 2; sp++) {
+        if (s.ns[sp] == 0) continue;
+        const int whole = mo_row_units(s, sp, 5 * d.W, sys->n_sm);
+        const int split = mo_row_units(s, sp, 5 * w0, sys->n_sm) + mo_row_units(s, sp, 5 * w1, sys->n_sm);
+        if (split * 100 > whole * 105) return 1;
+    }
+    return 2;
+}
+
+// (re)build the lane views from the crowd's arrays -- after creation and whenever the delay window was re-allocated
+static void build_lane_views(qmc_walkers* w) {
+    const SysDev& s = w->sys->d;
+    const WalkDev& d = w->d;
+    const int w0 = w->n_lanes == 2 ? (d.W + 1) / 2 : d.W;
+    for (int l = 0; l < w->n_lanes; l++) {
+        Lane& L = w->lane[l];
+        WalkDev own = L.d;  // the lane's private buffers survive the rebuild
+        L.off = l == 0 ? 0 : w0;
+        const long o = L.off;
+        L.d = d;
+        L.d.W = l == 0 ? w0 : d.W - w0;
+        L.d.lean = w->n_lanes == 2 ? 1 : 0;
+        L.d.R = d.R + o * 3 * d.nep;
+        for (int sp = 0; sp < 2; sp++) {
+            L.d.AinvT[sp] = d.AinvT[sp] + o * s.nsp[sp] * s.nsp[sp];
+            L.d.Orb[sp] = d.Orb[sp] + o * 5 * s.nsp[sp] * s.nsp[sp];
+        }
+        L.d.V = d.V + o * 5 * d.ldv;
+        L.d.Vbuf = d.Vbuf + o * d.kp * d.ldv; L.d.Wbuf = d.Wbuf + o * d.kp * d.ldv; L.d.W2 = d.W2 + o * d.kp * d.ldv;
+        L.d.SinvT = d.SinvT + o * d.kp * d.kp; L.d.YT = d.YT + o * d.ldv * d.kp;
+        L.d.bvec = d.bvec + o * d.kp; L.d.cvec = d.cvec + o * d.kp; L.d.xcol = d.xcol + o * d.ldv;
+        L.d.plist = d.plist + o * d.kp; L.d.mcount = d.mcount + o;
+        L.d.rp = d.rp + o * 3; L.d.G = d.G + o * 3; L.d.gJn = d.gJn + o * 3; L.d.u = d.u + o; L.d.dJ = d.dJ + o;
+        L.d.logpsi = d.logpsi + o; L.d.sign = d.sign + o; L.d.flags = d.flags + o;
+        L.d.eloc = d.eloc + o; L.d.ekin = d.ekin + o; L.d.ebuf = d.ebuf + o * s.ne * 2;
+        L.d.bits = d.bits ? d.bits + o : nullptr;                       // log rows keep the crowd's stride (log_off)
+        L.d.ratio_log = d.ratio_log ? d.ratio_log + o : nullptr; L.d.pacc_log = d.pacc_log ? d.pacc_log + o : nullptr;
+        L.d.first_walker = d.first_walker + (uint32_t)o;
+        L.d.weight = d.weight + o; L.d.eold = d.eold + o; L.d.tau_eff = d.tau_eff + o; L.d.dr2p = d.dr2p + o; L.d.dr2 = d.dr2 + o * 2;
+        if (l == 1) {  // private: basis matrix, stream-K workspace and flags, screening plan
+            L.d.Phi = own.Phi; L.d.mo_ws = own.mo_ws; L.d.mo_flags = own.mo_flags;
+            L.d.tilemax = own.tilemax; L.d.plan_cnt = own.plan_cnt; L.d.plan_pre = own.plan_pre; L.d.plan_kb = own.plan_kb;
+        }
+        L.d.mt = (5 * L.d.W + 127) / 128;
+    }
 }
 
 extern "C" void qmc_walkers_destroy(qmc_walkers* w) {
@@ -472,6 +560,27 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     CUW(w->pool.alloc((void**)&w->d_status, 4, st));
     rc = alloc_window(w, 16);
     if (rc) { std::string m = g_err; destroy_walkers(w); return fail(rc, m); }
+    w->n_lanes = 1;
+    memset(w->lane, 0, sizeof(w->lane));
+    w->lane[0].stream = st;
+    w->lane[0].mo_epoch = &w->mo_epoch;
+    w->lane[1].mo_epoch = &w->lane[1].own_epoch;
+    if (choose_lanes(sys, d, flags) == 2) {
+        Lane& L = w->lane[1];
+        const int w1 = n_walkers - (n_walkers + 1) / 2, mt1 = (5 * w1 + 127) / 128;
+        CUW(cudaStreamCreateWithFlags(&L.stream, cudaStreamNonBlocking));
+        CUW(cudaEventCreateWithFlags(&w->fork_ev, cudaEventDisableTiming));
+        CUW(cudaEventCreateWithFlags(&w->lane[0].done, cudaEventDisableTiming));
+        CUW(cudaEventCreateWithFlags(&L.done, cudaEventDisableTiming));
+        w->n_lanes = 2;
+        CUW(w->pool.alloc((void**)&L.d.Phi, phiT_bytes(s, 5 * w1), st));
+        CUW(w->pool.alloc((void**)&L.d.mo_ws, mo_ws_bytes(sys->n_sm), st));
+        CUW(w->pool.alloc((void**)&L.d.mo_flags, (size_t)sys->n_sm * 4, st));
+        CUW(w->pool.alloc((void**)&L.d.tilemax, (size_t)mt1 * s.kb * 8, st));
+        CUW(w->pool.alloc((void**)&L.d.plan_cnt, (size_t)mt1 * 4, st));
+        CUW(w->pool.alloc((void**)&L.d.plan_pre, (size_t)(mt1 + 1) * 4, st));
+        CUW(w->pool.alloc((void**)&L.d.plan_kb, (size_t)mt1 * s.kb * 4, st));
+    }
 
     // positions in (host or device) -> walker-major SoA
     {
@@ -533,7 +642,7 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
 
 // ------------------------------------------------------------------------------------------------ profiling hooks
 
-static void prof_begin(qmc_walkers* w, int stage, bool on) {
+static void prof_begin(qmc_walkers* w, cudaStream_t stream, int stage, bool on) {
     if (!on) return;
     StageTimer& t = w->timer;
     if (t.used + 2 > t.ev.size()) {
@@ -545,18 +654,19 @@ static void prof_begin(qmc_walkers* w, int stage, bool on) {
     }
     t.stage.resize(t.ev.size() / 2);
     t.stage[t.used / 2] = stage;
-    cudaEventRecord(t.ev[t.used], w->stream);
+    cudaEventRecord(t.ev[t.used], stream);
 }
-static void prof_end(qmc_walkers* w, bool on) {
+static void prof_end(qmc_walkers* w, cudaStream_t stream, bool on) {
     if (!on) return;
     StageTimer& t = w->timer;
-    cudaEventRecord(t.ev[t.used + 1], w->stream);
+    cudaEventRecord(t.ev[t.used + 1], stream);
     t.used += 2;
 }
 static void prof_collect(qmc_walkers* w) {
     StageTimer& t = w->timer;
     if (t.used == 0) return;
     cudaStreamSynchronize(w->stream);
+    if (w->n_lanes == 2) cudaStreamSynchronize(w->lane[1].stream);
     for (size_t i = 0; i < t.used; i += 2) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, t.ev[i], t.ev[i + 1]) == cudaSuccess) {
@@ -646,62 +756,65 @@ static int sweep_small(qmc_walkers* w, const SweepCall& c) {
     return QMC_OK;
 }
 
-// everything one set launches for electron p of spin sp in sweep t of the call; in_window: moves pending in its delay window
-static int sweep_electron(qmc_walkers* w, const SweepCall& c, int t, int sp, int p, int* in_window) {
+// everything one lane launches for electron p of spin sp in sweep t of the call; in_window: moves pending in its delay window
+static int sweep_electron(qmc_walkers* w, Lane& L, const SweepCall& c, int t, int sp, int p, int* in_window) {
     const SysDev& s = w->sys->d;
-    WalkDev& d = w->d;
-    cudaStream_t st = w->stream;
+    const WalkDev& d = L.d;
+    cudaStream_t st = L.stream;
     const int ns = s.ns[sp], e0 = sp == 0 ? 0 : s.ns[0];
     const int e = e0 + p;
-    const long log_off = ((long)(c.log_t0 + t) * s.ne + e) * d.W;
+    const long log_off = ((long)(c.log_t0 + t) * s.ne + e) * w->d.W;   // the crowd's stride: the lane's log pointers are offset
     const bool prof = w->prof_stride > 0 && (p % w->prof_stride) == 0;
     const bool pf = w->prof_stride > 0;
     if (*in_window == 0) {  // first proposal of a window: nothing to fuse it with
-        prof_begin(w, 0, pf);
+        prof_begin(w, st, 0, pf);
         CU(launch_step(s, d, sp, -1, p, 0, w->step, c.tau, 1, st));
-        prof_end(w, pf);
+        prof_end(w, st, pf);
     }
-    prof_begin(w, 1, prof);
+    prof_begin(w, st, 1, prof);
     const bool screen = d.screen_theta >= 0.0;
     CU(launch_basis(s, d.rp, d.W, d.Phi, screen ? d.tilemax : nullptr, st));
-    prof_end(w, prof);
-    prof_begin(w, 2, prof);
+    prof_end(w, st, prof);
+    prof_begin(w, st, 2, prof);
     if (screen) CU(launch_mo_plan(s, sp, d, 5 * d.W, st));
-    CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, d.mo_grid), ++w->mo_epoch,
+    CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, w->d.mo_grid), ++*L.mo_epoch,
                  screen ? &d : nullptr, st));
-    prof_end(w, prof);
+    prof_end(w, st, prof);
     ++*in_window;
     if (*in_window == c.delay_k || p == ns - 1) {
-        prof_begin(w, 0, pf);
+        prof_begin(w, st, 0, pf);
         CU(launch_step(s, d, sp, p, -1, log_off, w->step, c.tau, 1, st));
-        prof_end(w, pf);
-        prof_begin(w, 4, pf);
+        prof_end(w, st, pf);
+        prof_begin(w, st, 4, pf);
         CU(launch_flush(s, d, sp, st));
-        prof_end(w, pf);
+        prof_end(w, st, pf);
         *in_window = 0;
     } else {  // accept/reject of p and proposal of p + 1 in one launch
         const bool prof2 = w->prof_stride > 0 && ((p + 1) % w->prof_stride) == 0;
-        prof_begin(w, 3, prof2);
+        prof_begin(w, st, 3, prof2);
         CU(launch_step(s, d, sp, p, p + 1, log_off, w->step, c.tau, 1, st));
-        prof_end(w, prof2);
+        prof_end(w, st, prof2);
     }
     return QMC_OK;
 }
 
-// end of a sweep of one set: E_L, the DMC weight, the sweep counter
+// end of a sweep of one set: E_L, the DMC weight (lane by lane), the sweep counter
 static int sweep_finish_step(qmc_walkers* w, const SweepCall& c) {
     const bool pf = w->prof_stride > 0;
-    prof_begin(w, 5, pf);
-    CU(launch_eloc(w->sys->d, w->d, w->stream));
-    prof_end(w, pf);
-    if (c.dmc) CU(launch_dmc_weight(w->d, c.tau, c.e_trial, c.e_trial_dev, w->stream));
+    for (int l = 0; l < w->n_lanes; l++) {
+        Lane& L = w->lane[l];
+        prof_begin(w, L.stream, 5, pf);
+        CU(launch_eloc(w->sys->d, L.d, L.stream));
+        prof_end(w, L.stream, pf);
+        if (c.dmc) CU(launch_dmc_weight(L.d, c.tau, c.e_trial, c.e_trial_dev, L.stream));
+    }
     w->step++;
     if (w->timer.used > 8192) prof_collect(w);
     return QMC_OK;
 }
 
-// n_sets walker sets of ONE system advance together: the host enqueues electron p of every set (each on its own stream)
-// before electron p + 1 of any, so that the HBM-bound stages of one crowd overlap the contraction of another
+// n_sets walker sets of ONE system advance together: the host enqueues electron p of every lane of every set (each on its
+// own stream) before electron p + 1 of any, so that the HBM-bound stages of one lane overlap the contraction of another
 static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
     std::vector<qmc_walkers*> large;
     for (int i = 0; i < n_sets; i++) {
@@ -713,16 +826,26 @@ static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
         if (small) { rc = sweep_small(sets[i], ci); if (rc) return rc; }
         else large.push_back(sets[i]);
     }
-    if (large.empty()) return QMC_OK;
+    if (large.empty() || c.nsteps == 0) return QMC_OK;
     const SysDev& s = large[0]->sys->d;
-    std::vector<int> in_window(large.size(), 0);
-    for (qmc_walkers* w : large)
-        if (c.dmc) CU(launch_dmc_begin(w->d, w->stream));
+    struct Unit { qmc_walkers* w; Lane* L; int in_window; };
+    std::vector<Unit> units;
+    for (qmc_walkers* w : large) {
+        build_lane_views(w);
+        if (w->n_lanes == 2) {  // the second lane joins the crowd's stream order here and leaves it at the end of the call
+            CU(cudaEventRecord(w->fork_ev, w->stream));
+            CU(cudaStreamWaitEvent(w->lane[1].stream, w->fork_ev, 0));
+        }
+        for (int l = 0; l < w->n_lanes; l++) {
+            units.push_back(Unit{w, &w->lane[l], 0});
+            if (c.dmc) CU(launch_dmc_begin(w->lane[l].d, w->lane[l].stream));
+        }
+    }
     for (int t = 0; t < c.nsteps; t++) {
         for (int sp = 0; sp < 2; sp++)
             for (int p = 0; p < s.ns[sp]; p++)
-                for (size_t i = 0; i < large.size(); i++) {
-                    int rc = sweep_electron(large[i], c, t, sp, p, &in_window[i]);
+                for (Unit& u : units) {
+                    int rc = sweep_electron(u.w, *u.L, c, t, sp, p, &u.in_window);
                     if (rc) return rc;
                 }
         for (qmc_walkers* w : large) {
@@ -730,6 +853,11 @@ static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
             if (rc) return rc;
         }
     }
+    for (qmc_walkers* w : large)
+        if (w->n_lanes == 2) {
+            CU(cudaEventRecord(w->lane[1].done, w->lane[1].stream));
+            CU(cudaStreamWaitEvent(w->stream, w->lane[1].done, 0));
+        }
     return QMC_OK;
 }
 
@@ -1163,15 +1291,16 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
         return fail(QMC_ERR_ARG, "qmc_time_stage: bad argument");
     GUARD(w->sys);
     const SysDev& s = w->sys->d;
-    WalkDev& d = w->d;
     cudaStream_t st = w->stream;
     if (s.ns[spin] == 0) return fail(QMC_ERR_ARG, "qmc_time_stage: empty spin block");
     const int kp = round_up(delay_k, 16);
-    if (kp != d.kp) {
+    if (kp != w->d.kp) {
         int rc = alloc_window(w, kp);
         if (rc) return rc;
-        CU(launch_window_reset(d, st));
+        CU(launch_window_reset(w->d, st));
     }
+    build_lane_views(w);
+    WalkDev& d = w->lane[0].d;   // what a sweep launches: the first lane's kernels (the whole crowd if it runs as one lane)
     const int p = 0, e = spin == 0 ? 0 : s.ns[0];
     cudaEvent_t e0, e1;
     CU(cudaEventCreate(&e0));
@@ -1204,7 +1333,7 @@ extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, 
     if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    if (stage == 4) { cudaError_t e2 = launch_window_reset(d, st); if (err == cudaSuccess) err = e2; }
+    if (stage == 4) { cudaError_t e2 = launch_window_reset(w->d, st); if (err == cudaSuccess) err = e2; }
     CU(err);
     CU(cudaStreamSynchronize(st));
     *ms_per_launch = (double)ms / reps;

@@ -62,6 +62,7 @@ struct SysDev {
 
 struct WalkDev {
     int W, ne, nep, ldv, kp;
+    int lean;   // this set of walkers is one LANE of a crowd (its kernels share the SMs with the other lane's contraction)
     double* R;
     double* AinvT[2];
     double* Orb[2];

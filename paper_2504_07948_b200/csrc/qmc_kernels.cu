@@ -258,8 +258,8 @@ __global__ void __launch_bounds__(256) k_mo_plan(const double* __restrict__ tile
         int acc = 0;
         for (int tm = 0; tm < MT; tm++) { pre[tm] = acc; acc += NT * cnt[tm]; }
         pre[MT] = acc;
-        work[0] += (unsigned long long)acc;
-        work[1] += (unsigned long long)MT * NT * KB;
+        atomicAdd(&work[0], (unsigned long long)acc);   // (the lanes of a crowd plan concurrently)
+        atomicAdd(&work[1], (unsigned long long)MT * NT * KB);
     }
 }
 
@@ -300,12 +300,13 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 // a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st) {
-    static SmemAttr attr[2];
-    const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp);
-    const bool wide = step_threads(s.nsp[spin]) == 512;
-    const cudaError_t er = wide ? attr[1].ensure(k_step<512>, smem) : attr[0].ensure(k_step<128>, smem);
+    static SmemAttr attr[3];
+    const int pt = step_threads(s.nsp[spin], wd.lean != 0);
+    const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp, wd.lean != 0);
+    const cudaError_t er = pt == 512 ? attr[2].ensure(k_step<512>, smem) : (pt == 256 ? attr[1].ensure(k_step<256>, smem) : attr[0].ensure(k_step<128>, smem));
     if (er != cudaSuccess) return er;
-    if (wide) k_step<512><<<wd.W, 512, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+    if (pt == 512) k_step<512><<<wd.W, 512, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+    else if (pt == 256) k_step<256><<<wd.W, 256, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     else k_step<128><<<wd.W, 128, smem, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
     COUNT_LAUNCH();
     return cudaGetLastError();

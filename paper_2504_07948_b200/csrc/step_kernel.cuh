@@ -19,8 +19,10 @@
 namespace qmc {
 
 // threads per walker: 512 for the large systems the kernel was tuned on (8 KB rows at config 2), 128 where a row of the
-// inverse is at most 256 doubles -- there 512 threads would mostly wait at barriers, and four times as many CTAs fit an SM
-__host__ __device__ inline int step_threads(int nsp) { return nsp <= 256 ? 128 : 512; }
+// inverse is at most 256 doubles -- there 512 threads would mostly wait at barriers, and four times as many CTAs fit an SM.
+// lean: the crowd runs as two lanes whose step kernels share the SMs with the OTHER lane's persistent contraction
+// (168 registers x 288 threads resident): 256 threads x 64 registers is what fits beside it.
+__host__ __device__ inline int step_threads(int nsp, bool lean = false) { return nsp <= 256 ? 128 : (lean ? 256 : 512); }
 
 // shared-memory carve-up (in doubles)
 struct StepLayout {
@@ -32,7 +34,7 @@ struct StepLayout {
         red = ts + kp + 1; bc = red + 8 * PW; total = bc + 16;
     }
 };
-inline size_t step_smem_bytes(int nsp, int kp) { return (size_t)StepLayout(nsp, kp, step_threads(nsp) / 32).total * sizeof(double); }
+inline size_t step_smem_bytes(int nsp, int kp, bool lean = false) { return (size_t)StepLayout(nsp, kp, step_threads(nsp, lean) / 32).total * sizeof(double); }
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 
@@ -266,7 +268,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
     const int p = p_prop, e = e0 + p;
     const int m = m_old + (accepted ? 1 : 0);
     if (m > 0) {
-        // c = S^-1 b: c_n = sum_l SinvT[l][n] b_l, 4 threads per n over interleaved l, fixed-order combine (kp <= 128)
+        // c = S^-1 b: c_n = sum_l SinvT[l][n] b_l, PT / 128 threads per n over interleaved l, fixed-order combine (kp <= 128)
         constexpr int CP = PT / 128;  // threads per n
         {
             const int n = tid & 127, q = tid >> 7;
@@ -277,7 +279,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
         }
         __syncthreads();
         for (int n = tid; n < m; n += PT) {
-            const double c = CP == 4 ? (c4[n] + c4[128 + n]) + (c4[256 + n] + c4[384 + n]) : c4[n];
+            const double c = CP == 4 ? (c4[n] + c4[128 + n]) + (c4[256 + n] + c4[384 + n]) : (CP == 2 ? c4[n] + c4[128 + n] : c4[n]);
             cs[n] = c;
             wd.cvec[(long)w * kp + n] = c;
         }
