@@ -50,10 +50,12 @@ def parse():
                     help="row f4: the paper's own regime -- water clusters of 8/16/24/152 valence electrons, 4320 walkers per GPU "
                          "(PAPER.md L279-302) -- on the one-launch small-system path and on the per-electron path; one JSON line each")
     ap.add_argument("--one-lane", action="store_true", help="QMC_ONE_LANE: the crowd as one lane (the round-1 schedule), for comparison")
+    ap.add_argument("--mo-ctas", type=int, default=0, help="qmc_set_mo_ctas of the headline walker set (0 = all SMs)")
     ap.add_argument("--no-screened", action="store_true", help="skip the extra leg with QMC_SCREEN_MO")
     ap.add_argument("--no-dmc", action="store_true", help="skip the untimed row-f1 leg (one DMC generation + reconfiguration)")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-crowds", action="store_true", help="skip the two-crowds leg")
+    ap.add_argument("--crowds", action="store_true", help="also run the two-crowds leg (qmc_sweep_crowds over two walker sets; superseded by "
+                                                          "the lanes inside qmc_sweep, kept for comparison)")
     ap.add_argument("--crowd-ctas", type=int, default=124, help="CTAs of each crowd's contraction in the two-crowds leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-moves", type=int, default=96, help="electron moves per walker in the CPU-baseline sample")
@@ -250,6 +252,8 @@ def run_ours(args):
     pos_dev = pos_host.cuda()
     base_flags = qb.QMC_ONE_LANE if args.one_lane else 0
     gw = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=base_flags)
+    if args.mo_ctas:
+        qb.qmc_set_mo_ctas(gw, args.mo_ctas)
     for _ in range(args.warmup):
         qb.qmc_sweep(gw, 1, wl.tau, k)
     qb.qmc_synchronize(gw)
@@ -271,7 +275,7 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
     st1 = qb.qmc_get_stats(gw)
     eloc = qb.qmc_get_eloc(gw)[0].clone()
-    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not (args.no_screened and args.no_crowds) else None
+    dense_bits = qb.qmc_get_accept_log(gw).cpu().numpy() if not (args.no_screened and (not args.crowds)) else None
     # ---- the per-stage times come from a SECOND pass of K sweeps on the same crowd with the in-situ stage timers on (CUDA
     # events around every prof_stride-th electron's launches): the headline above is timed without that instrumentation
     qb.qmc_set_profiling(gw, args.prof_stride)
@@ -282,7 +286,22 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_profiled_pass = pe0.elapsed_time(pe1)
     stage = qb.qmc_get_stage_times(gw)
+    mo_span_us, mo_span_min_us, mo_span_n = qb.qmc_get_mo_spans(gw)
+    n_lanes, lane_walkers = qb.qmc_get_lanes(gw)
     qb.qmc_set_profiling(gw, 0)
+    # ---- the stages one at a time: with two lanes the in-situ event times above include queueing behind the other lane's
+    # kernels, so every stage's own roofline fraction is measured on a crowd of the same size moved as ONE lane (2 profiled
+    # sweeps after a warm-up sweep): there the launches of a sweep are a chain and each event pair brackets one kernel alone
+    if n_lanes == 2:
+        gwa = qb.qmc_walkers_create(gsys, pos_dev, wl.seed, first_walker_id=lo, flags=qb.QMC_ONE_LANE)
+        qb.qmc_sweep(gwa, 1, wl.tau, k)
+        qb.qmc_set_profiling(gwa, args.prof_stride)
+        qb.qmc_sweep(gwa, 2, wl.tau, k)
+        sa = qb.qmc_get_stage_times(gwa)
+        qb.qmc_walkers_destroy(gwa)
+    else:
+        sa = stage
+    alone = {st_: (sa[st_][0] / sa[st_][1] if sa[st_][1] else None) for st_ in sa}
     n_moves = st1["proposed"] - st0["proposed"]
     n_acc = st1["accepted"] - st0["accepted"]
     assert n_moves == W * sysm.n_elec * args.steps, (n_moves, W, sysm.n_elec, args.steps)
@@ -321,7 +340,7 @@ def run_ours(args):
     # contraction of each limited to 124 CTAs (the basis / step kernels of one crowd overlap the contraction of the
     # other).  Reported beside the headline, not as it: the headline and its roofline are the single-crowd run above.
     crowds = None
-    if not args.no_crowds and W >= 2:
+    if not (not args.crowds) and W >= 2:
         half = W // 2
         cstreams = [torch.cuda.Stream() for _ in range(2)]
         csets = []
@@ -450,9 +469,14 @@ def run_ours(args):
     value = red["n_moves"] / secs
     ns, nb = sysm.n_up, sysm.n_basis
     mo_ms, mo_n = stage["mo"]
-    mo_avg_ms = mo_ms / max(mo_n, 1)
-    mo_flop = 2.0 * 5 * W * nb * ns
-    achieved = mo_flop / (mo_avg_ms * 1e-3) * 1e-12 if mo_n else None
+    mo_events_ms = mo_ms / max(mo_n, 1)
+    # one launch contracts the rows of ONE lane; its duration is the span of the launch on the GPU (first CTA start to
+    # last CTA end, %globaltimer, sampled launches of the profiled pass) -- with two lanes an event pair on the stream also
+    # counts the time the kernel waited for the SMs of the other lane's contraction
+    W_launch = sum(lane_walkers) / n_lanes
+    mo_flop = 2.0 * 5 * W_launch * nb * ns
+    mo_avg_ms = mo_span_us * 1e-3 if mo_span_n else mo_events_ms
+    achieved = mo_flop / (mo_avg_ms * 1e-3) * 1e-12 if mo_avg_ms else None
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "mo_kernel_traffic.json")
     if os.path.exists(tpath):
@@ -479,14 +503,20 @@ def run_ours(args):
                       peak=peak, unit="TFLOP/s", frac=(achieved / peak) if achieved else None, traffic=traffic,
                       peak_source="FP64 DMMA issue-rate loop measured in this run (qmc_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                       peak_alt_bf16_scaled=(peaks.get("bf16_tflops_sustained", 0) * 37.2 / 2250.0) or None,
-                      flop_per_launch=mo_flop, ms_per_launch=mo_avg_ms, launches_timed=int(mo_n),
-                      share_of_step=share["mo"] / tot_share),
+                      flop_per_launch=mo_flop, ms_per_launch=mo_avg_ms, launches_timed=int(mo_span_n or mo_n),
+                      ms_per_launch_stream_events=mo_events_ms,
+                      timing="span of the sampled launches on the GPU (%globaltimer stamps of every CTA)" if mo_span_n else "CUDA events on the stream",
+                      rows_per_launch=5 * W_launch, lanes=n_lanes,
+                      share_of_step=(mo_avg_ms * n_lanes * sysm.n_elec) / (red["elapsed_ms"] / args.steps)),
         fp64_tflops_model=flop_model(sysm, red["n_moves"], n_acc * world) / secs * 1e-12,
         accept_frac=n_acc / max(n_moves, 1),
         stage_ms_per_launch=stage_ms,
         stage_timing="second pass of the same K sweeps with qmc_set_profiling on (%.1f ms per sweep against %.1f unprofiled)" % (
             ms_profiled_pass / args.steps, red["elapsed_ms"] / args.steps),
-        stage_roofline=stage_rooflines(sysm, W, k, n_acc / max(n_moves, 1), stage_ms, hbm_gbs, peak),
+        stage_roofline=stage_rooflines(sysm, W, k, n_acc / max(n_moves, 1), alone, hbm_gbs, peak),
+        stage_roofline_note="every stage alone on the GPU: the same crowd moved as ONE lane (QMC_ONE_LANE, 2 profiled sweeps, in-situ CUDA events); "
+                            "in the two-lane sweep the stages of the lanes overlap and their event times (stage_ms_per_launch) include queueing",
+        lanes=dict(n=n_lanes, walkers=lane_walkers),
         hbm_peak_source="MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "6.65 TB/s of fallback (B200_PROFILING.md)",
         stage_share={s: share[s] / tot_share for s in share},
         eloc_mean=red["e_sum"] / red["n_walkers"],

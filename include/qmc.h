@@ -261,6 +261,14 @@ int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, d
  * kernels).  stride = 0 turns it off and clears the totals. */
 int qmc_set_profiling(qmc_walkers* w, int stride);
 int qmc_get_stage_times(qmc_walkers* w, double* ms /* [6] */, uint64_t* counts /* [6] */);
+/* Lanes of a walker set (see QMC_ONE_LANE): *n_lanes = 1 or 2; walkers_per_lane[2] (may be NULL) = their sizes. */
+int qmc_get_lanes(const qmc_walkers* w, int* n_lanes, int* walkers_per_lane);
+/* Span on the GPU of the contraction launches that the in-situ profiling sampled (qmc_set_profiling stride > 0): every CTA
+ * of such a launch stamps %globaltimer when it starts and when it ends; the span of a launch is last end - first start.
+ * With two lanes the stream events of qmc_get_stage_times also count the time a kernel waited for SMs that the other
+ * lane's contraction still held; the span does not.  mean_us / min_us (may be NULL) over *n_launches launches (at most
+ * 8192 are recorded).  Synchronises the stream(s). */
+int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, uint64_t* n_launches);
 /* Register-resident DMMA issue-rate loop for `ms_target` milliseconds: the FP64 ceiling of this GPU as
  * it runs now (used as the roofline denominator of the contraction stages). */
 int qmc_measure_fp64_peak(double ms_target, double* tflops, void* cuda_stream);

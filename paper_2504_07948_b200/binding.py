@@ -28,7 +28,7 @@ EXPORTED = [
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
     "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl", "qmc_set_mo_ctas", "qmc_sweep_crowds",
-    "qmc_release_scratch", "qmc_philox_words",
+    "qmc_release_scratch", "qmc_philox_words", "qmc_get_lanes", "qmc_get_mo_spans",
 ]
 
 
@@ -102,6 +102,8 @@ def load_library(path: str | None = None):
     lib.qmc_dmc_run.argtypes = [vp, i, d, i, d, d, i, d, C.POINTER(d), vp, vp]
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_release_scratch.argtypes = [vp]
+    lib.qmc_get_lanes.argtypes = [vp, C.POINTER(i), C.POINTER(i)]
+    lib.qmc_get_mo_spans.argtypes = [vp, C.POINTER(d), C.POINTER(d), C.POINTER(u64)]
     lib.qmc_philox_words.argtypes = [i, vp, vp, vp]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
@@ -316,6 +318,21 @@ def qmc_philox_words(ctr_key, stream=None):
     out = np.zeros((ck.shape[0], 4), np.uint32)
     _check(load_library().qmc_philox_words(ck.shape[0], _ptr(ck), _ptr(out), _stream_ptr(stream)))
     return out
+
+
+def qmc_get_lanes(walkers: Walkers):
+    """(n_lanes, [walkers of lane 0, walkers of lane 1])"""
+    n = C.c_int()
+    per = (C.c_int * 2)()
+    _check(load_library().qmc_get_lanes(walkers.handle, C.byref(n), per))
+    return n.value, [per[0], per[1]]
+
+
+def qmc_get_mo_spans(walkers: Walkers):
+    """(mean, min) span in microseconds of the profiled contraction launches on the GPU, and how many were recorded"""
+    a, b, n = C.c_double(), C.c_double(), C.c_uint64()
+    _check(load_library().qmc_get_mo_spans(walkers.handle, C.byref(a), C.byref(b), C.byref(n)))
+    return a.value, b.value, n.value
 
 
 def qmc_set_mo_ctas(walkers: Walkers, n_ctas):

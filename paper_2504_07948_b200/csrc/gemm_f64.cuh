@@ -21,24 +21,37 @@ namespace qmc {
 // its launch site) remembers, per device ordinal, how many bytes have been granted there, so a process that drives several
 // GPUs -- or several host threads -- sets the attribute where and when it is needed and nowhere else.  Racing threads at
 // worst set the same attribute twice.
+// carveout_percent >= 0: the first call on a device also sets the kernel's preferred L1 / shared-memory split (percent of
+// the largest shared-memory size).  Only the contraction asks: the step and basis kernels of one lane are meant to share
+// an SM with the resident contraction CTA of the other lane, and an SM whose split was sized for the contraction alone
+// (the driver's default is the smallest split that fits the running kernel) would have no room for them; the other
+// kernels keep the default (asking for the largest split everywhere cost k_step 18 % of its speed: it lives on L1).
 struct SmemAttr {
     static constexpr int MAX_DEV = 64;
-    std::atomic<size_t> granted[MAX_DEV];   // zero-initialised (static storage); 48 KB need no grant
+    std::atomic<size_t> granted[MAX_DEV];   // zero-initialised (static storage): 0 = never configured on that device
     template <class K>
-    cudaError_t ensure(K kernel, size_t bytes) {
-        if (bytes <= 48 * 1024) return cudaSuccess;
+    cudaError_t ensure(K kernel, size_t bytes, int carveout_percent = -1) {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return e;
         const bool cached = dev >= 0 && dev < MAX_DEV;
-        if (cached && bytes <= granted[dev].load(std::memory_order_acquire)) return cudaSuccess;
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-        if (e == cudaSuccess && cached) {
-            size_t cur = granted[dev].load(std::memory_order_relaxed);
-            while (cur < bytes && !granted[dev].compare_exchange_weak(cur, bytes, std::memory_order_release)) {
+        const size_t have = cached ? granted[dev].load(std::memory_order_acquire) : 0;
+        const size_t want = bytes > 48 * 1024 ? bytes : 48 * 1024;
+        if (have >= want) return cudaSuccess;
+        if (have == 0 && carveout_percent >= 0) {
+            e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, carveout_percent);
+            if (e != cudaSuccess) return e;
+        }
+        if (bytes > 48 * 1024) {
+            e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+            if (e != cudaSuccess) return e;
+        }
+        if (cached) {
+            size_t cur = have;
+            while (cur < want && !granted[dev].compare_exchange_weak(cur, want, std::memory_order_release)) {
             }
         }
-        return e;
+        return cudaSuccess;
     }
 };
 

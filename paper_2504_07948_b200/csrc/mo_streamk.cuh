@@ -32,7 +32,16 @@ constexpr int MO_B_STAGE = MO_BK * MO_BLD;   // doubles
 #endif
 constexpr int MO_STAGES = QMC_MO_STAGES;
 constexpr int MO_CONSUMER_WARPS = 8;
-constexpr int MO_THREADS = (MO_CONSUMER_WARPS + 1) * 32;
+// QMC_MO_MERGED (default): no ninth warp -- lane 0 of consumer warp 0 issues the TMA copies between its DMMA steps.  An SM's
+// register file is four separate 16K-register files, one per sub-partition, and the warps of a CTA are dealt out to them
+// in turn: a ninth warp of 168 registers fills sub-partition 0 (3 x 5376 = 16128), and then no CTA of ANY other kernel
+// can become resident on the SM while the contraction runs (measured with a 34-register probe kernel: its CTAs started
+// only when the contraction's left).  With eight warps every sub-partition keeps 5632 registers free -- two 64-register
+// warps -- which is what the step and basis kernels of the other lane need to run beside the contraction.
+#ifndef QMC_MO_MERGED
+#define QMC_MO_MERGED 1
+#endif
+constexpr int MO_THREADS = (MO_CONSUMER_WARPS + (QMC_MO_MERGED ? 0 : 1)) * 32;
 constexpr size_t MO_SMEM_BYTES = (size_t)MO_STAGES * (MO_A_STAGE + MO_B_STAGE) * 8 + 2 * MO_STAGES * 8 + 16;
 constexpr int MO_TM = 8, MO_TN = 4;  // DMMA tiles per warp (64 x 32)
 constexpr int MO_WS_DOUBLES = MO_BM * MO_BN;  // workspace per CTA
@@ -92,7 +101,16 @@ struct MoArgs {
     const int* plan_cnt;   // [MT]      kept k-blocks of row tile tm (>= 1)
     const int* plan_pre;   // [MT + 1]  NT * (cnt[0] + ... + cnt[tm-1]); plan_pre[MT] = total iterations
     const int* plan_kb;    // [MT][KB]  the kept k-blocks of tm, ascending
+    // optional: [grid][2] %globaltimer (ns) at the start and the end of every CTA -- the span of the launch on the GPU,
+    // which CUDA events on the stream cannot give once two lanes run concurrently (an event pair also counts the time the
+    // kernel waited for SMs)
+    unsigned long long* trace;
 };
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
 // Where a flattened iteration lies.  Dense: tiles of KB iterations.  Screened: the tiles of row tile tm have cnt[tm]
 // iterations each (only the A stages whose largest entry reaches the threshold), tiles ordered tm-major.
@@ -119,7 +137,7 @@ __device__ __forceinline__ MoLoc mo_locate(const MoArgs& g, long it) {
 // iterations per CTA that 128-row tiles would be split over many CTAs (config 1: 20 tiles x 24 k-blocks on 148 CTAs);
 // g.MT then counts 64-row tiles.  Not combined with SCREEN (the plan is per 128-row tile).
 template <bool SCREEN, bool HALF>
-__global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
+__global__ void __maxnreg__(168) k_mo_streamk(MoArgs g) {
     static_assert(!(SCREEN && HALF), "screening plans are per 128-row tile");
     constexpr int BM = HALF ? 64 : 128, TM = BM / 16;
     extern __shared__ __align__(128) unsigned char mo_smem_raw[];
@@ -131,6 +149,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
 #pragma unroll
         for (int s = 0; s < MO_STAGES; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], MO_CONSUMER_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        if (g.trace) g.trace[2 * blockIdx.x] = global_timer_ns();
     }
     __syncthreads();
 
@@ -138,24 +157,55 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
     const long it0 = total * blockIdx.x / gridDim.x, it1 = total * (blockIdx.x + 1) / gridDim.x;
     constexpr uint32_t A_BYTES = BM * MO_ALD * 8, STAGE_BYTES = A_BYTES + MO_B_STAGE * 8;
 
-    if (warp == MO_CONSUMER_WARPS) {
-        // ===== producer: one thread streams the stages of this CTA's iteration range =====
-        if (lane == 0) {
-            uint32_t n = 0;
-            for (long it = it0; it < it1; it++, n++) {
-                const int s = n % MO_STAGES;
-                const uint32_t round = n / MO_STAGES;
-                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
-                const MoLoc L = mo_locate<SCREEN>(g, it);
-                const int tm = L.tm, tn = L.tn, kb = SCREEN ? g.plan_kb[(long)tm * g.KB + L.i] : L.i;
-                double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
-                mbar_expect_tx(&full[s], STAGE_BYTES);
-                bulk_g2s(As, g.PhiT + ((long)(HALF ? tm >> 1 : tm) * g.KB + kb) * MO_A_STAGE + (HALF ? (tm & 1) * BM * MO_ALD : 0), A_BYTES, &full[s]);
-                bulk_g2s(As + MO_A_STAGE, g.CT + ((long)tn * g.KB + kb) * MO_B_STAGE, MO_B_STAGE * 8, &full[s]);
+    // ===== producer: one thread streams the stages of this CTA's iteration range.  issue(): the copies of the next
+    // iteration, if its stage is free (block: wait for it); returns false when nothing could be issued.  The position in
+    // the iteration space advances incrementally (no divisions after the first iteration: with the producer merged into
+    // a consumer warp every instruction here is taken from that warp's DMMA stream).
+    long p_it = it0;
+    uint32_t p_n = 0;
+    int p_tm, p_tn, p_i, p_cnt;
+    {
+        const MoLoc L0 = mo_locate<SCREEN>(g, it0 < it1 ? it0 : 0);
+        p_tm = L0.tm; p_tn = L0.tn; p_i = L0.i; p_cnt = L0.cnt;
+    }
+    auto issue = [&](bool block) -> bool {
+        if (p_it >= it1) return false;
+        const int s = p_n % MO_STAGES;
+        const uint32_t round = p_n / MO_STAGES;
+        if (round > 0) {
+            if (block) mbar_wait(&empty[s], (round - 1) & 1);
+            else if (!mbar_try_wait(&empty[s], (round - 1) & 1)) return false;
+        }
+        const int kb = SCREEN ? g.plan_kb[(long)p_tm * g.KB + p_i] : p_i;
+        double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
+        mbar_expect_tx(&full[s], STAGE_BYTES);
+        bulk_g2s(As, g.PhiT + ((long)(HALF ? p_tm >> 1 : p_tm) * g.KB + kb) * MO_A_STAGE + (HALF ? (p_tm & 1) * BM * MO_ALD : 0), A_BYTES, &full[s]);
+        bulk_g2s(As + MO_A_STAGE, g.CT + ((long)p_tn * g.KB + kb) * MO_B_STAGE, MO_B_STAGE * 8, &full[s]);
+        p_it++; p_n++;
+        if (++p_i == p_cnt) {   // next tile (tiles are ordered tm-major; a row tile's tiles all have cnt[tm] iterations)
+            p_i = 0;
+            if (++p_tn == g.NT) {
+                p_tn = 0;
+                p_tm++;
+                if (SCREEN && p_tm < g.MT) p_cnt = g.plan_cnt[p_tm];
             }
         }
+        return true;
+    };
+#if !QMC_MO_MERGED
+    if (warp == MO_CONSUMER_WARPS) {
+        if (lane == 0)
+            while (issue(true)) {
+            }
         return;
     }
+    constexpr bool merged = false;
+#else
+    constexpr bool merged = true;
+    const bool producer = tid == 0;
+    if (producer)
+        for (int s = 0; s < MO_STAGES; s++) issue(false);   // the first round needs no wait
+#endif
 
     // ===== consumers =====
     const int wm0 = (warp >> 2) * (BM / 2), wn0 = (warp & 3) * 32;
@@ -175,6 +225,12 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
             for (int j = 0; j < MO_TN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
         for (int kb = ka; kb < kb_end; kb++, n++) {
             const int s = n % MO_STAGES;
+            if (merged) {
+                // the copies of iteration n must have been issued before anybody can wait for them
+                if (tid == 0)
+                    while (p_n <= n) issue(true);
+                __syncwarp();
+            }
             mbar_wait(&full[s], (n / MO_STAGES) & 1);
             const double* As = stages + (size_t)s * (MO_A_STAGE + MO_B_STAGE);
             const double* Bs = As + MO_A_STAGE;
@@ -189,6 +245,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
                 for (int i = 0; i < TM; i++)
 #pragma unroll
                     for (int j = 0; j < MO_TN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+                if (merged && (kk & 1) && tid == 0 && p_n < n + MO_STAGES) issue(false);   // refill a stage the moment its last reader has left
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);
@@ -254,6 +311,7 @@ __global__ void __launch_bounds__(MO_THREADS, 1) k_mo_streamk(MoArgs g) {
             }
         }
     }
+    if (g.trace && tid == 0) g.trace[2 * blockIdx.x + 1] = global_timer_ns();
 }
 
 }  // namespace qmc

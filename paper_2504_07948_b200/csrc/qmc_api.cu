@@ -13,6 +13,11 @@
 
 using namespace qmc;
 
+static constexpr size_t MO_TRACE_SLOTS = 8192;
+#ifndef QMC_LANE_FREE_SMS
+#define QMC_LANE_FREE_SMS 16
+#endif
+
 static thread_local std::string g_err;
 
 static int fail(int code, const std::string& msg) {
@@ -133,6 +138,8 @@ struct qmc_walkers {
     double* d_emixed;   // [1]
     unsigned mo_epoch;   // stream-K launch counter (flag stamps)
     int prof_stride;     // 0 = off
+    GrowBuf mo_trace;         // [MO_TRACE_SLOTS][n_sm][2] globaltimer stamps of the profiled contraction launches
+    std::vector<int> trace_grid;  // grid of every traced launch
     mutable GrowBuf scratch;  // qmc_get_dlogpsi_dR / qmc_get_deloc_dR / qmc_get_vnl
     mutable GrowBuf bounce;   // device staging of the getters that write to host memory
     StageTimer timer;
@@ -404,6 +411,7 @@ static void destroy_walkers(qmc_walkers* w) {
     }
     w->scratch.release();
     w->bounce.release();
+    w->mo_trace.release();
     w->pool.free_all();
     w->winpool.free_all();
     w->logpool.free_all();
@@ -573,6 +581,11 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
         CUW(cudaEventCreateWithFlags(&w->lane[0].done, cudaEventDisableTiming));
         CUW(cudaEventCreateWithFlags(&L.done, cudaEventDisableTiming));
         w->n_lanes = 2;
+        // Two lanes: each contraction leaves a few SMs to the other lane's kernels.  The step / basis CTAs that share an SM
+        // with a contraction CTA run slowly (one CTA per SM, the FP64 pipe taken); the ones that find a free SM run at
+        // full speed and shorten the lane's chain.  Measured at config 2 (moves/s): 148 CTAs 423 k, 140: 429 k, 132:
+        // 465 k, 124: 457 k, 116: 460 k (one lane: 436 k).  qmc_set_mo_ctas overrides.
+        if (sys->n_sm > 4 * QMC_LANE_FREE_SMS) d.mo_grid = sys->n_sm - QMC_LANE_FREE_SMS;
         CUW(w->pool.alloc((void**)&L.d.Phi, phiT_bytes(s, 5 * w1), st));
         CUW(w->pool.alloc((void**)&L.d.mo_ws, mo_ws_bytes(sys->n_sm), st));
         CUW(w->pool.alloc((void**)&L.d.mo_flags, (size_t)sys->n_sm * 4, st));
@@ -686,6 +699,8 @@ extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
     w->prof_stride = stride;
     memset(w->stage_ms, 0, sizeof(w->stage_ms));
     memset(w->stage_n, 0, sizeof(w->stage_n));
+    w->trace_grid.clear();
+    if (stride > 0) CU(w->mo_trace.reserve(MO_TRACE_SLOTS * 2 * (size_t)w->sys->n_sm * 8, w->stream));
     return QMC_OK;
 }
 extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t* counts /*[6]*/) {
@@ -777,8 +792,13 @@ static int sweep_electron(qmc_walkers* w, Lane& L, const SweepCall& c, int t, in
     prof_end(w, st, prof);
     prof_begin(w, st, 2, prof);
     if (screen) CU(launch_mo_plan(s, sp, d, 5 * d.W, st));
-    CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mo_grid_for(s, sp, 5 * d.W, w->d.mo_grid), ++*L.mo_epoch,
-                 screen ? &d : nullptr, st));
+    const int mgrid = mo_grid_for(s, sp, 5 * d.W, w->d.mo_grid);
+    unsigned long long* trace = nullptr;
+    if (prof && w->mo_trace.p && w->trace_grid.size() < MO_TRACE_SLOTS) {
+        trace = (unsigned long long*)w->mo_trace.p + w->trace_grid.size() * 2 * (size_t)w->sys->n_sm;
+        w->trace_grid.push_back(mgrid);
+    }
+    CU(launch_mo(s, sp, d.Phi, 5 * d.W, d.V, d.ldv, d.mo_ws, d.mo_flags, mgrid, ++*L.mo_epoch, screen ? &d : nullptr, st, trace));
     prof_end(w, st, prof);
     ++*in_window;
     if (*in_window == c.delay_k || p == ns - 1) {
@@ -1000,6 +1020,43 @@ extern "C" int qmc_release_scratch(qmc_walkers* w) {
     CU(cudaStreamSynchronize(w->stream));
     w->scratch.release();
     w->bounce.release();
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_lanes(const qmc_walkers* w, int* n_lanes, int* walkers_per_lane) {
+    if (!w || !n_lanes) return fail(QMC_ERR_ARG, "qmc_get_lanes: null argument");
+    *n_lanes = w->n_lanes;
+    if (walkers_per_lane) {
+        const int w0 = w->n_lanes == 2 ? (w->d.W + 1) / 2 : w->d.W;
+        walkers_per_lane[0] = w0;
+        walkers_per_lane[1] = w->d.W - w0;
+    }
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, uint64_t* n_launches) {
+    if (!w || !mean_us || !n_launches) return fail(QMC_ERR_ARG, "qmc_get_mo_spans: null argument");
+    GUARD(w->sys);
+    *mean_us = 0.0; *n_launches = 0;
+    if (min_us) *min_us = 0.0;
+    const size_t n = w->trace_grid.size(), nsm = (size_t)w->sys->n_sm;
+    if (n == 0 || !w->mo_trace.p) return QMC_OK;
+    CU(cudaStreamSynchronize(w->stream));
+    if (w->n_lanes == 2) CU(cudaStreamSynchronize(w->lane[1].stream));
+    std::vector<unsigned long long> h(n * 2 * nsm);
+    CU(cudaMemcpy(h.data(), w->mo_trace.p, h.size() * 8, cudaMemcpyDeviceToHost));
+    double sum = 0.0, mn = 1e300;
+    for (size_t i = 0; i < n; i++) {
+        unsigned long long t0 = ~0ull, t1 = 0;
+        for (int c = 0; c < w->trace_grid[i]; c++) {
+            t0 = std::min(t0, h[(i * nsm + c) * 2]);
+            t1 = std::max(t1, h[(i * nsm + c) * 2 + 1]);
+        }
+        const double us = (double)(t1 - t0) * 1e-3;
+        sum += us; mn = std::min(mn, us);
+    }
+    *mean_us = sum / n; *n_launches = n;
+    if (min_us) *min_us = mn;
     return QMC_OK;
 }
 

@@ -27,6 +27,9 @@
 #define QMC_UPD_WM 16
 #define QMC_UPD_WN 32
 #endif
+#ifndef QMC_MO_CARVEOUT
+#define QMC_MO_CARVEOUT 86   // percent of 228 KB: the 196 KB split
+#endif
 #ifndef QMC_Y_STAGES
 #define QMC_Y_STAGES 3
 #endif
@@ -272,17 +275,19 @@ cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int row
 
 // plan: NULL for the dense contraction, else the walker set whose plan_* buffers launch_mo_plan has just filled
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
-                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st) {
+                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st, unsigned long long* trace) {
     static SmemAttr attr[3];
-    cudaError_t ea = attr[0].ensure(k_mo_streamk<false, false>, MO_SMEM_BYTES);
-    if (ea == cudaSuccess) ea = attr[1].ensure(k_mo_streamk<true, false>, MO_SMEM_BYTES);
-    if (ea == cudaSuccess) ea = attr[2].ensure(k_mo_streamk<false, true>, MO_SMEM_BYTES);
+    // shared-memory split of an SM that holds a contraction CTA: room for the other lane's step (33 KB) or basis (42 KB) CTA
+    constexpr int CARVE = QMC_MO_CARVEOUT;
+    cudaError_t ea = attr[0].ensure(k_mo_streamk<false, false>, MO_SMEM_BYTES, CARVE);
+    if (ea == cudaSuccess) ea = attr[1].ensure(k_mo_streamk<true, false>, MO_SMEM_BYTES, CARVE);
+    if (ea == cudaSuccess) ea = attr[2].ensure(k_mo_streamk<false, true>, MO_SMEM_BYTES, CARVE);
     if (ea != cudaSuccess) return ea;
     MoArgs g;
     g.PhiT = PhiT; g.CT = s.CT[spin]; g.V = V; g.ldv = ldv;
     g.M = rows; g.N = s.nsp[spin];
     g.MT = (rows + MO_BM - 1) / MO_BM; g.NT = s.nt[spin]; g.KB = s.kb;
-    g.ws = ws; g.flags = flags; g.epoch = epoch;
+    g.ws = ws; g.flags = flags; g.epoch = epoch; g.trace = trace;
     g.plan_cnt = plan ? plan->plan_cnt : nullptr; g.plan_pre = plan ? plan->plan_pre : nullptr; g.plan_kb = plan ? plan->plan_kb : nullptr;
     if (grid < 1) return cudaSuccess;
     // few iterations per CTA: 64-row tiles, so that a tile is split over fewer CTAs and the partial sums are smaller

@@ -8,7 +8,7 @@ namespace qmc {
 cudaError_t launch_basis(const SysDev& s, const double* pts, int n_points, double* PhiT, double* tilemax, cudaStream_t st);
 cudaError_t launch_basis_values(const SysDev& s, const double* pts, int n_points, double* PhiT, cudaStream_t st);
 cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, double* V, long ldv, double* ws, unsigned* flags,
-                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st);
+                      int grid, unsigned epoch, const WalkDev* plan, cudaStream_t st, unsigned long long* trace = nullptr);
 cudaError_t launch_mo_plan(const SysDev& s, int spin, const WalkDev& wd, int rows, cudaStream_t st);
 int mo_grid_for(const SysDev& s, int spin, int rows, int n_sm);
 size_t mo_ws_bytes(int grid);

@@ -37,9 +37,49 @@ struct StepLayout {
 inline size_t step_smem_bytes(int nsp, int kp, bool lean = false) { return (size_t)StepLayout(nsp, kp, step_threads(nsp, lean) / 32).total * sizeof(double); }
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+// COH: the data may have been written earlier in the SAME launch (the window kernel of the mid-size path runs several
+// electron steps per launch): read it through L2 (ld.global.cg), not through the non-coherent read-only path
+template <bool COH>
+__device__ __forceinline__ double2 ld2(const double* p) {
+    return COH ? __ldcg(reinterpret_cast<const double2*>(p)) : __ldg(reinterpret_cast<const double2*>(p));
+}
+
+// The threads that work on one walker: a whole CTA (k_step) or a 128-thread group of a CTA (k_window), which then meets at
+// a named barrier instead of __syncthreads.
+struct CtaSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+template <int NT>
+struct GroupSync {
+    int id;   // named barrier 1..15
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;\n" ::"r"(id), "n"(NT) : "memory"); }
+};
+template <int NT, int NV, class Sync>
+__device__ __forceinline__ void group_sum(double (&v)[NV], double* red /* [NV * NT/32] */, int tid, const Sync& sync) {
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    }
+    sync();  // protect red from a previous use
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; i++) red[i * (NT / 32) + warp] = v[i];
+    }
+    sync();
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+        double sacc = 0.0;
+#pragma unroll
+        for (int k = 0; k < NT / 32; k++) sacc += red[i * (NT / 32) + k];
+        v[i] = sacc;
+    }
+}
 
 // One warp: accA = rowA . vecA and (if rowB) accB = rowB . vecB over n2 double2's; rows in HBM (read-only path),
 // vectors in shared memory; 8 independent 16-byte loads in flight per lane.
+template <bool COH>
 __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const double* vecA, const double* __restrict__ rowB, const double* vecB,
                                           int n2, int lane, double& accA, double& accB) {
     const double2* xa = reinterpret_cast<const double2*>(vecA);
@@ -50,7 +90,7 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
         for (; j + 3 * 32 < n2; j += 4 * 32) {
             double2 a[4], b[4];
 #pragma unroll
-            for (int u = 0; u < 4; u++) { a[u] = ldg2(rowA + 2 * (j + u * 32)); b[u] = ldg2(rowB + 2 * (j + u * 32)); }
+            for (int u = 0; u < 4; u++) { a[u] = ld2<COH>(rowA + 2 * (j + u * 32)); b[u] = ld2<COH>(rowB + 2 * (j + u * 32)); }
 #pragma unroll
             for (int u = 0; u < 4; u++) {
                 const double2 x = xa[j + u * 32], y = xb[j + u * 32];
@@ -59,7 +99,7 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
             }
         }
         for (; j < n2; j += 32) {
-            const double2 a = ldg2(rowA + 2 * j), b = ldg2(rowB + 2 * j), x = xa[j], y = xb[j];
+            const double2 a = ld2<COH>(rowA + 2 * j), b = ld2<COH>(rowB + 2 * j), x = xa[j], y = xb[j];
             sa += a.x * x.x + a.y * x.y;
             sb += b.x * y.x + b.y * y.y;
         }
@@ -67,7 +107,7 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
         for (; j + 7 * 32 < n2; j += 8 * 32) {
             double2 a[8];
 #pragma unroll
-            for (int u = 0; u < 8; u++) a[u] = ldg2(rowA + 2 * (j + u * 32));
+            for (int u = 0; u < 8; u++) a[u] = ld2<COH>(rowA + 2 * (j + u * 32));
 #pragma unroll
             for (int u = 0; u < 8; u++) {
                 const double2 x = xa[j + u * 32];
@@ -75,7 +115,7 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
             }
         }
         for (; j < n2; j += 32) {
-            const double2 a = ldg2(rowA + 2 * j), x = xa[j];
+            const double2 a = ld2<COH>(rowA + 2 * j), x = xa[j];
             sa += a.x * x.x + a.y * x.y;
         }
     }
@@ -94,13 +134,12 @@ __device__ __forceinline__ void limit_drift(double& gx, double& gy, double& gz, 
     gx *= sc; gy *= sc; gz *= sc;
 }
 
-// p_acc >= 0: finish the move of electron p_acc of this spin (needs its MO rows in V);  p_prop >= 0: propose the
-// move of electron p_prop.  commit == 0 evaluates the decision but changes no state (stage timing only).
-template <int PT>
-__global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
-                                                double tau, double sqrt_tau, int commit) {
-    extern __shared__ __align__(16) double sm[];
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// The body works on walker w with the PT threads tid = 0..PT-1 that `sync` joins, in their shared memory `sm`
+// (StepLayout(nsp, kp, PT / 32).total doubles).  Every branch that leaves it is uniform over those threads.
+template <int PT, bool COH, class Sync>
+__device__ __forceinline__ void step_body(const SysDev& s, const WalkDev& wd, int w, int tid, double* sm, const Sync& sync, int spin, int p_acc,
+                                          int p_prop, long log_off, uint32_t step, double tau, double sqrt_tau, int commit) {
+    const int lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], n2 = nsp >> 1, kp = wd.kp, nep = wd.nep;
     const int e0 = spin == 0 ? 0 : s.ns[0];
     constexpr int PW = PT / 32;
@@ -140,8 +179,8 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
         const double* arow = wd.AinvT[spin] + ((long)w * nsp + p) * nsp;
         double a4[4] = {0, 0, 0, 0};
         for (int j = tid; j < n2; j += PT) {
-            const double2 xj = ldg2(xcol + 2 * j);
-            const double2 v0 = ldg2(v + 2 * j), v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j);
+            const double2 xj = ld2<COH>(xcol + 2 * j);
+            const double2 v0 = ld2<COH>(v + 2 * j), v1 = ld2<COH>(v + wd.ldv + 2 * j), v2 = ld2<COH>(v + 2 * wd.ldv + 2 * j), v3 = ld2<COH>(v + 3 * wd.ldv + 2 * j);
             reinterpret_cast<double2*>(vs)[j] = v0;
             reinterpret_cast<double2*>(as)[j] = ldg2(arow + 2 * j);
             a4[0] += v0.x * xj.x + v0.y * xj.y;
@@ -149,7 +188,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             a4[2] += v2.x * xj.x + v2.y * xj.y;
             a4[3] += v3.x * xj.x + v3.y * xj.y;
         }
-        block_sum<PT, 4>(a4, red);
+        group_sum<PT, 4>(a4, red, tid, sync);
         rho = a4[0];
         if (tid == 0) {
             const double rx = Rw[e], ry = Rw[nep + e], rz = Rw[2 * nep + e];
@@ -193,7 +232,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             bc[0] = (accept && commit) ? 1.0 : 0.0;
         }
     }
-    __syncthreads();  // xs, vs, as, bc[0] and the new position are visible to the block
+    sync();  // xs, vs, as, bc[0] and the new position are visible to the block
     if (p_acc >= 0) accepted = bc[0] != 0.0;
     if (!accepted && p_prop < 0) return;
 
@@ -201,7 +240,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
     if (accepted) {
         double* orb = wd.Orb[spin] + ((long)w * nsp + p_acc) * 5 * nsp;
         for (int j = tid; j < n2; j += PT) {  // row caches and the new window rows: fire-and-forget stores
-            const double2 v1 = ldg2(v + wd.ldv + 2 * j), v2 = ldg2(v + 2 * wd.ldv + 2 * j), v3 = ldg2(v + 3 * wd.ldv + 2 * j), v4 = ldg2(v + 4 * wd.ldv + 2 * j);
+            const double2 v1 = ld2<COH>(v + wd.ldv + 2 * j), v2 = ld2<COH>(v + 2 * wd.ldv + 2 * j), v3 = ld2<COH>(v + 3 * wd.ldv + 2 * j), v4 = ld2<COH>(v + 4 * wd.ldv + 2 * j);
             const double2 v0 = reinterpret_cast<double2*>(vs)[j];
             reinterpret_cast<double2*>(orb)[j] = v0;
             reinterpret_cast<double2*>(orb + nsp)[j] = v1;
@@ -216,13 +255,13 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
     for (int l = warp; l < m_old; l += PW) {
         double ra = 0.0, rb = 0.0;
         if (accepted && p_prop >= 0) {
-            warp_dot2(Wb + (long)l * nsp, vs, Vb + (long)l * nsp, xs, n2, lane, ra, rb);
+            warp_dot2<COH>(Wb + (long)l * nsp, vs, Vb + (long)l * nsp, xs, n2, lane, ra, rb);
             if (lane == 0) { rs[l] = ra; bs[l] = rb; }
         } else if (accepted) {
-            warp_dot2(Wb + (long)l * nsp, vs, nullptr, vs, n2, lane, ra, rb);
+            warp_dot2<COH>(Wb + (long)l * nsp, vs, nullptr, vs, n2, lane, ra, rb);
             if (lane == 0) rs[l] = ra;
         } else {
-            warp_dot2(Vb + (long)l * nsp, xs, nullptr, xs, n2, lane, ra, rb);
+            warp_dot2<COH>(Vb + (long)l * nsp, xs, nullptr, xs, n2, lane, ra, rb);
             if (lane == 0) bs[l] = ra;
         }
     }
@@ -235,7 +274,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
         acc = warp_sum(acc);
         if (lane == 0) bs[m_old] = acc;
     }
-    __syncthreads();
+    sync();
     if (accepted) {
         // bordered update of S^-1:  t_l = sum_n r_n SinvT[l][n] (one warp per row l)
         const int m = m_old;
@@ -245,7 +284,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             acc = warp_sum(acc);
             if (lane == 0) ts[l] = acc;
         }
-        __syncthreads();
+        sync();
         const double sinv = 1.0 / rho;
         for (int idx = tid; idx < m * m; idx += PT) {
             const int l = idx / m, n = idx - l * m;
@@ -260,7 +299,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             wd.plist[(long)w * kp + m] = p_acc;
             wd.mcount[w] = m + 1;
         }
-        __syncthreads();  // S^-1 is read again below
+        sync();  // S^-1 is read again below
     }
     if (p_prop < 0) return;
 
@@ -277,13 +316,13 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
                 for (int l = q; l < m; l += CP) acc += Si[l * kp + n] * bs[l];
             c4[q * 128 + n] = acc;
         }
-        __syncthreads();
+        sync();
         for (int n = tid; n < m; n += PT) {
             const double c = CP == 4 ? (c4[n] + c4[128 + n]) + (c4[256 + n] + c4[384 + n]) : (CP == 2 ? c4[n] + c4[128 + n] : c4[n]);
             cs[n] = c;
             wd.cvec[(long)w * kp + n] = c;
         }
-        __syncthreads();
+        sync();
         // x = a_p - Wbuf^T c  (effective column of the delayed inverse)
         for (int j = tid; j < n2; j += PT) {
             double2 acc = reinterpret_cast<double2*>(xs)[j];
@@ -291,12 +330,12 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             for (; l + 4 <= m_old; l += 4) {
                 double2 wv[4];
 #pragma unroll
-                for (int u = 0; u < 4; u++) wv[u] = ldg2(Wb + (long)(l + u) * nsp + 2 * j);
+                for (int u = 0; u < 4; u++) wv[u] = ld2<COH>(Wb + (long)(l + u) * nsp + 2 * j);
 #pragma unroll
                 for (int u = 0; u < 4; u++) { acc.x -= cs[l + u] * wv[u].x; acc.y -= cs[l + u] * wv[u].y; }
             }
             for (; l < m_old; l++) {
-                const double2 wv = ldg2(Wb + (long)l * nsp + 2 * j);
+                const double2 wv = ld2<COH>(Wb + (long)l * nsp + 2 * j);
                 acc.x -= cs[l] * wv.x; acc.y -= cs[l] * wv.y;
             }
             if (accepted) {
@@ -333,7 +372,7 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             acc6[5] += wgt * dz;
         }
     }
-    block_sum<PT, 6>(acc6, red);
+    group_sum<PT, 6>(acc6, red, tid, sync);
     double Gx = acc6[0] + acc6[3], Gy = acc6[1] + acc6[4], Gz = acc6[2] + acc6[5];
     limit_drift(Gx, Gy, Gz, wd.lim_a, tau);
     const double qx = rx + tau * Gx + sqrt_tau * bc[4];
@@ -365,11 +404,20 @@ __global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, in
             acc4[3] += wgt * ez;
         }
     }
-    block_sum<PT, 4>(acc4, red);
+    group_sum<PT, 4>(acc4, red, tid, sync);
     if (tid == 0) {
         wd.dJ[w] = acc4[0];
         wd.gJn[3 * w] = acc4[1]; wd.gJn[3 * w + 1] = acc4[2]; wd.gJn[3 * w + 2] = acc4[3];
     }
+}
+
+// p_acc >= 0: finish the move of electron p_acc of this spin (needs its MO rows in V);  p_prop >= 0: propose the
+// move of electron p_prop.  commit == 0 evaluates the decision but changes no state (stage timing only).
+template <int PT>
+__global__ void __launch_bounds__(PT, 1024 / PT) k_step(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
+                                                double tau, double sqrt_tau, int commit) {
+    extern __shared__ __align__(16) double sm[];
+    step_body<PT, false>(s, wd, blockIdx.x, threadIdx.x, sm, CtaSync{}, spin, p_acc, p_prop, log_off, step, tau, sqrt_tau, commit);
 }
 
 }  // namespace qmc

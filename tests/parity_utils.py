@@ -29,7 +29,10 @@ def rel_frob(a, b):
 FLOOR_FACTOR = 8       # GPU may be this many times further from the double oracle than that is from long double
 RESYNC_EVERY = 10      # sweeps of free running between re-seeds of the oracle
 
-_cpu_slots = threading.BoundedSemaphore(oracle.default_threads())   # oracle computations in flight, whoever asks
+# oracle computations in flight: one pool for the followers a test is waiting for, one for the background followers of the
+# large configs (minutes per call, niced) -- which must not keep the foreground ones waiting for a slot
+_fg_slots = threading.BoundedSemaphore(oracle.default_threads())
+_bg_slots = threading.BoundedSemaphore(oracle.default_threads())
 
 
 def cond2(ainv):
@@ -53,8 +56,10 @@ class OracleFollower:
         self.first_step, self.tau, self.n_sweeps, self.want_cond, self.e_end = int(first_step), float(tau), int(n_sweeps), want_cond, e_end
         self.ld_inverse, self.keep_ainv_at, self.carried_vs_fresh = ld_inverse, set(keep_ainv_at), carried_vs_fresh
         self.background = background   # started long before it is needed: yields the cores to whatever test is running now
+        self.slots = _bg_slots if background else _fg_slots
         self.cv = threading.Condition()
         self.snaps, self.epoch, self.pending, self._creation, self.error, self.walker = [], 0, None, None, None, None
+        self.horizon = self.n_sweeps   # sweeps the worker may compute ahead of the comparison (set_horizon)
         self.thread = threading.Thread(target=self._run, daemon=True)
         self.thread.start()
 
@@ -70,7 +75,7 @@ class OracleFollower:
                     os.setpriority(os.PRIO_PROCESS, threading.get_native_id(), 10)   # Linux: per-thread nice value
                 except (OSError, AttributeError):
                     pass
-            with _cpu_slots:
+            with self.slots:
                 w = self.osys.walker(self.pos0)
                 if self.want_cond:
                     cond = [cond2(w.Ainv(sp)) if self.osys.ns(sp) else 1.0 for sp in (0, 1)]
@@ -91,12 +96,12 @@ class OracleFollower:
                     while True:
                         if self.n_sweeps < 0:               # closed
                             return
-                        if self.pending is not None or len(self.snaps) < self.n_sweeps:
+                        if self.pending is not None or len(self.snaps) < min(self.n_sweeps, self.horizon):
                             break
                         self.cv.wait()                      # done; a late reseed wakes us up again
                     pend, self.pending = self.pending, None
                     t, ep = len(self.snaps), self.epoch
-                with _cpu_slots:
+                with self.slots:
                     if pend is not None:
                         w.set_positions(pend)
                         if self.ld_inverse:
@@ -159,6 +164,12 @@ class OracleFollower:
         assert t < self.n_sweeps
         self._wait(lambda: len(self.snaps) > t and self.pending is None)
         return self.snaps[t]
+
+    def set_horizon(self, h):
+        """do not compute beyond sweep h - 1 yet (what follows a re-seed would be thrown away)"""
+        with self.cv:
+            self.horizon = h
+            self.cv.notify_all()
 
     def reseed(self, t, pos):
         with self.cv:
@@ -286,6 +297,9 @@ def run_and_compare(wl, walker_ids, n_sweeps, delay_k, first_step=0, flags=qb.QM
     pos_of = (lambda ids: None) if start_pos is None else (lambda ids: [start_pos[w - lo] for w in ids])
     ow = farm.request(wl, walker_ids, n_sweeps, first_step, want_cond=want_cond, e_end=e_end, keep_ainv_at=ainv_at,
                       carried_vs_fresh=carried_vs_fresh, positions=pos_of(walker_ids))
+    if resync_every:
+        for f in ow:
+            f.set_horizon(resync_every)
     floor_mode = "ld" if floor is True else floor
     floor_ids = ([int(w) for w in floor_ids] if floor_ids is not None else walker_ids) if floor else []
     floor_sweeps = float_sweeps if floor_sweeps is None else min(floor_sweeps, n_sweeps)
@@ -383,6 +397,7 @@ def run_and_compare(wl, walker_ids, n_sweeps, delay_k, first_step=0, flags=qb.QM
                   ("" if asserted else "   (free-running beyond the asserted window)"), flush=True)
         if resync_every and (t + 1) % resync_every == 0 and t + 1 < n_sweeps:
             for n, w in enumerate(walker_ids):
+                ow[n].set_horizon(t + 1 + resync_every)
                 ow[n].reseed(t, gpos[w - lo])
                 if w in owl and t + 1 < floor_sweeps:
                     owl[w].reseed(t, gpos[w - lo])
