@@ -72,6 +72,12 @@ extern "C" {
                              one run in the shadow of the other's contraction; results differ from the one-lane run only by
                              the rounding of the stream-K partition (it depends on the row count). */
 
+#define QMC_PER_ELECTRON 16u /* never use the window kernel of the mid-size path: systems with 33..256 electrons per spin whose
+                               basis fits (5 x 4 rows of N_b functions in shared memory) otherwise run all electron steps of a
+                               delay window in ONE launch -- four walkers per CTA, basis functions and MO rows never leaving
+                               the SM -- followed by the flush.  Same arithmetic; the contraction sums in another order
+                               (rounding). */
+
 typedef struct qmc_system qmc_system;   /* immutable after qmc_init: atoms, basis, MO coefficients, Jastrow (device) */
 typedef struct qmc_walkers qmc_walkers; /* mutable crowd state */
 
@@ -258,9 +264,10 @@ int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, d
  * the first proposal and the last accept of a delay window), flush and local-energy evaluation, with CUDA
  * events on the walker set's stream.  qmc_get_stage_times synchronises and returns accumulated milliseconds
  * and launch counts per stage id (a "launch" of stage 4 is the whole flush = 4 kernels, of stage 5 two
- * kernels).  stride = 0 turns it off and clears the totals. */
+ * kernels; stage 6 = one window kernel of the mid-size path, QMC_PER_ELECTRON).  stride = 0 turns it off and clears
+ * the totals. */
 int qmc_set_profiling(qmc_walkers* w, int stride);
-int qmc_get_stage_times(qmc_walkers* w, double* ms /* [6] */, uint64_t* counts /* [6] */);
+int qmc_get_stage_times(qmc_walkers* w, double* ms /* [7] */, uint64_t* counts /* [7] */);
 /* Lanes of a walker set (see QMC_ONE_LANE): *n_lanes = 1 or 2; walkers_per_lane[2] (may be NULL) = their sizes. */
 int qmc_get_lanes(const qmc_walkers* w, int* n_lanes, int* walkers_per_lane);
 /* Span on the GPU of the contraction launches that the in-situ profiling sampled (qmc_set_profiling stride > 0): every CTA

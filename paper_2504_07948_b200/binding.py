@@ -19,7 +19,8 @@ QMC_LOG_RATIOS = 1
 QMC_LARGE_PATH = 2
 QMC_SCREEN_MO = 4
 QMC_ONE_LANE = 8
-STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc")
+QMC_PER_ELECTRON = 16
+STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc", "window")
 
 EXPORTED = [
     "qmc_init", "qmc_finalize", "qmc_walkers_create", "qmc_walkers_destroy", "qmc_sweep", "qmc_get_positions",
@@ -502,10 +503,10 @@ def qmc_set_profiling(walkers: Walkers, stride):
 
 
 def qmc_get_stage_times(walkers: Walkers):
-    ms = (C.c_double * 6)()
-    n = (C.c_uint64 * 6)()
+    ms = (C.c_double * 7)()
+    n = (C.c_uint64 * 7)()
     _check(load_library().qmc_get_stage_times(walkers.handle, ms, n))
-    return {STAGES[i]: (ms[i], n[i]) for i in range(6)}
+    return {STAGES[i]: (ms[i], n[i]) for i in range(7)}
 
 
 def qmc_measure_fp64_peak(ms_target=200.0, stream=None) -> float:

@@ -691,7 +691,8 @@ static void prof_collect(qmc_walkers* w) {
 }
 
 /* stage ids: 0 step kernel with one half (first proposal / last accept of a delay window), 1 basis, 2 MO contraction,
-   3 fused step kernel (accept of p + proposal of p + 1), 4 flush, 5 local energy */
+   3 fused step kernel (accept of p + proposal of p + 1), 4 flush, 5 local energy, 6 window kernel (mid-size path: all
+   electron steps of one delay window in one launch) */
 extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
     if (!w || stride < 0) return fail(QMC_ERR_ARG, "qmc_set_profiling");
     GUARD(w->sys);
@@ -703,11 +704,11 @@ extern "C" int qmc_set_profiling(qmc_walkers* w, int stride) {
     if (stride > 0) CU(w->mo_trace.reserve(MO_TRACE_SLOTS * 2 * (size_t)w->sys->n_sm * 8, w->stream));
     return QMC_OK;
 }
-extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[6]*/, uint64_t* counts /*[6]*/) {
+extern "C" int qmc_get_stage_times(qmc_walkers* w, double* ms /*[7]*/, uint64_t* counts /*[7]*/) {
     if (!w || !ms || !counts) return fail(QMC_ERR_ARG, "qmc_get_stage_times");
     GUARD(w->sys);
     prof_collect(w);
-    for (int i = 0; i < 6; i++) { ms[i] = w->stage_ms[i]; counts[i] = w->stage_n[i]; }
+    for (int i = 0; i < 7; i++) { ms[i] = w->stage_ms[i]; counts[i] = w->stage_n[i]; }
     return QMC_OK;
 }
 
@@ -833,6 +834,32 @@ static int sweep_finish_step(qmc_walkers* w, const SweepCall& c) {
     return QMC_OK;
 }
 
+// the mid-size path: one launch per delay window (window_kernel.cuh) + the flush; the whole call of one set
+static int sweep_windows(qmc_walkers* w, const SweepCall& c) {
+    const SysDev& s = w->sys->d;
+    build_lane_views(w);
+    Lane& L = w->lane[0];
+    cudaStream_t st = L.stream;
+    const bool pf = w->prof_stride > 0;
+    if (c.dmc) CU(launch_dmc_begin(L.d, st));
+    for (int t = 0; t < c.nsteps; t++) {
+        const long log_base = (long)(c.log_t0 + t) * s.ne * w->d.W;
+        for (int sp = 0; sp < 2; sp++)
+            for (int p0 = 0; p0 < s.ns[sp]; p0 += c.delay_k) {
+                const int n = s.ns[sp] - p0 < c.delay_k ? s.ns[sp] - p0 : c.delay_k;
+                prof_begin(w, st, 6, pf);
+                CU(launch_window(s, L.d, sp, p0, n, log_base, w->d.W, w->step, c.tau, st));
+                prof_end(w, st, pf);
+                prof_begin(w, st, 4, pf);
+                CU(launch_flush(s, L.d, sp, st));
+                prof_end(w, st, pf);
+            }
+        int rc = sweep_finish_step(w, c);
+        if (rc) return rc;
+    }
+    return QMC_OK;
+}
+
 // n_sets walker sets of ONE system advance together: the host enqueues electron p of every lane of every set (each on its
 // own stream) before electron p + 1 of any, so that the HBM-bound stages of one lane overlap the contraction of another
 static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
@@ -844,7 +871,9 @@ static int sweep_sets(qmc_walkers* const* sets, int n_sets, SweepCall c) {
         if (rc) return rc;
         if (i == 0) c.log_T = ci.log_T;
         if (small) { rc = sweep_small(sets[i], ci); if (rc) return rc; }
-        else large.push_back(sets[i]);
+        else if (!(sets[i]->flags & QMC_PER_ELECTRON) && sets[i]->n_lanes == 1 && window_path_ok(sets[i]->sys->d, sets[i]->d, sets[i]->d.kp)) {
+            if (ci.nsteps > 0) { rc = sweep_windows(sets[i], ci); if (rc) return rc; }
+        } else large.push_back(sets[i]);
     }
     if (large.empty() || c.nsteps == 0) return QMC_OK;
     const SysDev& s = large[0]->sys->d;

@@ -236,6 +236,29 @@ cudaError_t launch_basis_values(const SysDev& s, const double* pts, int n_points
     return cudaGetLastError();
 }
 
+}  // namespace qmc
+#include "window_kernel.cuh"   // the mid-size path: needs exp_neg3 above
+namespace qmc {
+
+// one delay window of one spin in one launch (window_kernel.cuh); false: the system does not fit that path
+bool window_path_ok(const SysDev& s, const WalkDev& wd, int kp) {
+    const int nspm = s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1];
+    if (nspm > 256) return false;
+    return window_smem_bytes(nspm, kp, s.nbp) <= 227 * 1024;
+}
+cudaError_t launch_window(const SysDev& s, const WalkDev& wd, int spin, int p_first, int n_steps, long log_base, int W_total, uint32_t step,
+                          double tau, cudaStream_t st) {
+    static SmemAttr attr;
+    const size_t smem = window_smem_bytes(s.nsp[spin], wd.kp, s.nbp);
+    cudaError_t e = attr.ensure(k_window, smem);
+    if (e != cudaSuccess) return e;
+    WinArgs a;
+    a.spin = spin; a.p_first = p_first; a.n_steps = n_steps; a.log_base = log_base; a.W_total = W_total; a.step = step; a.tau = tau; a.sqrt_tau = sqrt(tau);
+    k_window<<<(wd.W + WIN_G - 1) / WIN_G, WIN_THREADS, smem, st>>>(s, wd, a);
+    COUNT_LAUNCH();
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------------------------------------
 // a4: MO rows V = Phi * C_s: persistent stream-K FP64 DMMA GEMM (mo_streamk.cuh)       [north_star item 2]
 size_t phiT_bytes(const SysDev& s, int rows) { return (size_t)((rows + MO_BM - 1) / MO_BM) * s.kb * MO_A_STAGE * sizeof(double); }

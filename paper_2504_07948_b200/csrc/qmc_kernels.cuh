@@ -42,6 +42,10 @@ cudaError_t launch_dmc_weight(const WalkDev& wd, double tau, double e_trial, con
 cudaError_t launch_branch(const SysDev& s, const WalkDev& wd, int* ibuf, double* e_mixed, uint32_t step, double* e_trial_dev, double feedback,
                           double* branch_log, cudaStream_t st);
 bool small_path_ok(const SysDev& s, const WalkDev& wd);
+// the mid-size path (window_kernel.cuh): electrons p_first .. p_first + n_steps - 1 of one spin in one launch
+bool window_path_ok(const SysDev& s, const WalkDev& wd, int kp);
+cudaError_t launch_window(const SysDev& s, const WalkDev& wd, int spin, int p_first, int n_steps, long log_base, int W_total, uint32_t step,
+                          double tau, cudaStream_t st);
 cudaError_t launch_sweep_small(const SysDev& s, const WalkDev& wd, int nsteps, uint32_t step0, double tau, int dmc, double e_trial,
                                const double* e_trial_dev, cudaStream_t st);
 cudaError_t launch_plain_C(const double* in, int nb, int ns, double* Cp, int nsp, const int* fmap, cudaStream_t st);

@@ -29,7 +29,7 @@ struct StepLayout {
     int xs, vs, as, c4, bs, cs, rs, ts, red, bc, total;
     __host__ __device__ StepLayout(int nsp, int kp, int PW /* warps per CTA */) {
         xs = 0; vs = xs + nsp; as = vs + nsp; c4 = as + nsp;
-        bs = c4 + 512;
+        bs = c4 + 32 * PW;   // c4: PT / 128 partial sums for each of 128 window rows
         cs = bs + kp + 1; rs = cs + kp + 1; ts = rs + kp + 1;
         red = ts + kp + 1; bc = red + 8 * PW; total = bc + 16;
     }
