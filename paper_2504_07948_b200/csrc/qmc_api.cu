@@ -320,6 +320,27 @@ extern "C" int qmc_init(qmc_system** out, const qmc_atoms* atoms, const qmc_basi
         CUS(cudaStreamSynchronize(st));
         d.kb_counts = dcn;
         d.kb_list = dli;
+        {   // occupied slots for the window kernel: first the k-blocks of the lower half of K, each half ordered by l
+            std::vector<int> items;
+            const int kbh = (d.kb + 1) / 2;
+            for (int half = 0; half < 2; half++) {
+                for (int l = 0; l < 3; l++)
+                    for (int kb = half ? kbh : 0; kb < (half ? d.kb : kbh); kb++) {
+                        const int c[3] = {cnts[kb].x, cnts[kb].y, cnts[kb].z};
+                        int first = 0;
+                        for (int q = 0; q < l; q++) first += c[q];
+                        for (int q = 0; q < c[l]; q++) items.push_back(kb * 32 + first + q);
+                    }
+                if (half == 0) d.n_win_first = (int)items.size();
+            }
+            d.n_win_items = (int)items.size();
+            if (items.empty()) items.push_back(0);
+            int* dwi;
+            CUS(S->pool.alloc((void**)&dwi, items.size() * sizeof(int), st));
+            CUS(cudaMemcpyAsync(dwi, items.data(), items.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+            CUS(cudaStreamSynchronize(st));
+            d.win_items = dwi;
+        }
         int* dfm;
         CUS(S->pool.alloc((void**)&dfm, fmap.size() * sizeof(int), st));
         CUS(cudaMemcpyAsync(dfm, fmap.data(), fmap.size() * sizeof(int), cudaMemcpyHostToDevice, st));

@@ -42,6 +42,8 @@ struct SysDev {
     const ShellRec* shells;
     const int4* kb_counts;  // [kb]: number of s, p, d shells owning a function of k-block kb (32 functions), list offset
     const KbShell* kb_list; // shells of every k-block, grouped s | p | d (a shell may be in two blocks)
+    const int* win_items;   // window kernel: the occupied slots (kb * 32 + slot) of kb_list, those of the k-blocks below kb/2
+    int n_win_items, n_win_first;  //   first (n_win_first of them), each half ordered s | p | d
     const int* fmap;        // [n_basis] caller's function index -> internal one (shells grouped by reach, Morton-ordered)
     const double* Cplain[2];   // [nbp][nsp] MO coefficients, internal function order, plain row-major (row f2: C A^-1)
     const int* atom_shell_off; // [n_atoms + 1] shells of every atom in atom_shell_list

@@ -244,6 +244,12 @@ namespace qmc {
 bool window_path_ok(const SysDev& s, const WalkDev& wd, int kp) {
     const int nspm = s.nsp[0] > s.nsp[1] ? s.nsp[0] : s.nsp[1];
     if (nspm > 256) return false;
+    // A CTA holds 4 walkers and an SM one CTA: beyond two waves of CTAs the per-electron kernels have rows enough to run
+    // efficiently and win (measured: 152 electrons x 4320 walkers 36.5 ms per sweep per electron against 41.5 ms here;
+    // configs[1], 512 walkers: 17 ms against 12.3 ms).
+    int dev = 0, n_sm = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (wd.W > 2 * WIN_G * n_sm) return false;
     return window_smem_bytes(nspm, kp, s.nbp) <= 227 * 1024;
 }
 cudaError_t launch_window(const SysDev& s, const WalkDev& wd, int spin, int p_first, int n_steps, long log_base, int W_total, uint32_t step,

@@ -123,6 +123,35 @@ __device__ __forceinline__ void warp_dot2(const double* __restrict__ rowA, const
     accB = warp_sum(sb);
 }
 
+// Short rows (n2 <= 128 double2: at most 256 orbitals per spin): a warp takes R window rows at once -- rows l, l + dl,
+// ... -- so that R x 2 loads are in flight per lane instead of two; one row at a time is one memory latency per row.
+template <bool COH, int R>
+__device__ __forceinline__ void warp_dot2_rows(const double* __restrict__ rowA, const double* vecA, const double* __restrict__ rowB, const double* vecB,
+                                               long row_stride, int n_rows, int n2, int lane, double (&accA)[R], double (&accB)[R]) {
+    const double2* xa = reinterpret_cast<const double2*>(vecA);
+    const double2* xb = reinterpret_cast<const double2*>(vecB);
+    double sa[R], sb[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) sa[r] = sb[r] = 0.0;
+    for (int j = lane; j < n2; j += 32) {
+        double2 a[R], b[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const long o = (r < n_rows ? r : 0) * row_stride + 2 * j;
+            a[r] = rowA ? ld2<COH>(rowA + o) : make_double2(0.0, 0.0);
+            b[r] = rowB ? ld2<COH>(rowB + o) : make_double2(0.0, 0.0);
+        }
+        const double2 x = xa[j], y = xb[j];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            sa[r] += a[r].x * x.x + a[r].y * x.y;
+            sb[r] += b[r].x * y.x + b[r].y * y.y;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) { accA[r] = warp_sum(sa[r]); accB[r] = warp_sum(sb[r]); }
+}
+
 // Drift limiter of the DMC generation (row f1, reading A28; Umrigar-Nightingale-Runge 1993 eq. 35 with one constant a):
 // vbar = v (-1 + sqrt(1 + 2 a v^2 tau)) / (a v^2 tau), evaluated as v * 2 / (1 + sqrt(1 + 2x)), x = a v^2 tau (the same
 // number without the cancellation at small x).  a <= 0: off (reading A6).
@@ -252,6 +281,21 @@ __device__ __forceinline__ void step_body(const SysDev& s, const WalkDev& wd, in
         }
         for (int n = tid; n < m_old; n += PT) cs[n] = wd.cvec[(long)w * kp + n];
     }
+    if constexpr (PT == 128) {   // short rows (PT = 128 <=> at most 256 orbitals): four rows per warp at a time (same sums, term by term, as the loop below)
+        constexpr int R = 4;
+        for (int l = warp; l < m_old; l += R * PW) {
+            const int nr = (m_old - l + PW - 1) / PW < R ? (m_old - l + PW - 1) / PW : R;
+            double ra[R], rb[R];
+            const double* rowW = accepted ? Wb + (long)l * nsp : nullptr;
+            const double* rowV = p_prop >= 0 ? Vb + (long)l * nsp : nullptr;
+            warp_dot2_rows<COH, R>(rowW, vs, rowV, xs, (long)PW * nsp, nr, n2, lane, ra, rb);
+            if (lane == 0)
+                for (int r = 0; r < nr; r++) {
+                    if (accepted) rs[l + r * PW] = ra[r];
+                    if (p_prop >= 0) bs[l + r * PW] = rb[r];
+                }
+        }
+    } else
     for (int l = warp; l < m_old; l += PW) {
         double ra = 0.0, rb = 0.0;
         if (accepted && p_prop >= 0) {
@@ -327,6 +371,14 @@ __device__ __forceinline__ void step_body(const SysDev& s, const WalkDev& wd, in
         for (int j = tid; j < n2; j += PT) {
             double2 acc = reinterpret_cast<double2*>(xs)[j];
             int l = 0;
+            if constexpr (PT == 128)
+            for (; l + 8 <= m_old; l += 8) {
+                double2 wv[8];
+#pragma unroll
+                for (int u = 0; u < 8; u++) wv[u] = ld2<COH>(Wb + (long)(l + u) * nsp + 2 * j);
+#pragma unroll
+                for (int u = 0; u < 8; u++) { acc.x -= cs[l + u] * wv[u].x; acc.y -= cs[l + u] * wv[u].y; }
+            }
             for (; l + 4 <= m_old; l += 4) {
                 double2 wv[4];
 #pragma unroll

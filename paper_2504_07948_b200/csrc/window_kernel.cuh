@@ -23,7 +23,8 @@ constexpr int WIN_G = 4;                 // walkers per CTA
 constexpr int WIN_GT = 128;              // threads per walker group
 constexpr int WIN_THREADS = WIN_G * WIN_GT;
 constexpr int WIN_MMA_WARPS = 8;         // warps 0..7 contract; warp 8 lane 0 streams the coefficient stages
-constexpr int WIN_STAGES = 2;
+constexpr int WIN_STAGES = 4;             // ring of HALF coefficient blocks (16 of the 32 k-rows of a CT block, 16.9 KB each)
+constexpr int WIN_HALF = MO_B_STAGE / 2;  // doubles per ring slot
 constexpr int WIN_MT = (5 * WIN_G + 7) / 8;   // 8-row DMMA tiles over the 5 G rows
 
 struct WinLayout {
@@ -35,8 +36,8 @@ struct WinLayout {
         phi = step + WIN_G * per_group;
         cst = phi + 5 * WIN_G * phi_ld;
         cst = (cst + 15) & ~15;                 // 128-byte alignment of the TMA destination
-        bars = cst + WIN_STAGES * MO_B_STAGE;
-        total = bars + 2 * WIN_STAGES + 2;
+        bars = cst + WIN_STAGES * WIN_HALF;
+        total = bars + 2 * WIN_STAGES + 2;   // full[], empty[], phi_hi
     }
 };
 inline size_t window_smem_bytes(int nsp, int kp, int nbp) { return (size_t)WinLayout(nsp, kp, nbp).total * sizeof(double); }
@@ -98,6 +99,8 @@ __global__ void __launch_bounds__(WIN_THREADS, 1) k_window(SysDev s, WalkDev wd,
     double* cst = wsm + L.cst;
     uint64_t* full = reinterpret_cast<uint64_t*>(wsm + L.bars);
     uint64_t* empty = full + WIN_STAGES;
+    uint64_t* phi_hi = empty + WIN_STAGES;
+    const int kbh = (KB + 1) / 2;
     const int w0 = blockIdx.x * WIN_G;
     const int w = w0 + grp;
     const bool live = w < wd.W;
@@ -108,6 +111,7 @@ __global__ void __launch_bounds__(WIN_THREADS, 1) k_window(SysDev s, WalkDev wd,
 
     if (tid == 0) {
         for (int st = 0; st < WIN_STAGES; st++) { mbar_init(&full[st], 1); mbar_init(&empty[st], WIN_MMA_WARPS); }
+        mbar_init(phi_hi, WIN_THREADS / 32 - WIN_MMA_WARPS - 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     // padded functions (n_basis .. nbp) are never written: zero the operand once
@@ -125,47 +129,52 @@ __global__ void __launch_bounds__(WIN_THREADS, 1) k_window(SysDev s, WalkDev wd,
         }
         if (p_prop < 0) break;
         __syncthreads();   // the proposals (wd.rp) are written
-        // ---- [B] basis functions at the proposed positions -> phi[row = g*5 + c][function]
-        {
-            const int items = n_live * 32 * KB;   // (k-block, walker, shell slot)
-            for (int it = tid; it < items; it += WIN_THREADS) {
-                const int kb = it / (n_live * 32), rem = it - kb * (n_live * 32), g = rem >> 5, slot = rem & 31;
-                const int4 cnt = __ldg(s.kb_counts + kb);
-                if (slot >= cnt.x + cnt.y + cnt.z) continue;
-                const KbShell* rp = s.kb_list + (size_t)kb * 32 + slot;
+        // ---- [B] basis functions at the proposed positions -> phi[row = g*5 + c][function].  The shells of the lower half of
+        // K by all warps; those of the upper half by warps 9..15 while warps 0..7 already contract the lower half (they
+        // wait at `phi_hi` before they enter the upper half).
+        auto basis_items = [&](int it0, int it1, int t0, int nt) {
+            for (int it = it0 + t0; it < it1; it += nt) {
+                const int idx = it / n_live, g = it - idx * n_live;
+                const int ks = __ldg(s.win_items + idx);
+                const int kb = ks >> 5;
                 KbShell rec;
                 {
-                    const double2* src = reinterpret_cast<const double2*>(rp);
+                    const double2* src = reinterpret_cast<const double2*>(s.kb_list + ks);
                     double2* dst = reinterpret_cast<double2*>(&rec);
 #pragma unroll
                     for (int q = 0; q < 6; q++) dst[q] = __ldg(src + q);
                 }
                 const double* r3 = wd.rp + 3 * (size_t)(w0 + g);
-                const double px = r3[0], py = r3[1], pz = r3[2];
                 const int c0 = rec.f0 - kb * 32;
                 double* base = phi + (size_t)(g * 5) * L.phi_ld + kb * 32;
-                win_eval_shell(s, rec, px, py, pz, [&](int m, const double (&v)[5]) {
+                win_eval_shell(s, rec, r3[0], r3[1], r3[2], [&](int m, const double (&v)[5]) {
                     const int c = c0 + m;
                     if (c < 0 || c >= 32) return;   // the part of a straddling shell that belongs to the neighbour block
 #pragma unroll
                     for (int q = 0; q < 5; q++) base[q * L.phi_ld + c] = v[q];
                 });
             }
-        }
+        };
+        basis_items(0, s.n_win_first * n_live, tid, WIN_THREADS);
         __syncthreads();
         // ---- [C] V = Phi C: warps 0..7 contract (each 16 columns of a 128-column tile), warp 8 lane 0 streams C
         if (warp == WIN_MMA_WARPS) {
             if (lane == 0) {
                 for (int tn = 0; tn < NT; tn++)
-                    for (int kb = 0; kb < KB; kb++, n_load++) {
+                    for (int hb = 0; hb < 2 * KB; hb++, n_load++) {   // half blocks are contiguous in CT: 16 rows of 132
                         const int st = n_load % WIN_STAGES;
                         const uint32_t round = n_load / WIN_STAGES;
                         if (round > 0) mbar_wait(&empty[st], (round - 1) & 1);
-                        mbar_expect_tx(&full[st], MO_B_STAGE * 8);
-                        bulk_g2s(cst + (size_t)st * MO_B_STAGE, s.CT[spin] + ((long)tn * KB + kb) * MO_B_STAGE, MO_B_STAGE * 8, &full[st]);
+                        mbar_expect_tx(&full[st], WIN_HALF * 8);
+                        bulk_g2s(cst + (size_t)st * WIN_HALF, s.CT[spin] + (long)tn * KB * MO_B_STAGE + (long)hb * WIN_HALF, WIN_HALF * 8, &full[st]);
                     }
             }
-        } else if (warp < WIN_MMA_WARPS) {
+        } else if (warp > WIN_MMA_WARPS) {
+            basis_items(s.n_win_first * n_live, s.n_win_items * n_live, tid - (WIN_MMA_WARPS + 1) * 32, WIN_THREADS - (WIN_MMA_WARPS + 1) * 32);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(phi_hi);
+        }
+        if (warp < WIN_MMA_WARPS) {
             const int lr = lane >> 2, lc = lane & 3;
             const int wn0 = warp * 16;
             for (int tn = 0; tn < NT; tn++) {
@@ -174,13 +183,15 @@ __global__ void __launch_bounds__(WIN_THREADS, 1) k_window(SysDev s, WalkDev wd,
                 for (int mi = 0; mi < WIN_MT; mi++)
 #pragma unroll
                     for (int j = 0; j < 2; j++) acc[mi][j][0] = acc[mi][j][1] = 0.0;
-                for (int kb = 0; kb < KB; kb++, n_use++) {
+                for (int hb = 0; hb < 2 * KB; hb++, n_use++) {
+                    if (tn == 0 && hb == 2 * kbh) mbar_wait(phi_hi, i & 1);   // the upper half of the operand is complete
                     const int st = n_use % WIN_STAGES;
                     mbar_wait(&full[st], (n_use / WIN_STAGES) & 1);
-                    const double* Bs = cst + (size_t)st * MO_B_STAGE;
-                    const double* Ap = phi + kb * 32;
+                    const double* Bs = cst + (size_t)st * WIN_HALF;
+                    const double* Ap = phi + hb * 16;
+                    if (tn * MO_BN + wn0 < nsp)   // (a warp whose 16 columns lie beyond the orbitals only keeps the ring going)
 #pragma unroll
-                    for (int kk = 0; kk < MO_BK / 4; kk++) {
+                    for (int kk = 0; kk < MO_BK / 8; kk++) {
                         double af[WIN_MT], bf[2];
 #pragma unroll
                         for (int mi = 0; mi < WIN_MT; mi++) {
