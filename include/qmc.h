@@ -287,6 +287,11 @@ int qmc_philox_words(int n, const uint32_t* ctr_key, uint32_t* out, void* cuda_s
 uint64_t qmc_launch_count(void);
 
 const char* qmc_last_error(void);
+/* Diagnostic: the last non-sticky CUDA error that an entry point found PENDING on the calling thread when it was entered
+ * -- left there by an earlier runtime call of another library that shares the thread -- and dropped, with the entry point's
+ * name; "" if there never was one.  (Without this, the cudaGetLastError() after our next kernel launch would report it as
+ * that launch's failure.) */
+const char* qmc_stale_error(void);
 const char* qmc_version(void);
 
 #ifdef __cplusplus

@@ -29,7 +29,7 @@ EXPORTED = [
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
     "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl", "qmc_set_mo_ctas", "qmc_sweep_crowds",
-    "qmc_release_scratch", "qmc_philox_words", "qmc_get_lanes", "qmc_get_mo_spans",
+    "qmc_release_scratch", "qmc_philox_words", "qmc_get_lanes", "qmc_get_mo_spans", "qmc_stale_error",
 ]
 
 
@@ -108,10 +108,11 @@ def load_library(path: str | None = None):
     lib.qmc_philox_words.argtypes = [i, vp, vp, vp]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
+    lib.qmc_stale_error.restype = C.c_char_p
     lib.qmc_version.restype = C.c_char_p
     for name in EXPORTED:
         fn = getattr(lib, name)
-        if name not in ("qmc_finalize", "qmc_walkers_destroy", "qmc_launch_count", "qmc_last_error", "qmc_version"):
+        if name not in ("qmc_finalize", "qmc_walkers_destroy", "qmc_launch_count", "qmc_last_error", "qmc_version", "qmc_stale_error"):
             fn.restype = i
     if path is None:
         _lib = lib
@@ -521,6 +522,10 @@ def qmc_launch_count() -> int:
 
 def qmc_version() -> str:
     return load_library().qmc_version().decode()
+
+
+def qmc_stale_error() -> str:
+    return load_library().qmc_stale_error().decode()
 
 
 def qmc_last_error() -> str:

@@ -95,7 +95,18 @@ struct DeviceGuard {
     }
     ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
+// A non-sticky CUDA error that some earlier runtime call on this host thread left behind (ours are all checked where they
+// are made; PyTorch and other libraries share the thread) would otherwise be picked up by the cudaGetLastError() that
+// follows our next kernel launch and be reported as that launch's failure.  Entry points drop it and remember what it was
+// (qmc_stale_error), so that it is neither mistaken for ours nor lost.
+static thread_local std::string g_stale;
+static void drop_stale_error(const char* where) {
+    const cudaError_t se = cudaGetLastError();
+    if (se != cudaSuccess) g_stale = std::string(cudaGetErrorString(se)) + " (found pending at " + where + ")";
+}
+extern "C" const char* qmc_stale_error(void) { return g_stale.c_str(); }
 #define GUARD(sysptr)                                                                                    \
+    drop_stale_error(__func__);                                                                          \
     DeviceGuard _guard((sysptr)->device);                                                                \
     if (_guard.err != cudaSuccess) { cudaGetLastError(); return fail(QMC_ERR_CUDA, std::string("cannot select the system's device: ") + cudaGetErrorString(_guard.err)); }
 
