@@ -253,6 +253,22 @@ int qmc_get_mo_work(const qmc_walkers* w, uint64_t* executed, uint64_t* dense);
 int qmc_eval_basis(const qmc_system* sys, int n_points, const double* xyz /* [n][3] */, double* out, void* cuda_stream);
 /* Orbital rows at n_points positions: out[n][5][n_s] (basis kernel + FP64 contraction kernel). */
 int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream);
+/* qmc_eval_basis for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same basis kernel (the AO values, gradients
+ * and Laplacians of one electron position) and the same export kernel, with the pre-tiled A operand -- the kernel's
+ * scratch -- in a fixed array inside the library instead of a per-call allocation.
+ *   xyz  DEVICE pointer, [n_points][3] doubles (the caller's; read only)
+ *   out  DEVICE pointer, [n_points][5][n_basis] doubles (the caller's; value, d/dx, d/dy, d/dz, laplacian)
+ * Both must be device (or managed) memory of the system's device: a host pointer is rejected with QMC_ERR_ARG.
+ * Limit: ceil(5 n_points / 128) * ceil(n_basis / 32) * 36864 bytes <= QMC_NOALLOC_SCRATCH_BYTES (the used part of the
+ * array is cleared on the stream first); beyond it the call returns QMC_ERR_ARG and qmc_last_error() names the largest
+ * n_points this system allows.  The call makes no cudaMalloc / cudaFree and calls no allocating routine; it only
+ * enqueues (memset, two kernels) on `cuda_stream` and does NOT synchronise: `out` is complete when that work is.
+ * Every GPU that loads the library holds the array (8 MiB) until the process exits.  All calls on a device share it and
+ * it keeps the last call's contents: two calls whose work overlaps on the GPU (different streams, no ordering between
+ * them) race; calls on one stream are safe. */
+#define QMC_NOALLOC_SCRATCH_BYTES (8u << 20)
+int qmc_eval_basis_noalloc(const qmc_system* sys, int n_points, const double* xyz, double* out, void* cuda_stream);
 /* Time `reps` launches of one stage of the move on the walker set's current state with CUDA events on its
  * stream (no state is committed).  stage: 0 = step kernel, proposal half only (effective column + drift + RNG +
  * Jastrow), 1 = basis, 2 = MO contraction, 3 = step kernel with both halves (ratio/accept with the decision

@@ -25,7 +25,7 @@ STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc", "window")
 EXPORTED = [
     "qmc_init", "qmc_finalize", "qmc_walkers_create", "qmc_walkers_destroy", "qmc_sweep", "qmc_get_positions",
     "qmc_get_Ainv", "qmc_get_logpsi", "qmc_get_eloc", "qmc_get_accept_log", "qmc_get_ratio_log", "qmc_get_stats",
-    "qmc_synchronize", "qmc_eval_basis", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
+    "qmc_synchronize", "qmc_eval_basis", "qmc_eval_basis_noalloc", "qmc_eval_mo", "qmc_time_stage", "qmc_set_profiling", "qmc_get_stage_times",
     "qmc_measure_fp64_peak", "qmc_launch_count", "qmc_last_error", "qmc_version",
     "qmc_dmc_step", "qmc_get_weights", "qmc_branch", "qmc_get_mo_work", "qmc_get_dlogpsi_dR",
     "qmc_dmc_run", "qmc_get_deloc_dR", "qmc_set_ecp", "qmc_get_vnl", "qmc_set_mo_ctas", "qmc_sweep_crowds",
@@ -86,6 +86,7 @@ def load_library(path: str | None = None):
     lib.qmc_get_stats.argtypes = [vp] + [C.POINTER(u64)] * 4
     lib.qmc_synchronize.argtypes = [vp]
     lib.qmc_eval_basis.argtypes = [vp, i, vp, vp, vp]
+    lib.qmc_eval_basis_noalloc.argtypes = [vp, i, vp, vp, vp]
     lib.qmc_eval_mo.argtypes = [vp, i, i, vp, vp, vp]
     lib.qmc_time_stage.argtypes = [vp, i, i, i, i, C.POINTER(d)]
     lib.qmc_set_profiling.argtypes = [vp, i]
@@ -478,6 +479,20 @@ def qmc_eval_basis(system: System, xyz, out=None, stream=None):
         xyz = np.ascontiguousarray(xyz, np.float64)
     out = _out((n, 5, system.n_basis), torch.float64, out)
     _check(load_library().qmc_eval_basis(system.handle, n, _ptr(xyz), _ptr(out), _stream_ptr(stream)))
+    return out
+
+
+def qmc_eval_basis_noalloc(system: System, xyz, out, stream=None):
+    """qmc_eval_basis without any device allocation (include/qmc.h): `xyz` [n][3] and `out` [n][5][n_basis] are the caller's
+    CUDA float64 tensors; the call only enqueues on the stream and does not synchronise."""
+    import torch
+    for t, name in ((xyz, "xyz"), (out, "out")):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise TypeError(f"qmc_eval_basis_noalloc: {name} must be a contiguous CUDA float64 tensor")
+    n = int(xyz.shape[0])
+    if tuple(xyz.shape) != (n, 3) or tuple(out.shape) != (n, 5, system.n_basis):
+        raise ValueError("qmc_eval_basis_noalloc: xyz must be [n][3] and out [n][5][n_basis]")
+    _check(load_library().qmc_eval_basis_noalloc(system.handle, n, _ptr(xyz), _ptr(out), _stream_ptr(stream)))
     return out
 
 

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -1402,6 +1403,64 @@ extern "C" int qmc_eval_basis(const qmc_system* sys, int n_points, const double*
 }
 extern "C" int qmc_eval_mo(const qmc_system* sys, int spin, int n_points, const double* xyz, double* out, void* cuda_stream) {
     return eval_common(sys, spin, n_points, xyz, out, cuda_stream, true);
+}
+
+// ---- qmc_eval_basis_noalloc: the basis kernel with its scratch (the pre-tiled A operand PhiT) in a fixed array of the
+// library.  In host code `g_noalloc_scratch` is only the host-side stand-in of the symbol, never a device address: the
+// address a kernel may use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+static __device__ __align__(256) double g_noalloc_scratch[QMC_NOALLOC_SCRATCH_BYTES / sizeof(double)];
+static constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::atomic<double*> g_noalloc_ptr[NOALLOC_MAX_DEVICES];
+
+static int noalloc_scratch(int device, double** out) {   // the caller has made `device` current (GUARD)
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return fail(QMC_ERR_ARG, "qmc_eval_basis_noalloc: device ordinal beyond 63");
+    double* p = g_noalloc_ptr[device].load(std::memory_order_acquire);
+    if (!p) {   // two threads racing here look up the same address
+        cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(QMC_ERR_CUDA, std::string("qmc_eval_basis_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        }
+        g_noalloc_ptr[device].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return QMC_OK;
+}
+
+static bool on_device(const void* p, int device) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (a.type == cudaMemoryTypeManaged) return true;
+    return a.type == cudaMemoryTypeDevice && a.device == device;
+}
+
+extern "C" int qmc_eval_basis_noalloc(const qmc_system* sys, int n_points, const double* xyz, double* out, void* cuda_stream) {
+    if (!sys || n_points < 0) return fail(QMC_ERR_ARG, "qmc_eval_basis_noalloc: bad argument");
+    if (n_points == 0) return QMC_OK;
+    if (!xyz || !out) return fail(QMC_ERR_ARG, "qmc_eval_basis_noalloc: null buffer");
+    GUARD(sys);
+    const SysDev& s = sys->d;
+    constexpr int TILE_ROWS = 128;                        // rows of one tile of PhiT (MO_BM)
+    const size_t stage_bytes = phiT_bytes(s, 1);          // one tile: ceil(n_basis / 32) blocks of 128 x 36 doubles
+    const long max_points = (long)(QMC_NOALLOC_SCRATCH_BYTES / stage_bytes) * TILE_ROWS / 5;
+    if (n_points > max_points)
+        return fail(QMC_ERR_ARG, "qmc_eval_basis_noalloc: n_points = " + std::to_string(n_points) + " needs " +
+                                     std::to_string((size_t)((5L * n_points + TILE_ROWS - 1) / TILE_ROWS) * stage_bytes) + " bytes of scratch, the fixed array has " +
+                                     std::to_string(QMC_NOALLOC_SCRATCH_BYTES) + ": at most " + std::to_string(max_points) +
+                                     " points per call for this basis (use qmc_eval_basis, which allocates)");
+    if (!on_device(xyz, sys->device) || !on_device(out, sys->device))
+        return fail(QMC_ERR_ARG, "qmc_eval_basis_noalloc: xyz and out must be device memory of the system's device");
+    double* PhiT = nullptr;
+    int rc = noalloc_scratch(sys->device, &PhiT);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t used = phiT_bytes(s, 5 * n_points);
+    // the kernel writes the real functions of the real rows only; padding must read as zero and the array keeps the last
+    // call's contents
+    CU(cudaMemsetAsync(PhiT, 0, used, st));
+    CU(launch_basis(s, xyz, n_points, PhiT, nullptr, st));
+    CU(launch_export_phi(PhiT, (long)n_points * 5, s.n_basis, s.kb, s.fmap, out, st));
+    return QMC_OK;
 }
 
 extern "C" int qmc_time_stage(qmc_walkers* w, int stage, int spin, int delay_k, int reps, double* ms_per_launch) {
