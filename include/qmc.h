@@ -78,6 +78,10 @@ extern "C" {
                                the SM -- followed by the flush.  Same arithmetic; the contraction sums in another order
                                (rounding). */
 
+#define QMC_STEP_ONEPASS 32u /* use the one-pass step kernel (the delay window read once, as an FP64 DMMA pass against eight
+                               vectors; csrc/step_onepass.cuh) whatever the size.  It is the default of the per-electron
+                               kernels for rows of the inverse longer than 256; the flag forces it for shorter rows (tests). */
+
 typedef struct qmc_system qmc_system;   /* immutable after qmc_init: atoms, basis, MO coefficients, Jastrow (device) */
 typedef struct qmc_walkers qmc_walkers; /* mutable crowd state */
 

@@ -20,6 +20,7 @@ QMC_LARGE_PATH = 2
 QMC_SCREEN_MO = 4
 QMC_ONE_LANE = 8
 QMC_PER_ELECTRON = 16
+QMC_STEP_ONEPASS = 32
 STAGES = ("step_half", "basis", "mo", "step", "flush", "eloc", "window")
 
 EXPORTED = [

@@ -592,6 +592,7 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     CUW(w->pool.alloc((void**)&w->d_comb, (4 * W + 1) * 4, st));
     CUW(w->pool.alloc((void**)&w->d_emixed, 8, st));
     CUW(launch_fill_double(d.weight, n_walkers, 1.0, st));
+    d.onepass = (flags & QMC_STEP_ONEPASS) ? 1 : 0;
     d.screen_theta = (flags & QMC_SCREEN_MO) ? QMC_SCREEN_THETA : -1.0;
     CUW(w->pool.alloc((void**)&d.tilemax, (size_t)d.mt * s.kb * 8, st));
     CUW(w->pool.alloc((void**)&d.plan_cnt, (size_t)d.mt * 4, st));

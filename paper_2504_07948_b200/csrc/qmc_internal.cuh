@@ -64,6 +64,7 @@ struct SysDev {
 
 struct WalkDev {
     int W, ne, nep, ldv, kp;
+    int onepass;   // QMC_STEP_ONEPASS: the one-pass step kernel whatever the row length
     int lean;   // this set of walkers is one LANE of a crowd (its kernels share the SMs with the other lane's contraction)
     double* R;
     double* AinvT[2];

@@ -10,6 +10,7 @@
 #include "mo_streamk.cuh"
 #include "device_utils.cuh"
 #include "step_kernel.cuh"
+#include "step_onepass.cuh"
 #include "block_inverse.cuh"
 #include "dmc_kernels.cuh"
 #include "small_sweep.cuh"
@@ -334,7 +335,15 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 // a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st) {
-    static SmemAttr attr[3];
+    static SmemAttr attr[3], attr1;
+    if (step1_fits(s.nsp[spin], wd.kp, wd.onepass != 0)) {   // large systems: the delay window read once (step_onepass.cuh)
+        const size_t smem1 = step1_smem_bytes(s.nsp[spin], wd.kp);
+        const cudaError_t e1 = attr1.ensure(k_step1p, smem1);
+        if (e1 != cudaSuccess) return e1;
+        k_step1p<<<wd.W, S1_PT, smem1, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+        COUNT_LAUNCH();
+        return cudaGetLastError();
+    }
     const int pt = step_threads(s.nsp[spin], wd.lean != 0);
     const size_t smem = step_smem_bytes(s.nsp[spin], wd.kp, wd.lean != 0);
     const cudaError_t er = pt == 512 ? attr[2].ensure(k_step<512>, smem) : (pt == 256 ? attr[1].ensure(k_step<256>, smem) : attr[0].ensure(k_step<128>, smem));
@@ -1148,3 +1157,10 @@ cudaError_t launch_philox_words(int n, const uint32_t* in, uint32_t* out, cudaSt
 uint64_t launch_count() { return g_launches; }
 
 }  // namespace qmc
+
+#ifdef QMC_STEP_TRACE
+extern "C" int qmc_debug_step_trace(unsigned long long* out, int n) {
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(out, qmc::g_step_trace, (size_t)n * 8);
+}
+#endif

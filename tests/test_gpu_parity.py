@@ -157,6 +157,13 @@ def test_config0_full_trajectories():
 
 
 @pytest.mark.parametrize("k", [1, 4, 5])
+def test_config0_onepass_step_kernel(k):
+    # ... and through the one-pass step kernel of the large systems (rows of 16 doubles: one DMMA step per row group)
+    wl = qi.make_workload(0)
+    _assert_report(run_and_compare(wl, range(16), 20, k, flags=qb.QMC_LOG_RATIOS | qb.QMC_LARGE_PATH | qb.QMC_STEP_ONEPASS))
+
+
+@pytest.mark.parametrize("k", [1, 4, 5])
 def test_config0_large_system_path(k):
     # config 0 qualifies for the one-launch small-system path (row f4), which the test above exercises; here the same
     # system is forced through the per-electron kernels and the delayed update (QMC_LARGE_PATH)
@@ -192,6 +199,42 @@ def test_config1_trajectories_subset_delay32():
     wl = qi.make_workload(1)
     rep = run_and_compare(wl, range(100, 124), 4, wl.delay_k, floor=True)
     _assert_report(rep)
+
+
+@pytest.mark.parametrize("k,nw,T", [(32, 24, 4), (1, 8, 2)])
+def test_config1_onepass_step_kernel(k, nw, T):
+    # the step kernel of the LARGE systems (csrc/step_onepass.cuh: the delay window read once, as a DMMA pass against eight
+    # vectors; configs[2] and [3] run it by default) forced onto configs[1], where the oracle follows every walker: the
+    # stated delay rank and rank 1 (never a pending row)
+    wl = qi.make_workload(1)
+    rep = run_and_compare(wl, range(100, 100 + nw), T, k, flags=qb.QMC_LOG_RATIOS | qb.QMC_PER_ELECTRON | qb.QMC_STEP_ONEPASS, floor=True)
+    _assert_report(rep)
+
+
+@pytest.mark.parametrize("k", [64, 128])
+def test_config1_onepass_step_kernel_large_ranks(k):
+    # delay ranks beyond the stated 32: 64, and 128 = a whole spin block of configs[1] inside ONE window (up to 127 rows
+    # pending: 16 row groups, S^-1 of order 127 built by bordering).  A delayed update of that rank is less accurate than the
+    # oracle's rank-1 updates whichever kernel does it (measured at rank 128: ratios 5.5e-10 relative with the two-pass
+    # kernel, 7.7e-10 with this one, floor 3.7e-11; at rank 64: E_L 2.1e-9 / 3.0e-9 Ha, floor 3.0e-10), so decisions are
+    # compared with the oracle and the floats are held to four times what the two-pass kernel shows.
+    wl = qi.make_workload(1)
+    fl = qb.QMC_LOG_RATIOS | qb.QMC_PER_ELECTRON
+    two = run_and_compare(wl, range(100, 108), 2, k, flags=fl, floor=True)
+    one = run_and_compare(wl, range(100, 108), 2, k, flags=fl | qb.QMC_STEP_ONEPASS, floor=True)
+    assert one["failures"] == [] and two["failures"] == []
+    for key, tol in (("ratio_rel", TOL_RATIO), ("logpsi_rel", TOL_RATIO), ("pos_abs", TOL_POS), ("ainv_rel", TOL_AINV), ("eloc_abs", TOL_ELOC)):
+        assert one["max_" + key] < max(tol, FLOOR_FACTOR * one["floor_" + key], 4 * two["max_" + key]), (key, one["max_" + key], two["max_" + key])
+
+
+def test_onepass_and_two_pass_step_kernels_agree():
+    # the same crowd through both step kernels (per-electron path): identical decisions, state to twice the tolerance
+    wl = qi.make_workload(1)
+    a = _run_gpu(wl, 0, 16, 3, 32, flags=qb.QMC_PER_ELECTRON)
+    b = _run_gpu(wl, 0, 16, 3, 32, flags=qb.QMC_PER_ELECTRON | qb.QMC_STEP_ONEPASS)
+    assert np.array_equal(a[0] & 1, b[0] & 1)
+    assert np.abs(a[1] - b[1]).max() < 2 * TOL_POS and np.abs(a[2] - b[2]).max() < 2 * TOL_ELOC
+    assert max(rel_frob(a[3][n], b[3][n]) for n in range(16)) < 2 * TOL_AINV
 
 
 def test_config1_full_crowd_sampled_walkers(oracle_farm):
@@ -522,12 +565,13 @@ def _uniform(seed, walker, step, electron):
 
 # ------------------------------------------------------------------ ragged everything
 
-@pytest.mark.parametrize("n_water,W,k,flags", [(5, 33, 7, 2), (5, 33, 7, 0), (11, 19, 13, 0)])
+@pytest.mark.parametrize("n_water,W,k,flags", [(5, 33, 7, 2), (5, 33, 7, 0), (11, 19, 13, 0), (5, 33, 7, 2 | 32), (11, 19, 13, 16 | 32)])
 def test_odd_sizes_against_oracle(n_water, W, k, flags):
     """Sizes that are multiples of nothing: 20 / 44 orbitals per spin (padded to 32 / 48), 120 / 264 basis functions (a
     partial last k-block), 33 / 19 walkers (a partial row tile), delay ranks 7 / 13 (partial windows at the end of a spin
     block).  5 waters qualify for the one-launch path (flags 0) and are also forced through the per-electron kernels
-    (flags 2 = QMC_LARGE_PATH); 11 waters (44 per spin) only run the latter."""
+    (flags 2 = QMC_LARGE_PATH); 11 waters (44 per spin) only run the latter.  | 32 = QMC_STEP_ONEPASS: the per-electron
+    kernels with the one-pass step kernel of the large systems (16 = QMC_PER_ELECTRON keeps 11 waters off the window kernel)."""
     sysm = qi.water_cluster(n_water, qi.MASTER_SEED, cfg=1)
     wl = qi.Workload(config=1, system=sysm, n_walkers=W, tau=0.01, n_sweeps=3, delay_k=k)
     rep = run_and_compare(wl, range(W), 3, k, flags=qb.QMC_LOG_RATIOS | flags)
