@@ -91,15 +91,15 @@ def stage_rooflines(sysm, W, k, acc, ms, hbm_gbs, fp64_tflops):
       + 16 mbar N_s           the window (Vbuf and Wbuf rows pending), once each
       + 24 N_e                the walker's positions (Jastrow)
       + 7 * 8 N_s acc         commit of an accepted move: five row-cache rows + two window rows written
-    `impl_bytes_per_launch` is what this implementation moves by its own count (Wbuf twice, the x column written and read
-    back, two Jastrow passes, S^-1) -- reported beside the algorithmic figure, never used for `frac`."""
+    `impl_bytes_per_launch` is what this implementation moves by its own count (the one-pass step kernel: the algorithmic
+    rows plus v_4 / a_p read a second time on accept, S^-1) -- reported beside the algorithmic figure, never used for `frac`."""
     ns, nb, ne, na = sysm.n_up, sysm.n_basis, sysm.n_elec, sysm.n_atoms
     mbar = acc * (k - 1) / 2.0
     per_walker_step = 8.0 * ns * (1 + 3 + 4) + 16.0 * mbar * ns + 24.0 * ne + 7 * 8.0 * ns * acc
-    impl_step = (8.0 * ns * (5 + 1 + 1 + acc * (5 + 2) + 1 + 3 + 1)          # V rows, x column r/w, a_p rows, row caches, new window rows
-                 + 8.0 * ns * mbar * (acc * 1 + 2)                            # Wbuf (commit), Vbuf + Wbuf (proposal)
-                 + 8.0 * mbar * mbar * (acc * 2 + 1)                          # S^-1 update and use
-                 + 2 * 24.0 * (ne + na))                                      # partner coordinates, two Jastrow passes
+    impl_step = (8.0 * ns * (4 + 1 + 1 + 3 + acc * (7 + 2))                   # V rows, a_p, a_q, gradient rows; on accept 7 rows stored, v_4 and a_p read again (L2)
+                 + 16.0 * ns * mbar                                          # Wbuf and Vbuf, once each (csrc/step_onepass.cuh)
+                 + 8.0 * mbar * mbar * (acc * 2 + 1)                          # S^-1 read, and rewritten on accept
+                 + 24.0 * (ne + na))                                          # partner coordinates, one Jastrow pass
     m = acc * k
     alg = {
         "basis": ("hbm", 8.0 * 5 * W * nb),

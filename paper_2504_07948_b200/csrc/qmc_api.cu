@@ -651,8 +651,8 @@ extern "C" int qmc_walkers_create(const qmc_system* sys, qmc_walkers** out, int 
     }
 #define CUF(call)                                                                                      \
     do {                                                                                               \
-        cudaError_t _e = (call);                                                                       \
-        if (_e != cudaSuccess) { cudaStreamSynchronize(st); cudaFree(E); cudaFree(Z); CUW(_e); }       \
+        const cudaError_t _ef = (call);   /* (not _e: CUW declares its own) */                       \
+        if (_ef != cudaSuccess) { cudaStreamSynchronize(st); cudaFree(E); cudaFree(Z); CUW(_ef); }     \
     } while (0)
     // orbital rows of every electron: basis kernel + FP64 contraction, one electron index at a time
     for (int sp = 0; sp < 2; sp++) {

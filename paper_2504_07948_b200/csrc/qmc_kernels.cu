@@ -1157,10 +1157,3 @@ cudaError_t launch_philox_words(int n, const uint32_t* in, uint32_t* out, cudaSt
 uint64_t launch_count() { return g_launches; }
 
 }  // namespace qmc
-
-#ifdef QMC_STEP_TRACE
-extern "C" int qmc_debug_step_trace(unsigned long long* out, int n) {
-    cudaDeviceSynchronize();
-    return (int)cudaMemcpyFromSymbol(out, qmc::g_step_trace, (size_t)n * 8);
-}
-#endif

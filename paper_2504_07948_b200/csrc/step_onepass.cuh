@@ -29,14 +29,6 @@
 
 namespace qmc {
 
-#ifdef QMC_STEP_TRACE
-__device__ unsigned long long g_step_trace[16 * 4096];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define S1_TRACE(i) do { if (threadIdx.x == 0 && p_prop == 40 && spin == 0) g_step_trace[(blockIdx.x & 4095) * 16 + (i)] = gtime(); } while (0)
-#else
-#define S1_TRACE(i) do { } while (0)
-#endif
-
 constexpr int S1_PT = 256;            // threads per walker
 constexpr int S1_PW = S1_PT / 32;
 constexpr int S1_NX = 8;              // vectors in shared memory, the A operand of the pass: v0 v1 v2 v3 | o1 o2 o3 | a_q
@@ -91,7 +83,6 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
     const bool has_acc = p_acc >= 0, has_prop = p_prop >= 0;
     const int e_acc = e0 + p_acc, e_prop = e0 + p_prop;
     const CtaSync sync{};
-    S1_TRACE(0);
 
     if (has_prop && warp == 1 && lane < 3) {
         // the random numbers of the proposal depend on nothing: one Philox block per lane (reading A11)
@@ -196,7 +187,6 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
         }
     };
     jastrow_sums();
-    S1_TRACE(12);
 
     // ================================================================ the vectors, and every dot product that needs no window row
     {
@@ -252,9 +242,7 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
         wbeg[tid] = b;
         wbeg[S1_PW + 1 + tid] = b / St;
     }
-    S1_TRACE(1);
     sync();   // vec, red, cs, wbeg, bc[4..7]
-    S1_TRACE(2);
 
     // ================================================================ the pass over the window: [8 vectors] x [N_s] x [8 rows] DMMA tiles
     if (m_old > 0) {
@@ -301,9 +289,7 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
         }
     }
     if (tid < 8) bc[8 + tid] = dec_scalar;
-    S1_TRACE(3);
     sync();
-    S1_TRACE(4);
     // partial tiles summed in ascending order of the orbital index: rw[i][l] = Wbuf_l . (vector i), i = 0..6;  bs[l] = Vbuf_l . a_q
     for (int idx = tid; idx < m_old * 8; idx += S1_PT) {
         const int l = idx >> 3, i = idx & 7, n = l & 7;
@@ -319,7 +305,6 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
         if (i < 7) rw[i * rld + l] = sacc; else bs[l] = sacc;
     }
     sync();
-    S1_TRACE(5);
 
     // ================================================================ a5 + a7: the decision for electron p_acc
     bool accepted = false;
@@ -380,12 +365,10 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
         }
         rho = bc[1];
     }
-    S1_TRACE(6);
     if (!accepted && !has_prop) return;
     const double sinv = 1.0 / rho;
     const int m = m_old;
 
-    S1_TRACE(7);
     // ---- one pass over the old S^-1: t_l = sum_n r_n SinvT[l][n] (bordered update) and y_n = sum_l SinvT[l][n] b_l (c' = S'^-1 b')
     double* ypart = part;   // [S1_PW][kp]
     if (m > 0) {
@@ -444,9 +427,7 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
             cn[m] = c;
             wd.cvec[(long)w * kp + m] = c;
         }
-        S1_TRACE(8);
         sync();   // cn
-        S1_TRACE(9);
 
         // ============================================================ a1 + a2 for electron p_prop (a6: the Jastrow sums above)
         if (warp == 0) {
@@ -481,7 +462,6 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
             wd.dr2p[w] = tau * (bc[4] * bc[4] + bc[5] * bc[5] + bc[6] * bc[6]);
         }
         }
-        S1_TRACE(10);
     }
     // ---- the row caches, the new window rows and the bordered S^-1, last: nothing in this launch reads them again
     if (accepted) {
@@ -513,7 +493,6 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
             wd.mcount[w] = m + 1;
         }
     }
-    S1_TRACE(11);
 }
 
 }  // namespace qmc
