@@ -368,6 +368,15 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
     if (!accepted && !has_prop) return;
     const double sinv = 1.0 / rho;
     const int m = m_old;
+    // the two rows of the commit that are not in shared memory (Laplacian row, a_p): requested now, stored at the end
+    constexpr int SR = 2;
+    double2 v4r[SR], apr[SR];
+#pragma unroll
+    for (int i = 0; i < SR; i++) {
+        const int j = tid + i * S1_PT;
+        v4r[i] = apr[i] = make_double2(0.0, 0.0);
+        if (accepted && j < n2) { v4r[i] = ldg2(v + 4 * wd.ldv + 2 * j); apr[i] = ldg2(arow_p + 2 * j); }
+    }
 
     // ---- one pass over the old S^-1: t_l = sum_n r_n SinvT[l][n] (bordered update) and y_n = sum_l SinvT[l][n] b_l (c' = S'^-1 b')
     double* ypart = part;   // [S1_PW][kp]
@@ -397,6 +406,15 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
                 }
                 tacc = warp_sum(tacc);
                 if (lane == 0) ts[l] = tacc;
+                if (accepted) {   // the bordered S^-1, row l, from the values just read: SinvT[l][n] += c_n t_l / rho, SinvT[l][m] = -t_l / rho
+                    const double tl = tacc * sinv;
+#pragma unroll
+                    for (int jj = 0; jj < 4; jj++) {
+                        const int n = lane + 32 * jj;
+                        if (n < m) Si[l * kp + n] = sv[i][jj] + cs[n] * tl;
+                    }
+                    if (lane == 0) Si[l * kp + m] = -tl;
+                }
             }
         }
 #pragma unroll
@@ -467,8 +485,12 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
     if (accepted) {
         double* orb = wd.Orb[spin] + ((long)w * nsp + p_acc) * 5 * nsp;
         const int h = ld >> 1;
-        for (int j = tid; j < n2; j += S1_PT) {
-            const double2 v4 = ldg2(v + 4 * wd.ldv + 2 * j), ap = ldg2(arow_p + 2 * j);   // (not in shared memory; L2 has them)
+        int it = 0;
+        for (int j = tid; j < n2; j += S1_PT, it++) {
+            double2 v4, ap;
+            if (it == 0) { v4 = v4r[0]; ap = apr[0]; }
+            else if (it == 1) { v4 = v4r[1]; ap = apr[1]; }
+            else { v4 = ldg2(v + 4 * wd.ldv + 2 * j); ap = ldg2(arow_p + 2 * j); }   // (longer rows: L2 has them)
             const double2* srcv = reinterpret_cast<const double2*>(vec) + j;
             const double2 v0 = srcv[0];
             reinterpret_cast<double2*>(orb)[j] = v0;
@@ -479,14 +501,7 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
             reinterpret_cast<double2*>(Vb + (long)m * nsp)[j] = v0;
             reinterpret_cast<double2*>(Wb + (long)m * nsp)[j] = ap;
         }
-        for (int l = warp; l < m; l += S1_PW) {
-            const double tl = ts[l] * sinv;
-            for (int n = lane; n < m; n += 32) Si[l * kp + n] += cs[n] * tl;
-        }
-        for (int n = tid; n < m; n += S1_PT) {
-            Si[m * kp + n] = -cs[n] * sinv;
-            Si[n * kp + m] = -ts[n] * sinv;
-        }
+        for (int n = tid; n < m; n += S1_PT) Si[m * kp + n] = -cs[n] * sinv;   // (rows 0 .. m - 1 were rewritten in the pass over S^-1)
         if (tid == 0) {
             Si[m * kp + m] = sinv;
             wd.plist[(long)w * kp + m] = p_acc;
