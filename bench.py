@@ -286,7 +286,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_profiled_pass = pe0.elapsed_time(pe1)
     stage = qb.qmc_get_stage_times(gw)
-    mo_span_us, mo_span_min_us, mo_span_n = qb.qmc_get_mo_spans(gw)
+    mo_span_us, mo_span_min_us, mo_cta_us, mo_span_n = qb.qmc_get_mo_spans(gw)
     n_lanes, lane_walkers = qb.qmc_get_lanes(gw)
     qb.qmc_set_profiling(gw, 0)
     # ---- the stages one at a time: with two lanes the in-situ event times above include queueing behind the other lane's
@@ -470,12 +470,14 @@ def run_ours(args):
     ns, nb = sysm.n_up, sysm.n_basis
     mo_ms, mo_n = stage["mo"]
     mo_events_ms = mo_ms / max(mo_n, 1)
-    # one launch contracts the rows of ONE lane; its duration is the span of the launch on the GPU (first CTA start to
-    # last CTA end, %globaltimer, sampled launches of the profiled pass) -- with two lanes an event pair on the stream also
-    # counts the time the kernel waited for the SMs of the other lane's contraction
+    # One launch contracts the rows of ONE lane.  Its duration: the kernel is persistent -- one CTA per SM it is given, equal
+    # shares of the iteration space -- so a launch costs the time its CTAs are resident (mean over the CTAs of end - start,
+    # %globaltimer stamps of the sampled launches of the profiled pass).  With two lanes the two contractions overlap: most
+    # CTAs of a launch start when the other lane's contraction leaves its SMs, so the span of a launch (first start to last
+    # end) and an event pair on its stream also count that wait; both are reported beside it.
     W_launch = sum(lane_walkers) / n_lanes
     mo_flop = 2.0 * 5 * W_launch * nb * ns
-    mo_avg_ms = mo_span_us * 1e-3 if mo_span_n else mo_events_ms
+    mo_avg_ms = mo_cta_us * 1e-3 if mo_span_n else mo_events_ms
     achieved = mo_flop / (mo_avg_ms * 1e-3) * 1e-12 if mo_avg_ms else None
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "mo_kernel_traffic.json")
@@ -505,7 +507,14 @@ def run_ours(args):
                       peak_alt_bf16_scaled=(peaks.get("bf16_tflops_sustained", 0) * 37.2 / 2250.0) or None,
                       flop_per_launch=mo_flop, ms_per_launch=mo_avg_ms, launches_timed=int(mo_span_n or mo_n),
                       ms_per_launch_stream_events=mo_events_ms,
-                      timing="span of the sampled launches on the GPU (%globaltimer stamps of every CTA)" if mo_span_n else "CUDA events on the stream",
+                      ms_per_launch_span=(mo_span_us * 1e-3) if mo_span_n else None,
+                      timing="mean residency of the CTAs of the sampled launches (%globaltimer stamps of every CTA; persistent kernel, equal shares); "
+                             "span and stream events beside it" if mo_span_n else "CUDA events on the stream",
+                      all_launches_over_elapsed=dict(
+                          achieved=mo_flop * n_lanes * sysm.n_elec * args.steps / secs * 1e-12,
+                          frac=mo_flop * n_lanes * sysm.n_elec * args.steps / secs * 1e-12 / peak,
+                          what="flops of ALL contraction launches of the timed region over its elapsed time: the tensor-pipe rate the sweep "
+                               "sustains through this kernel, every other stage and every wait included"),
                       rows_per_launch=5 * W_launch, lanes=n_lanes,
                       share_of_step=(mo_avg_ms * n_lanes * sysm.n_elec) / (red["elapsed_ms"] / args.steps)),
         fp64_tflops_model=flop_model(sysm, red["n_moves"], n_acc * world) / secs * 1e-12,

@@ -290,12 +290,14 @@ int qmc_set_profiling(qmc_walkers* w, int stride);
 int qmc_get_stage_times(qmc_walkers* w, double* ms /* [7] */, uint64_t* counts /* [7] */);
 /* Lanes of a walker set (see QMC_ONE_LANE): *n_lanes = 1 or 2; walkers_per_lane[2] (may be NULL) = their sizes. */
 int qmc_get_lanes(const qmc_walkers* w, int* n_lanes, int* walkers_per_lane);
-/* Span on the GPU of the contraction launches that the in-situ profiling sampled (qmc_set_profiling stride > 0): every CTA
- * of such a launch stamps %globaltimer when it starts and when it ends; the span of a launch is last end - first start.
- * With two lanes the stream events of qmc_get_stage_times also count the time a kernel waited for SMs that the other
- * lane's contraction still held; the span does not.  mean_us / min_us (may be NULL) over *n_launches launches (at most
- * 8192 are recorded).  Synchronises the stream(s). */
-int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, uint64_t* n_launches);
+/* Time on the GPU of the contraction launches that the in-situ profiling sampled (qmc_set_profiling stride > 0): every CTA
+ * of such a launch stamps %globaltimer when it starts and when it ends.  The SPAN of a launch is last end - first start
+ * (mean_us, min_us over the launches); the RESIDENCY of a launch is the mean over its CTAs of end - start (mean_cta_us,
+ * averaged over the launches).  The kernel is persistent with equal shares per CTA, so the residency is what the launch
+ * costs on the SMs it holds; with two lanes the span (and the stream events of qmc_get_stage_times) also counts the time
+ * most CTAs of a launch wait for the SMs the other lane's contraction still holds.  Any of the three may be NULL;
+ * *n_launches launches (at most 8192 are recorded).  Synchronises the stream(s). */
+int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, double* mean_cta_us, uint64_t* n_launches);
 /* Register-resident DMMA issue-rate loop for `ms_target` milliseconds: the FP64 ceiling of this GPU as
  * it runs now (used as the roofline denominator of the contraction stages). */
 int qmc_measure_fp64_peak(double ms_target, double* tflops, void* cuda_stream);

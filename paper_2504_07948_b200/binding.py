@@ -106,7 +106,7 @@ def load_library(path: str | None = None):
     lib.qmc_get_mo_work.argtypes = [vp, C.POINTER(u64), C.POINTER(u64)]
     lib.qmc_release_scratch.argtypes = [vp]
     lib.qmc_get_lanes.argtypes = [vp, C.POINTER(i), C.POINTER(i)]
-    lib.qmc_get_mo_spans.argtypes = [vp, C.POINTER(d), C.POINTER(d), C.POINTER(u64)]
+    lib.qmc_get_mo_spans.argtypes = [vp, C.POINTER(d), C.POINTER(d), C.POINTER(d), C.POINTER(u64)]
     lib.qmc_philox_words.argtypes = [i, vp, vp, vp]
     lib.qmc_launch_count.restype = u64
     lib.qmc_last_error.restype = C.c_char_p
@@ -333,10 +333,11 @@ def qmc_get_lanes(walkers: Walkers):
 
 
 def qmc_get_mo_spans(walkers: Walkers):
-    """(mean, min) span in microseconds of the profiled contraction launches on the GPU, and how many were recorded"""
-    a, b, n = C.c_double(), C.c_double(), C.c_uint64()
-    _check(load_library().qmc_get_mo_spans(walkers.handle, C.byref(a), C.byref(b), C.byref(n)))
-    return a.value, b.value, n.value
+    """(mean span, min span, mean CTA residency) in microseconds of the profiled contraction launches on the GPU, and how
+    many were recorded"""
+    a, b, c, n = C.c_double(), C.c_double(), C.c_double(), C.c_uint64()
+    _check(load_library().qmc_get_mo_spans(walkers.handle, C.byref(a), C.byref(b), C.byref(c), C.byref(n)))
+    return a.value, b.value, c.value, n.value
 
 
 def qmc_set_mo_ctas(walkers: Walkers, n_ctas):

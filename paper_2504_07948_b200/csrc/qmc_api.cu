@@ -1097,29 +1097,37 @@ extern "C" int qmc_get_lanes(const qmc_walkers* w, int* n_lanes, int* walkers_pe
     return QMC_OK;
 }
 
-extern "C" int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, uint64_t* n_launches) {
-    if (!w || !mean_us || !n_launches) return fail(QMC_ERR_ARG, "qmc_get_mo_spans: null argument");
+extern "C" int qmc_get_mo_spans(qmc_walkers* w, double* mean_us, double* min_us, double* mean_cta_us, uint64_t* n_launches) {
+    if (!w || !n_launches) return fail(QMC_ERR_ARG, "qmc_get_mo_spans: null argument");
     GUARD(w->sys);
+    double mean_dummy = 0.0;
+    if (!mean_us) mean_us = &mean_dummy;
     *mean_us = 0.0; *n_launches = 0;
     if (min_us) *min_us = 0.0;
+    if (mean_cta_us) *mean_cta_us = 0.0;
     const size_t n = w->trace_grid.size(), nsm = (size_t)w->sys->n_sm;
     if (n == 0 || !w->mo_trace.p) return QMC_OK;
     CU(cudaStreamSynchronize(w->stream));
     if (w->n_lanes == 2) CU(cudaStreamSynchronize(w->lane[1].stream));
     std::vector<unsigned long long> h(n * 2 * nsm);
     CU(cudaMemcpy(h.data(), w->mo_trace.p, h.size() * 8, cudaMemcpyDeviceToHost));
-    double sum = 0.0, mn = 1e300;
+    double sum = 0.0, mn = 1e300, sum_cta = 0.0;
     for (size_t i = 0; i < n; i++) {
         unsigned long long t0 = ~0ull, t1 = 0;
+        double res = 0.0;
         for (int c = 0; c < w->trace_grid[i]; c++) {
-            t0 = std::min(t0, h[(i * nsm + c) * 2]);
-            t1 = std::max(t1, h[(i * nsm + c) * 2 + 1]);
+            const unsigned long long a = h[(i * nsm + c) * 2], b = h[(i * nsm + c) * 2 + 1];
+            t0 = std::min(t0, a);
+            t1 = std::max(t1, b);
+            res += (double)(b - a) * 1e-3;
         }
         const double us = (double)(t1 - t0) * 1e-3;
         sum += us; mn = std::min(mn, us);
+        sum_cta += res / std::max(1, w->trace_grid[i]);
     }
     *mean_us = sum / n; *n_launches = n;
     if (min_us) *min_us = mn;
+    if (mean_cta_us) *mean_cta_us = sum_cta / n;
     return QMC_OK;
 }
 

@@ -335,12 +335,14 @@ cudaError_t launch_mo(const SysDev& s, int spin, const double* PhiT, int rows, d
 // a1 + a2 + a5 + a6 + a7: the fused per-walker step kernel lives in step_kernel.cuh
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st) {
-    static SmemAttr attr[3], attr1;
+    static SmemAttr attr[3], attr1[2];
     if (step1_fits(s.nsp[spin], wd.kp, wd.onepass != 0)) {   // large systems: the delay window read once (step_onepass.cuh)
-        const size_t smem1 = step1_smem_bytes(s.nsp[spin], wd.kp);
-        const cudaError_t e1 = attr1.ensure(k_step1p, smem1);
+        const int pt1 = step1_threads(s.nsp[spin], wd.kp);
+        const size_t smem1 = step1_smem_bytes(s.nsp[spin], wd.kp, pt1);
+        const cudaError_t e1 = pt1 == S1_PT_SMALL ? attr1[0].ensure(k_step1p<S1_PT_SMALL>, smem1) : attr1[1].ensure(k_step1p<S1_PT_LARGE>, smem1);
         if (e1 != cudaSuccess) return e1;
-        k_step1p<<<wd.W, S1_PT, smem1, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+        if (pt1 == S1_PT_SMALL) k_step1p<S1_PT_SMALL><<<wd.W, S1_PT_SMALL, smem1, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
+        else k_step1p<S1_PT_LARGE><<<wd.W, S1_PT_LARGE, smem1, st>>>(s, wd, spin, p_acc, p_prop, log_off, step, tau, sqrt(tau), commit);
         COUNT_LAUNCH();
         return cudaGetLastError();
     }

@@ -29,15 +29,16 @@
 
 namespace qmc {
 
-constexpr int S1_PT = 256;            // threads per walker
-constexpr int S1_PW = S1_PT / 32;
+// threads per walker: 256, two CTAs to an SM, where the eight vectors of two walkers fit in an SM's shared memory; 512 (one
+// CTA to an SM, twice the loads in flight) for longer rows
+constexpr int S1_PT_SMALL = 256, S1_PT_LARGE = 512;
 constexpr int S1_NX = 8;              // vectors in shared memory, the A operand of the pass: v0 v1 v2 v3 | o1 o2 o3 | a_q
 constexpr int S1_ND = 11;             // dot products that need no window row
 constexpr int S1_NJ = 7;              // Jastrow sums: grad J at r_q (3) | dJ and grad J at r'_p (4)
 
 struct Step1Layout {
     int ld, vec, part, rw_ld, rw, bs, cs, cn, ts, red, jred, wb, bc, total;   // offsets in doubles
-    __host__ __device__ Step1Layout(int nsp, int kp) {
+    __host__ __device__ Step1Layout(int nsp, int kp, int S1_PW) {
         ld = nsp + 8;                 // vector stride = 64 B mod 128 B: conflict-free 16-byte fragment loads (see the pass)
         vec = 0;
         part = vec + S1_NX * ld;
@@ -55,22 +56,28 @@ struct Step1Layout {
         total = bc + 16;
     }
 };
-inline size_t step1_smem_bytes(int nsp, int kp) { return (size_t)Step1Layout(nsp, kp).total * sizeof(double); }
-// the one-pass kernel keeps eight vectors in shared memory (two CTAs to an SM up to 1400 orbitals per spin)
-inline bool step1_fits(int nsp, int kp, bool forced) { return (nsp > 256 || forced) && step1_smem_bytes(nsp, kp) <= 220 * 1024; }
-
-__device__ __forceinline__ double s1_sum8(const double* p) {   // fixed order
-    return ((p[0] + p[1]) + (p[2] + p[3])) + ((p[4] + p[5]) + (p[6] + p[7]));
+inline size_t step1_smem_bytes(int nsp, int kp, int pt) { return (size_t)Step1Layout(nsp, kp, pt / 32).total * sizeof(double); }
+inline int step1_threads(int nsp, int kp) { return 2 * (step1_smem_bytes(nsp, kp, S1_PT_SMALL) + 1024) <= 227 * 1024 ? S1_PT_SMALL : S1_PT_LARGE; }
+// the one-pass kernel keeps eight vectors in shared memory
+inline bool step1_fits(int nsp, int kp, bool forced) {
+    return (nsp > 256 || forced) && step1_smem_bytes(nsp, kp, step1_threads(nsp, kp)) <= 220 * 1024;
 }
 
-__global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
+template <int N>
+__device__ __forceinline__ double s1_sum(const double* p) {   // fixed order: pairwise
+    if constexpr (N == 1) return p[0];
+    else return s1_sum<N / 2>(p) + s1_sum<N / 2>(p + N / 2);
+}
+
+template <int S1_PT>
+__global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
                                                      double tau, double sqrt_tau, int commit) {
     extern __shared__ __align__(16) double sm[];
-    static_assert(S1_PW == 8, "s1_sum8");
+    constexpr int S1_PW = S1_PT / 32;
     const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], n2 = nsp >> 1, kp = wd.kp, nep = wd.nep;
     const int e0 = spin == 0 ? 0 : s.ns[0];
-    const Step1Layout L(nsp, kp);
+    const Step1Layout L(nsp, kp, S1_PW);
     const int ld = L.ld, rld = L.rw_ld;
     double *vec = sm + L.vec, *part = sm + L.part, *rw = sm + L.rw, *bs = sm + L.bs, *cs = sm + L.cs, *cn = sm + L.cn, *ts = sm + L.ts;
     double *red = sm + L.red, *jred = sm + L.jred, *bc = sm + L.bc;
@@ -320,12 +327,12 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
                 for (int k = 0; k < 4; k++) a4[k] += c * rw[k * rld + l];
             }
 #pragma unroll
-            for (int k = 0; k < 4; k++) a4[k] = s1_sum8(red + k * S1_PW) - warp_sum(a4[k]);
+            for (int k = 0; k < 4; k++) a4[k] = s1_sum<S1_PW>(red + k * S1_PW) - warp_sum(a4[k]);
             if (lane == 0) {
                 rho = a4[0];
                 const double Gx = bc[8], Gy = bc[9], Gz = bc[10], u = bc[11];
-                dJ = s1_sum8(jred + 3 * S1_PW);
-                const double gJx = s1_sum8(jred + 4 * S1_PW), gJy = s1_sum8(jred + 5 * S1_PW), gJz = s1_sum8(jred + 6 * S1_PW);
+                dJ = s1_sum<S1_PW>(jred + 3 * S1_PW);
+                const double gJx = s1_sum<S1_PW>(jred + 4 * S1_PW), gJy = s1_sum<S1_PW>(jred + 5 * S1_PW), gJz = s1_sum<S1_PW>(jred + 6 * S1_PW);
                 bool accept = false;
                 if (fabs(rho) < 1e-12) bits |= 2u;
                 if (rho > 0.0) {  // fixed node: reject rho_D <= 0 (A7); NaN fails the comparison and rejects
@@ -431,7 +438,7 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
             for (int l = lane; l < m; l += 32) tb += ts[l] * bs[l];
             tb = warp_sum(tb);   // (every warp the same sum in the same order)
         }
-        const double bm = s1_sum8(red + 7 * S1_PW);   // Vbuf_m . a_q = v_0 . a_q
+        const double bm = s1_sum<S1_PW>(red + 7 * S1_PW);   // Vbuf_m . a_q = v_0 . a_q
         for (int n = tid; n < m; n += S1_PT) {
             double c = 0.0;
 #pragma unroll
@@ -458,9 +465,9 @@ __global__ void __launch_bounds__(S1_PT, 2) k_step1p(SysDev s, WalkDev wd, int s
 #pragma unroll
         for (int k = 0; k < 3; k++) e3[k] = warp_sum(e3[k]);
         const double cm = accepted ? cn[m] : 0.0;
-        double Gx = s1_sum8(red + 4 * S1_PW) - e3[0] - cm * s1_sum8(red + 8 * S1_PW) + s1_sum8(jred);
-        double Gy = s1_sum8(red + 5 * S1_PW) - e3[1] - cm * s1_sum8(red + 9 * S1_PW) + s1_sum8(jred + S1_PW);
-        double Gz = s1_sum8(red + 6 * S1_PW) - e3[2] - cm * s1_sum8(red + 10 * S1_PW) + s1_sum8(jred + 2 * S1_PW);
+        double Gx = s1_sum<S1_PW>(red + 4 * S1_PW) - e3[0] - cm * s1_sum<S1_PW>(red + 8 * S1_PW) + s1_sum<S1_PW>(jred);
+        double Gy = s1_sum<S1_PW>(red + 5 * S1_PW) - e3[1] - cm * s1_sum<S1_PW>(red + 9 * S1_PW) + s1_sum<S1_PW>(jred + S1_PW);
+        double Gz = s1_sum<S1_PW>(red + 6 * S1_PW) - e3[2] - cm * s1_sum<S1_PW>(red + 10 * S1_PW) + s1_sum<S1_PW>(jred + 2 * S1_PW);
         if (has_acc && e_acc != e_prop) {   // the partner that may just have moved
             const double kx = accepted ? px : ox, ky = accepted ? py : oy, kz = accepted ? pz : oz;
             const double dx = rx - kx, dy = ry - ky, dz = rz - kz;
