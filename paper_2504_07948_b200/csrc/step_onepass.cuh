@@ -63,6 +63,31 @@ inline bool step1_fits(int nsp, int kp, bool forced) {
     return (nsp > 256 || forced) && step1_smem_bytes(nsp, kp, step1_threads(nsp, kp)) <= 220 * 1024;
 }
 
+// 1 / sqrt(x) and 1 / x for the Jastrow sums, branch-free: an FP32 seed (MUFU, 2^-22) and two Newton steps in FP64 (error
+// 2^-44, then below the rounding of the steps themselves: about 1 ulp).  The library routines carry a slow path behind a
+// branch for arguments outside the FP32 exponent range -- never met here: squared distances in bohr^2 and (1 + b r)^3 --
+// and that branch keeps the compiler from interleaving the chains of the partners a thread works on (measured: the sums
+// of a launch 11 us with the library calls, each thread 11 partners one after the other).
+__device__ __forceinline__ double s1_rsqrt(double x) {
+    float y0;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"((float)x));
+    double y = (double)y0;
+    const double h = 0.5 * x;
+    y = y * fma(-(h * y), y, 1.5);
+    y = y * fma(-(h * y), y, 1.5);
+    return y;
+}
+__device__ __forceinline__ double s1_rcp(double x) {
+    float y0;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"((float)x));
+    double y = (double)y0;
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    return y;
+}
+
 template <int N>
 __device__ __forceinline__ double s1_sum(const double* p) {   // fixed order: pairwise
     if constexpr (N == 1) return p[0];
@@ -168,19 +193,19 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
                 if (has_prop && k != e_prop && !(has_acc && k == e_acc)) {   // (electron e_acc may still move: its term follows the decision)
                     const double dx = rx - kx[i], dy = ry - ky[i], dz = rz - kz[i];
                     const double d2 = dx * dx + dy * dy + dz * dz;
-                    const double ir = rsqrt(d2);
+                    const double ir = s1_rsqrt(d2);
                     const double q = 1.0 + b * (d2 * ir);
-                    const double wgt = a * ir * __drcp_rn(q * q);
+                    const double wgt = a * ir * s1_rcp(q * q);
                     jg[0] += wgt * dx; jg[1] += wgt * dy; jg[2] += wgt * dz;
                 }
                 if (has_acc && k != e_acc) {
                     const double dx = ox - kx[i], dy = oy - ky[i], dz = oz - kz[i];
                     const double ex = px - kx[i], ey = py - ky[i], ez = pz - kz[i];
                     const double d2o = dx * dx + dy * dy + dz * dz, d2n = ex * ex + ey * ey + ez * ez;
-                    const double iro = rsqrt(d2o), irn = rsqrt(d2n);
+                    const double iro = s1_rsqrt(d2o), irn = s1_rsqrt(d2n);
                     const double r_old = d2o > 0.0 ? d2o * iro : 0.0, r_new = d2n > 0.0 ? d2n * irn : 0.0;
                     const double qo = 1.0 + b * r_old, qn = 1.0 + b * r_new;
-                    const double t = a * __drcp_rn(qn * qn * qo);
+                    const double t = a * s1_rcp(qn * qn * qo);
                     jg[3] += (r_new - r_old) * (t * qn);
                     const double wgt = t * qo * irn;
                     jg[4] += wgt * ex; jg[5] += wgt * ey; jg[6] += wgt * ez;
@@ -472,9 +497,9 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
             const double kx = accepted ? px : ox, ky = accepted ? py : oy, kz = accepted ? pz : oz;
             const double dx = rx - kx, dy = ry - ky, dz = rz - kz;
             const double d2 = dx * dx + dy * dy + dz * dz;
-            const double ir = rsqrt(d2);
+            const double ir = s1_rsqrt(d2);
             const double q = 1.0 + s.b_ee * (d2 * ir);
-            const double wgt = s.a_para * ir * __drcp_rn(q * q);
+            const double wgt = s.a_para * ir * s1_rcp(q * q);
             Gx += wgt * dx; Gy += wgt * dy; Gz += wgt * dz;
         }
         limit_drift(Gx, Gy, Gz, wd.lim_a, tau);
