@@ -94,12 +94,16 @@ __device__ __forceinline__ double s1_sum(const double* p) {   // fixed order: pa
     else return s1_sum<N / 2>(p) + s1_sum<N / 2>(p + N / 2);
 }
 
-template <int S1_PT>
-__global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
-                                                     double tau, double sqrt_tau, int commit) {
-    extern __shared__ __align__(16) double sm[];
+// The body works on walker w with the S1_PT threads tid = 0 .. S1_PT - 1 that `sync` joins, in their shared memory `sm`
+// (Step1Layout(nsp, kp, S1_PT / 32).total doubles): a whole CTA (k_step1p) or a 128-thread group of the window kernel of the
+// mid-size path.  COH: V and the window rows may have been written earlier in the SAME launch (window kernel): they are
+// read through L2 (ld.global.cg), not through the non-coherent read-only path.  Every branch that leaves the body is uniform
+// over those threads.
+template <int S1_PT, bool COH, class Sync>
+__device__ __forceinline__ void step1_body(const SysDev& s, const WalkDev& wd, const int w, const int tid, double* sm, const Sync& sync, int spin,
+                                           int p_acc, int p_prop, long log_off, uint32_t step, double tau, double sqrt_tau, int commit) {
     constexpr int S1_PW = S1_PT / 32;
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = tid & 31, warp = tid >> 5;
     const int nsp = s.nsp[spin], n2 = nsp >> 1, kp = wd.kp, nep = wd.nep;
     const int e0 = spin == 0 ? 0 : s.ns[0];
     const Step1Layout L(nsp, kp, S1_PW);
@@ -114,7 +118,6 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
     const int m_old = wd.mcount[w];
     const bool has_acc = p_acc >= 0, has_prop = p_prop >= 0;
     const int e_acc = e0 + p_acc, e_prop = e0 + p_prop;
-    const CtaSync sync{};
 
     if (has_prop && warp == 1 && lane < 3) {
         // the random numbers of the proposal depend on nothing: one Philox block per lane (reading A11)
@@ -231,7 +234,7 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
             const double2 z = make_double2(0.0, 0.0);
             double2 v0 = z, v1 = z, v2 = z, v3 = z, ap = z, aq = z, o1 = z, o2 = z, o3 = z;
             if (has_acc) {
-                v0 = ldg2(v + 2 * j); v1 = ldg2(v + wd.ldv + 2 * j); v2 = ldg2(v + 2 * wd.ldv + 2 * j); v3 = ldg2(v + 3 * wd.ldv + 2 * j);
+                v0 = ld2<COH>(v + 2 * j); v1 = ld2<COH>(v + wd.ldv + 2 * j); v2 = ld2<COH>(v + 2 * wd.ldv + 2 * j); v3 = ld2<COH>(v + 3 * wd.ldv + 2 * j);
                 ap = ldg2(arow_p + 2 * j);
             }
             if (has_prop) {
@@ -300,8 +303,8 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
 #pragma unroll
                 for (int q = 0; q < UN; q++) {
                     const bool on = st + q < s1;   // (past the range: zeros -- the DMMAs add nothing)
-                    b[q][0] = on ? ldg2(src + 16 * (st + q)) : make_double2(0.0, 0.0);
-                    b[q][1] = on ? ldg2(src + 16 * (st + q) + 8) : make_double2(0.0, 0.0);
+                    b[q][0] = on ? ld2<COH>(src + 16 * (st + q)) : make_double2(0.0, 0.0);
+                    b[q][1] = on ? ld2<COH>(src + 16 * (st + q) + 8) : make_double2(0.0, 0.0);
                 }
 #pragma unroll
                 for (int q = 0; q < UN; q++) {
@@ -407,7 +410,7 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
     for (int i = 0; i < SR; i++) {
         const int j = tid + i * S1_PT;
         v4r[i] = apr[i] = make_double2(0.0, 0.0);
-        if (accepted && j < n2) { v4r[i] = ldg2(v + 4 * wd.ldv + 2 * j); apr[i] = ldg2(arow_p + 2 * j); }
+        if (accepted && j < n2) { v4r[i] = ld2<COH>(v + 4 * wd.ldv + 2 * j); apr[i] = ldg2(arow_p + 2 * j); }
     }
 
     // ---- one pass over the old S^-1: t_l = sum_n r_n SinvT[l][n] (bordered update) and y_n = sum_l SinvT[l][n] b_l (c' = S'^-1 b')
@@ -522,7 +525,7 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
             double2 v4, ap;
             if (it == 0) { v4 = v4r[0]; ap = apr[0]; }
             else if (it == 1) { v4 = v4r[1]; ap = apr[1]; }
-            else { v4 = ldg2(v + 4 * wd.ldv + 2 * j); ap = ldg2(arow_p + 2 * j); }   // (longer rows: L2 has them)
+            else { v4 = ld2<COH>(v + 4 * wd.ldv + 2 * j); ap = ldg2(arow_p + 2 * j); }   // (longer rows: L2 has them)
             const double2* srcv = reinterpret_cast<const double2*>(vec) + j;
             const double2 v0 = srcv[0];
             reinterpret_cast<double2*>(orb)[j] = v0;
@@ -540,6 +543,15 @@ __global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(
             wd.mcount[w] = m + 1;
         }
     }
+}
+
+// p_acc >= 0: finish the move of electron p_acc of this spin (needs its MO rows in V);  p_prop >= 0: propose the move of
+// electron p_prop.  commit == 0 evaluates the decision but changes no state (stage timing only).
+template <int S1_PT>
+__global__ void __launch_bounds__(S1_PT, S1_PT == S1_PT_SMALL ? 2 : 1) k_step1p(SysDev s, WalkDev wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step,
+                                                                                double tau, double sqrt_tau, int commit) {
+    extern __shared__ __align__(16) double sm[];
+    step1_body<S1_PT, false>(s, wd, blockIdx.x, threadIdx.x, sm, CtaSync{}, spin, p_acc, p_prop, log_off, step, tau, sqrt_tau, commit);
 }
 
 }  // namespace qmc
