@@ -82,3 +82,26 @@ def test_crowds_argument_errors():
     qb.qmc_set_mo_ctas(a, 0)
     qb.qmc_sweep_crowds([a], 1, wl.tau, 1)
     assert qb.qmc_get_stats(a)["proposed"] == 4 * wl.system.n_elec
+
+
+def test_stage_timers_and_contraction_residency_do_not_change_the_run():
+    # the in-situ timers (qmc_set_profiling) bracket every n-th electron's launches with events and make the CTAs of the
+    # sampled contractions stamp %globaltimer: the trajectory must not notice, every timed contraction has its stamps, and
+    # a launch's mean CTA residency can never exceed its span (first CTA start to last CTA end)
+    wl = qi.make_workload(1)
+    g = qb.qmc_init_from(wl.system)
+    runs = []
+    for stride in (0, 4):
+        gw = qb.qmc_walkers_create(g, wl.positions(0, 12), wl.seed, flags=qb.QMC_PER_ELECTRON)
+        qb.qmc_set_profiling(gw, stride)
+        qb.qmc_sweep(gw, 2, wl.tau, 16)
+        runs.append(_state(gw))
+        if stride:
+            st = qb.qmc_get_stage_times(gw)
+            span, span_min, residency, n = qb.qmc_get_mo_spans(gw)
+            assert n == st["mo"][1] > 0
+            assert st["mo"][0] > 0 and st["step"][1] > 0 and st["flush"][1] > 0
+            assert 0 < residency <= span and 0 < span_min <= span
+            assert qb.qmc_get_lanes(gw)[0] == 1
+    for a, b in zip(*runs):
+        assert np.array_equal(a, b)
