@@ -1,6 +1,6 @@
 // step_onepass.cuh -- the per-walker part of one electron step for LARGE systems (rows of the inverse longer than 256):
 // rows a5 + a7 of electron p fused with rows a1 + a2 + a6 of electron q = p + 1, as step_kernel.cuh, but with the delay
-// window read ONCE and the Jastrow sums under that read.                      [BASELINE.json north_star items 3, 4]
+// window read ONCE.                                                           [BASELINE.json north_star items 3, 4]
 //
 // step_kernel.cuh forms the effective column of the delayed inverse explicitly, x = a_q - Wbuf^T c, which costs a second
 // pass over Wbuf, a round trip of x through HBM, and a chain of phases each exposing a memory latency; its two Jastrow
@@ -16,9 +16,9 @@
 // [N_s] x [2 m rows]: FP64 DMMA m8n8k4 with the vectors as the A operand (shared memory, conflict-free by the row stride)
 // and eight window rows as the B operand, loaded straight from HBM in fragment order (four lanes cover 64 contiguous
 // bytes of a row).  The Jastrow sums -- the ratio and gradient at r'_p of the move being decided, the gradient at r_q for
-// the drift of the next one -- depend on positions only: they are evaluated while the loads of the vectors are in flight,
-// four partners at a time per thread (independent chains: the sums are bound by the latency of rsqrt / reciprocal, not by
-// the FP64 pipe).  Bytes per walker: 10 rows + 2 m rows + 7 rows stored on accept = SURVEY 8(d).3's count for a1 + a5 + a6 + a7.
+// the drift of the next one -- depend on positions only: they come first, all partner coordinates of a thread requested
+// at once (twelve partners per thread in flight), while the rows of the vectors are prefetched into L2.  Bytes per
+// walker: 10 rows + 2 m rows + 7 rows stored on accept = SURVEY 8(d).3's count for a1 + a5 + a6 + a7.
 //
 // State between launches: c of the pending proposal (cvec), its position r', drift G, uniform u.  (The two-pass kernel
 // also keeps x, dJ and grad J(r'); this one recomputes the Jastrow terms of the pending proposal in the launch that
@@ -141,7 +141,7 @@ __device__ __forceinline__ void step1_body(const SysDev& s, const WalkDev& wd, c
     // ================================================================ the Jastrow sums (reading A5), while the rows below come up from HBM
     // With q = 1 + b r:  grad u = a / (q^2 r) (r_i - r_k);  u(r') - u(r) = a (r' - r) / (q' q), term by term (reading "new").
     // r = d^2 rsqrt(d^2), and ONE reciprocal t = 1 / (q'^2 q) serves the ratio and the gradient at r': 1 / (q' q) = t q',
-    // 1 / (q'^2 r') = t q / r'.  Four partners per thread at a time: four independent chains.
+    // 1 / (q'^2 r') = t q / r'.  All loads of a round of twelve partners per thread first, then their chains.
     {
         const int nline = nsp >> 4;   // 128-byte lines of a row
         for (int i = tid; i < 9 * nline; i += S1_PT) {
