@@ -841,7 +841,7 @@ static int sweep_electron(qmc_walkers* w, Lane& L, const SweepCall& c, int t, in
         CU(launch_step(s, d, sp, p, -1, log_off, w->step, c.tau, 1, st));
         prof_end(w, st, pf);
         prof_begin(w, st, 4, pf);
-        CU(launch_flush(s, d, sp, st));
+        CU(launch_flush(s, d, sp, st, c.delay_k));
         prof_end(w, st, pf);
         *in_window = 0;
     } else {  // accept/reject of p and proposal of p + 1 in one launch
@@ -885,7 +885,7 @@ static int sweep_windows(qmc_walkers* w, const SweepCall& c) {
                 CU(launch_window(s, L.d, sp, p0, n, log_base, w->d.W, w->step, c.tau, st));
                 prof_end(w, st, pf);
                 prof_begin(w, st, 4, pf);
-                CU(launch_flush(s, L.d, sp, st));
+                CU(launch_flush(s, L.d, sp, st, c.delay_k));
                 prof_end(w, st, pf);
             }
         int rc = sweep_finish_step(w, c);

@@ -413,9 +413,86 @@ cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st) {
+// Flush of a SHORT window (at most FLUSH_SMALL_M moves pending: delay_k <= 4) in one kernel that reads A^-T once.  Row q of
+// the updated inverse needs row q of the old one only -- YT[q][:] = delta - AinvT0[q][:] . Vbuf^T, then AinvT[q][:] += YT[q][:] W2
+// -- and for a short window Vbuf and W2 = SinvT Wbuf (m rows each) fit in shared memory: a warp reads its row, forms the m dot
+// products, reads the row again (L1) and writes it back updated.  The three GEMMs read A^-T twice and write it once, and a
+// rank-1 "GEMM" is a matrix-vector product on tensor-core tiles that are fifteen-sixteenths padding; at delay_k = 1..4 the flush
+// is bound by HBM, so this is the whole difference (configs[4] at 256 walkers: k = 1 148 k -> 200 k moves/s, the flush at 5.7 TB/s;
+// k = 4 323 k -> 351 k).  With eight rows the shared-memory reads of the 2 m vectors per row cost more than the second read of
+// A^-T (k = 8: 316 k against 398 k with the GEMMs).  Grid (row chunks, walkers).
+constexpr int FLUSH_SMALL_M = 4, FLUSH_SMALL_ROWS = 64;
+inline size_t flush_small_smem(int nsp, int m_cap) { return ((size_t)2 * m_cap * nsp + (size_t)m_cap * m_cap + m_cap + 2) * sizeof(double); }
+__global__ void __launch_bounds__(256) k_flush_small(WalkDev wd, double* __restrict__ Ainv, int nsp, int m_cap) {
+    extern __shared__ __align__(16) double fsm[];
+    const int w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int m = wd.mcount[w], kp = wd.kp, n2 = nsp >> 1;
+    if (m == 0) return;
+    double* Vs = fsm;
+    double* W2s = Vs + (size_t)m_cap * nsp;
+    double* Ss = W2s + (size_t)m_cap * nsp;
+    int* pl = reinterpret_cast<int*>(Ss + m_cap * m_cap);
+    const double* Vb = wd.Vbuf + (long)w * kp * nsp;
+    const double* Wb = wd.Wbuf + (long)w * kp * nsp;
+    for (int i = tid; i < m * n2; i += 256) reinterpret_cast<double2*>(Vs)[i] = __ldg(reinterpret_cast<const double2*>(Vb) + i);   // rows 0 .. m-1 are contiguous
+    for (int i = tid; i < m * m; i += 256) Ss[i] = wd.SinvT[(long)w * kp * kp + (i / m) * kp + (i % m)];
+    if (tid < m) pl[tid] = wd.plist[(long)w * kp + tid];
+    __syncthreads();
+    for (int j2 = tid; j2 < n2; j2 += 256) {   // W2[l][j] = sum_n SinvT[l][n] Wbuf[n][j]
+        double2 wv[FLUSH_SMALL_M];
+#pragma unroll
+        for (int n = 0; n < FLUSH_SMALL_M; n++) wv[n] = n < m ? __ldg(reinterpret_cast<const double2*>(Wb + (long)n * nsp) + j2) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int l = 0; l < FLUSH_SMALL_M; l++) {
+            if (l >= m) break;
+            double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int n = 0; n < FLUSH_SMALL_M; n++)
+                if (n < m) { const double c = Ss[l * m + n]; acc.x += c * wv[n].x; acc.y += c * wv[n].y; }
+            reinterpret_cast<double2*>(W2s + (size_t)l * nsp)[j2] = acc;
+        }
+    }
+    __syncthreads();
+    const int q0 = blockIdx.x * FLUSH_SMALL_ROWS;
+    const int q1 = q0 + FLUSH_SMALL_ROWS < nsp ? q0 + FLUSH_SMALL_ROWS : nsp;
+    for (int q = q0 + warp; q < q1; q += 8) {
+        double2* row = reinterpret_cast<double2*>(Ainv + ((long)w * nsp + q) * nsp);
+        double y[FLUSH_SMALL_M];
+#pragma unroll
+        for (int n = 0; n < FLUSH_SMALL_M; n++) y[n] = 0.0;
+        for (int j2 = lane; j2 < n2; j2 += 32) {
+            const double2 a = row[j2];
+#pragma unroll
+            for (int n = 0; n < FLUSH_SMALL_M; n++)
+                if (n < m) { const double2 v = reinterpret_cast<const double2*>(Vs + (size_t)n * nsp)[j2]; y[n] += a.x * v.x + a.y * v.y; }
+        }
+#pragma unroll
+        for (int n = 0; n < FLUSH_SMALL_M; n++)
+            if (n < m) y[n] = (pl[n] == q ? 1.0 : 0.0) - warp_sum(y[n]);
+        for (int j2 = lane; j2 < n2; j2 += 32) {
+            double2 a = row[j2];   // (L1: this warp has just read the row)
+#pragma unroll
+            for (int l = 0; l < FLUSH_SMALL_M; l++)
+                if (l < m) { const double2 u = reinterpret_cast<const double2*>(W2s + (size_t)l * nsp)[j2]; a.x += y[l] * u.x; a.y += y[l] * u.y; }
+            row[j2] = a;
+        }
+    }
+}
+
+cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st, int max_m) {
     const int nsp = s.nsp[spin], kp = wd.kp;
     cudaError_t e;
+    if (max_m >= 1 && max_m <= FLUSH_SMALL_M && flush_small_smem(nsp, max_m) <= 200 * 1024) {
+        static SmemAttr attr;
+        const size_t smem = flush_small_smem(nsp, max_m);
+        e = attr.ensure(k_flush_small, smem);
+        if (e != cudaSuccess) return e;
+        k_flush_small<<<dim3((nsp + FLUSH_SMALL_ROWS - 1) / FLUSH_SMALL_ROWS, wd.W), 256, smem, st>>>(wd, wd.AinvT[spin], nsp, max_m);
+        COUNT_LAUNCH();
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        return launch_window_reset(wd, st);
+    }
     GemmArgs g;
     // YT = AinvT0 * Vbuf^T
     g.A = wd.AinvT[spin]; g.lda = nsp; g.strideA = (long)nsp * nsp;

@@ -18,7 +18,7 @@ cudaError_t launch_export_phi(const double* PhiT, long n_rows, int width, int kb
 // p_acc >= 0: ratio + accept/reject + commit of electron p_acc (spin-local index); p_prop >= 0: proposal of p_prop
 cudaError_t launch_step(const SysDev& s, const WalkDev& wd, int spin, int p_acc, int p_prop, long log_off, uint32_t step, double tau,
                         int commit, cudaStream_t st);
-cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st);
+cudaError_t launch_flush(const SysDev& s, const WalkDev& wd, int spin, cudaStream_t st, int max_m = 1 << 30);   // max_m: the most moves that can be pending (delay_k): short windows flush in one kernel
 cudaError_t launch_window_reset(const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_eloc(const SysDev& s, const WalkDev& wd, cudaStream_t st);
 cudaError_t launch_gather_rp(const WalkDev& wd, int e, cudaStream_t st);
