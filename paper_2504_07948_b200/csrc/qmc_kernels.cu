@@ -428,6 +428,10 @@ __global__ void __launch_bounds__(256) k_flush_small(WalkDev wd, double* __restr
     const int w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int m = wd.mcount[w], kp = wd.kp, n2 = nsp >> 1;
     if (m == 0) return;
+    if (m > m_cap || m > FLUSH_SMALL_M) {   // (never: the scheduler passes delay_k; raise the walker's sticky flag rather than overrun shared memory)
+        if (tid == 0) wd.flags[w] = 1u;
+        return;
+    }
     double* Vs = fsm;
     double* W2s = Vs + (size_t)m_cap * nsp;
     double* Ss = W2s + (size_t)m_cap * nsp;
